@@ -1,0 +1,148 @@
+"""CPU fp64 oracle for Sparse Reference Attention (SRA).   *** TEST INFRASTRUCTURE ***
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this.  It shares no code with the CUDA path and never imports the
+product package.
+
+What it computes ("Generation tokens attend to all reference tokens ...
+while reference tokens only self-attend"; :119 structured sparsity, near-linear in
+reference length; :223 cached reference K/V concatenated with fresh generation K/V;
+:561 restatement).  The paper gives no equation; the mask below is SURVEY.md section 8c's
+reading (A1-A5, listed in DESIGN.md):
+
+    rows/cols ordered [G ; R], n = N_g + N_r, block(t) = k with off[k] <= t < off[k+1]
+    M[i][j] = 1  if i in G                                  (any j in G u R)
+    M[i][j] = 1  if i in R, j in R and block(i) == block(j)
+    M[i][j] = 0  otherwise  (R->G masked; R->other R blocks masked)
+    S = s * Q K^T;  P = softmax over {j : M[i][j]=1} of S;  O = P V;  LSE = max + log(sum)
+    backward (standard softmax-attention calculus, paper silent):
+    D = rowsum(dO o O); dV = P^T dO; dP = dO V^T; dS = P o (dP - D); dQ = s dS K; dK = s dS^T Q
+
+SRA is exact attention under a fixed mask, so the oracle is that definition written
+out: the mask is materialised as an explicit n x n byte matrix, every quantity is
+fp64, nothing is tiled, fused or reordered.  Inputs are bf16 bit patterns (uint16),
+upcast exactly to fp64.
+
+Pins: tests/test_oracle_pins.py (brute force, closed forms, invariants, library
+cross-checks, finite differences).  No function here is "parity unpinned".
+"""
+from __future__ import annotations
+
+import numpy as np
+
+
+def bf16_bits_to_f64(bits: np.ndarray) -> np.ndarray:
+    """Exact upcast of bf16 bit patterns (uint16) to float64."""
+    bits = np.ascontiguousarray(bits, dtype=np.uint16)
+    return (bits.astype(np.uint32) << np.uint32(16)).view(np.float32).astype(np.float64)
+
+
+def block_of(t: int, offsets) -> int:
+    """block(t) = k with off[k] <= t < off[k+1]."""
+    for k in range(len(offsets) - 1):
+        if offsets[k] <= t < offsets[k + 1]:
+            return k
+    raise ValueError(f"token {t} outside reference blocks {offsets}")
+
+
+def sra_mask(n_gen: int, ref_block_offsets) -> np.ndarray:
+    """The explicit SRA mask M, uint8 [n, n] with n = n_gen + n_ref, rows/cols [G ; R]."""
+    off = [int(x) for x in ref_block_offsets] if len(ref_block_offsets) else [0]
+    n_ref = off[-1]
+    n = n_gen + n_ref
+    M = np.zeros((n, n), dtype=np.uint8)
+    for i in range(n):
+        if i < n_gen:  # i in G: sees everything
+            M[i, :] = 1
+        else:  # i in R: sees only its own block of R
+            bi = block_of(i - n_gen, off)
+            for j in range(n_gen, n):
+                if block_of(j - n_gen, off) == bi:
+                    M[i, j] = 1
+    return M
+
+
+def masked_attention(Q, K, V, M, scale):
+    """softmax(scale Q K^T restricted to M) V for one head, fp64.  Returns O, LSE, P."""
+    S = scale * (Q @ K.T)
+    vis = M.astype(bool)
+    Sm = np.where(vis, S, -np.inf)
+    mx = Sm.max(axis=1, keepdims=True)
+    E = np.where(vis, np.exp(Sm - mx), 0.0)
+    Z = E.sum(axis=1, keepdims=True)
+    P = E / Z
+    O = P @ V
+    LSE = (mx + np.log(Z))[:, 0]
+    return O, LSE, P
+
+
+def _concat_head(x_gen, x_ref, b, h):
+    parts = [x_gen[b, :, h, :]]
+    if x_ref is not None and x_ref.shape[1] > 0:
+        parts.append(x_ref[b, :, h, :])
+    return np.concatenate(parts, axis=0)
+
+
+def sra_forward(q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, ref_block_offsets, scale):
+    """SRA forward on bf16-bit inputs [B, N, H, d].
+
+    Returns dict(o_gen, o_ref, lse_gen, lse_ref): O fp64 [B,N,H,d], LSE fp64 [B,H,N].
+    q_ref may be None (cached denoising step: R rows skipped).
+    """
+    f = bf16_bits_to_f64
+    qg, kg, vg = f(q_gen), f(k_gen), f(v_gen)
+    kr, vr = f(k_ref), f(v_ref)
+    B, Ng, H, d = qg.shape
+    Nr = kr.shape[1]
+    have_qr = q_ref is not None
+    qr = f(q_ref) if have_qr else np.zeros((B, Nr, H, d))
+    M = sra_mask(Ng, ref_block_offsets)
+    o = np.zeros((B, Ng + Nr, H, d))
+    lse = np.zeros((B, H, Ng + Nr))
+    for b in range(B):
+        for h in range(H):
+            Q = _concat_head(qg, qr, b, h)
+            K = _concat_head(kg, kr, b, h)
+            V = _concat_head(vg, vr, b, h)
+            O, L, _ = masked_attention(Q, K, V, M, scale)
+            o[b, :, h, :] = O
+            lse[b, h, :] = L
+    out = {"o_gen": o[:, :Ng], "lse_gen": lse[:, :, :Ng]}
+    if have_qr:
+        out["o_ref"] = o[:, Ng:]
+        out["lse_ref"] = lse[:, :, Ng:]
+    return out
+
+
+def sra_backward(q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, do_gen, do_ref, ref_block_offsets, scale):
+    """SRA backward on bf16-bit inputs.  Returns dq/dk/dv for G and R, fp64 [B,N,H,d]."""
+    f = bf16_bits_to_f64
+    qg, kg, vg, qr, kr, vr = f(q_gen), f(k_gen), f(v_gen), f(q_ref), f(k_ref), f(v_ref)
+    dog, dor = f(do_gen), f(do_ref)
+    B, Ng, H, d = qg.shape
+    Nr = kr.shape[1]
+    M = sra_mask(Ng, ref_block_offsets)
+    dq = np.zeros((B, Ng + Nr, H, d))
+    dk = np.zeros_like(dq)
+    dv = np.zeros_like(dq)
+    for b in range(B):
+        for h in range(H):
+            Q = _concat_head(qg, qr, b, h)
+            K = _concat_head(kg, kr, b, h)
+            V = _concat_head(vg, vr, b, h)
+            dO = _concat_head(dog, dor, b, h)
+            O, _, P = masked_attention(Q, K, V, M, scale)
+            D = (dO * O).sum(axis=1, keepdims=True)
+            dV = P.T @ dO
+            dP = dO @ V.T
+            dS = P * (dP - D)
+            dq[b, :, h, :] = scale * (dS @ K)
+            dk[b, :, h, :] = scale * (dS.T @ Q)
+            dv[b, :, h, :] = dV
+    return {"dq_gen": dq[:, :Ng], "dk_gen": dk[:, :Ng], "dv_gen": dv[:, :Ng],
+            "dq_ref": dq[:, Ng:], "dk_ref": dk[:, Ng:], "dv_ref": dv[:, Ng:]}
+
+
+def count_pairs(n_gen: int, ref_block_offsets) -> int:
+    """Number of unmasked (query,key) pairs per (batch, head), counted from the explicit mask."""
+    return int(sra_mask(n_gen, ref_block_offsets).sum(dtype=np.int64))

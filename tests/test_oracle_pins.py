@@ -1,0 +1,428 @@
+"""Pins for the CPU fp64 oracle (oracle/sra_oracle.py and oracle/sra_oracle.c).
+
+The paper prints NO worked numeric example of Sparse Reference Attention,
+no equation and no mask figure, so the oracle is pinned to what the
+mathematics fixes instead: closed forms, invariants named by BASELINE.json north_star,
+special cases that reduce to a library routine (torch CPU fp64 SDPA / autograd), a
+pure-Python brute force on tiny inputs and central finite differences for the backward.
+Each check is chosen so that a plausible mistake (dropped term, wrong sign/index,
+transposed operand, wrong block lookup) fails at least one of them.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import c_oracle, sra_oracle
+from tests.util import bits_to_f64, rand_bits, to_bf16_bits
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _problem(rng, B=1, H=2, d=8, Ng=5, blocks=(3, 1, 4), scale_q=1.0):
+    Nr = sum(blocks)
+    off = np.concatenate([[0], np.cumsum(blocks)]).astype(np.int32)
+    t = {}
+    for name, n in (("q_gen", Ng), ("k_gen", Ng), ("v_gen", Ng), ("q_ref", Nr), ("k_ref", Nr), ("v_ref", Nr),
+                    ("do_gen", Ng), ("do_ref", Nr)):
+        s = scale_q if name[0] in "qk" else 1.0
+        t[name] = rand_bits(rng, (B, n, H, d), s)
+    return t, off, 1.0 / math.sqrt(d)
+
+
+def _fwd(t, off, s, with_qref=True):
+    return sra_oracle.sra_forward(t["q_gen"], t["k_gen"], t["v_gen"], t["q_ref"] if with_qref else None,
+                                  t["k_ref"], t["v_ref"], off, s)
+
+
+# ----------------------------------------------------------------------------- upcast
+def test_bf16_upcast_exact():
+    bits = np.arange(0, 65536, dtype=np.uint32).astype(np.uint16)
+    finite = np.isfinite(bits_to_f64(bits))
+    a = sra_oracle.bf16_bits_to_f64(bits)[finite]
+    b = bits_to_f64(bits)[finite]
+    assert np.array_equal(a, b)
+
+
+# ----------------------------------------------------------------------------- mask
+def _closed_form_pairs(Ng, blocks):
+    return Ng * (Ng + sum(blocks)) + sum(b * b for b in blocks)
+
+
+def test_mask_density_golden():
+    """pairs = N_g (N_g + N_r) + sum_j b_j^2 ; values in tests/golden/pairs.txt."""
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "pairs.txt")) if l.strip() and not l.startswith("#")]
+    for name, Ng, nblk, bsz, pairs, total in rows:
+        Ng, nblk, bsz, total = int(Ng), int(nblk), int(bsz), int(total)
+        got = _closed_form_pairs(Ng, [bsz] * nblk)
+        if pairs.startswith("~"):
+            assert abs(got - float(pairs[1:])) <= 5e-4 * float(pairs[1:]), name
+        else:
+            assert got == int(pairs), name
+        assert (Ng + nblk * bsz) ** 2 == total, name
+    # the explicit mask (python and C) on the Tiny config: 262,144 of 589,824
+    off = [0, 128, 256, 384, 512]
+    assert sra_oracle.count_pairs(256, off) == 262144
+    assert c_oracle.count_pairs(256, off) == 262144
+    M = sra_oracle.sra_mask(256, off)
+    assert M.shape == (768, 768) and M.size == 589824
+
+
+@pytest.mark.parametrize("Ng,blocks", [(5, (3, 1, 4)), (1, (2,)), (7, ()), (3, (1, 1, 1)), (4, (5, 2))])
+def test_mask_structure(Ng, blocks):
+    off = np.concatenate([[0], np.cumsum(blocks)]).astype(int) if blocks else np.array([0])
+    M = sra_oracle.sra_mask(Ng, off)
+    n = Ng + sum(blocks)
+    assert M.shape == (n, n)
+    assert int(M.sum()) == _closed_form_pairs(Ng, blocks) == c_oracle.count_pairs(Ng, off)
+    assert M[:Ng].all()  # G rows see everything
+    assert not M[Ng:, :Ng].any()  # R -> G always masked
+    R = M[Ng:, Ng:]
+    assert np.array_equal(R, R.T)  # block-diagonal is symmetric
+    # independent construction: block id per token, equality matrix
+    bid = np.repeat(np.arange(len(blocks)), blocks)
+    assert np.array_equal(R.astype(bool), bid[:, None] == bid[None, :])
+
+
+def test_group_indicator_mass():
+    """V[j] = e_{g(j)} (g=0 for G, 1+block for R) => O[i][g] = probability mass on group g."""
+    rng = np.random.default_rng(1)
+    blocks = (3, 2, 4)
+    t, off, s = _problem(rng, H=1, d=8, Ng=6, blocks=blocks)
+    n_groups = 1 + len(blocks)
+    assert n_groups <= 8
+    vg = np.zeros((1, 6, 1, 8)); vg[..., 0] = 1.0
+    vr = np.zeros((1, 9, 1, 8))
+    bid = np.repeat(np.arange(len(blocks)), blocks)
+    for j, g in enumerate(bid):
+        vr[0, j, 0, 1 + g] = 1.0
+    t["v_gen"], t["v_ref"] = to_bf16_bits(vg), to_bf16_bits(vr)
+    out = _fwd(t, off, s)
+    og, orf = out["o_gen"][0, :, 0], out["o_ref"][0, :, 0]
+    assert np.allclose(og[:, :n_groups].sum(axis=1), 1.0, atol=1e-14)
+    assert (og[:, :n_groups] > 0).all()  # G rows put mass on every group
+    for i, g in enumerate(bid):  # R rows: exactly 1 on own group, exactly 0 elsewhere
+        expect = np.zeros(8); expect[1 + g] = 1.0
+        assert np.allclose(orf[i], expect, atol=1e-15), (i, orf[i])
+        assert orf[i][0] == 0.0 and all(orf[i][1 + k] == 0.0 for k in range(len(blocks)) if k != g)
+    # same through the C oracle
+    rows = np.arange(15, dtype=np.int32)
+    oc, _ = c_oracle.forward_rows(t["q_gen"], t["k_gen"], t["v_gen"], t["q_ref"], t["k_ref"], t["v_ref"], off, s, rows)
+    assert np.allclose(oc[0, :6, 0], og, atol=1e-14) and np.allclose(oc[0, 6:, 0], orf, atol=1e-14)
+
+
+# ----------------------------------------------------------------------------- softmax closed forms
+def test_constant_v_and_row_sums():
+    rng = np.random.default_rng(2)
+    t, off, s = _problem(rng, B=2, H=2, d=8, Ng=5, blocks=(3, 1, 4), scale_q=3.0)
+    for const in (1.0, -2.5):
+        t["v_gen"] = to_bf16_bits(np.full((2, 5, 2, 8), const))
+        t["v_ref"] = to_bf16_bits(np.full((2, 8, 2, 8), const))
+        out = _fwd(t, off, s)
+        assert np.allclose(out["o_gen"], const, atol=1e-14) and np.allclose(out["o_ref"], const, atol=1e-14)
+
+
+def test_zero_q_gives_means():
+    """Q = 0 => uniform softmax: O_g = mean of all V rows; O_r[block j] = mean of block j's V rows;
+    LSE = log(number of visible keys)."""
+    rng = np.random.default_rng(3)
+    blocks = (3, 1, 4)
+    t, off, s = _problem(rng, B=1, H=2, d=8, Ng=5, blocks=blocks)
+    t["q_gen"] = np.zeros_like(t["q_gen"]); t["q_ref"] = np.zeros_like(t["q_ref"])
+    out = _fwd(t, off, s)
+    vg, vr = bits_to_f64(t["v_gen"]), bits_to_f64(t["v_ref"])
+    mean_all = np.concatenate([vg, vr], axis=1).mean(axis=1)  # [B,H,d]
+    assert np.allclose(out["o_gen"], mean_all[:, None], atol=1e-15)
+    assert np.allclose(out["lse_gen"], math.log(5 + 8), atol=1e-15)
+    for j, b in enumerate(blocks):
+        lo, hi = off[j], off[j + 1]
+        assert np.allclose(out["o_ref"][:, lo:hi], vr[:, lo:hi].mean(axis=1)[:, None], atol=1e-15)
+        assert np.allclose(out["lse_ref"][:, :, lo:hi], math.log(b), atol=1e-15)
+    rows = np.arange(13, dtype=np.int32)
+    oc, lc = c_oracle.forward_rows(t["q_gen"], t["k_gen"], t["v_gen"], t["q_ref"], t["k_ref"], t["v_ref"], off, s, rows)
+    assert np.allclose(oc[:, :5], out["o_gen"], atol=1e-15) and np.allclose(oc[:, 5:], out["o_ref"], atol=1e-15)
+    assert np.allclose(lc[:, :, :5], out["lse_gen"], atol=1e-15)
+
+
+# ----------------------------------------------------------------------------- library cross-checks
+def _sdpa(Q, K, V, s):
+    """torch CPU fp64 SDPA (library routine) for one head: Q [n,d], K/V [m,d]."""
+    q, k, v = (torch.as_tensor(x)[None, None] for x in (Q, K, V))
+    return torch.nn.functional.scaled_dot_product_attention(q, k, v, scale=s)[0, 0].numpy()
+
+
+def test_g_rows_equal_dense_attention_and_lse_merge():
+    rng = np.random.default_rng(4)
+    t, off, s = _problem(rng, B=2, H=2, d=16, Ng=7, blocks=(3, 5, 2), scale_q=2.0)
+    out = _fwd(t, off, s)
+    f = bits_to_f64
+    for b in range(2):
+        for h in range(2):
+            Q = f(t["q_gen"])[b, :, h]
+            Kg, Vg, Kr, Vr = (f(t[k])[b, :, h] for k in ("k_gen", "v_gen", "k_ref", "v_ref"))
+            ref = _sdpa(Q, np.concatenate([Kg, Kr]), np.concatenate([Vg, Vr]), s)
+            assert np.allclose(out["o_gen"][b, :, h], ref, atol=1e-13)
+            # LSE-merge identity: Attn(Q,[Kg;Kr]) = merge of Attn(Q,Kg,Vg) and Attn(Q,Kr,Vr) by LSE weights
+            Sg, Sr = s * Q @ Kg.T, s * Q @ Kr.T
+            lg = np.log(np.exp(Sg).sum(1)); lr = np.log(np.exp(Sr).sum(1))
+            og, orr = _sdpa(Q, Kg, Vg, s), _sdpa(Q, Kr, Vr, s)
+            lse = np.logaddexp(lg, lr)
+            merged = np.exp(lg - lse)[:, None] * og + np.exp(lr - lse)[:, None] * orr
+            assert np.allclose(out["o_gen"][b, :, h], merged, atol=1e-13)
+            assert np.allclose(out["lse_gen"][b, h], lse, atol=1e-13)
+
+
+def test_r_rows_equal_blockwise_dense_attention():
+    rng = np.random.default_rng(5)
+    blocks = (3, 5, 1, 2)
+    t, off, s = _problem(rng, B=1, H=2, d=16, Ng=4, blocks=blocks, scale_q=2.0)
+    out = _fwd(t, off, s)
+    f = bits_to_f64
+    for h in range(2):
+        for j in range(len(blocks)):
+            lo, hi = off[j], off[j + 1]
+            ref = _sdpa(f(t["q_ref"])[0, lo:hi, h], f(t["k_ref"])[0, lo:hi, h], f(t["v_ref"])[0, lo:hi, h], s)
+            assert np.allclose(out["o_ref"][0, lo:hi, h], ref, atol=1e-13)
+    # n_ref_blocks = 1 => plain self-attention over R
+    out1 = _fwd(t, np.array([0, sum(blocks)]), s)
+    for h in range(2):
+        ref = _sdpa(f(t["q_ref"])[0, :, h], f(t["k_ref"])[0, :, h], f(t["v_ref"])[0, :, h], s)
+        assert np.allclose(out1["o_ref"][0, :, h], ref, atol=1e-13)
+
+
+def test_zero_ref_is_plain_self_attention_and_single_gen_token():
+    rng = np.random.default_rng(6)
+    t, off, s = _problem(rng, B=1, H=2, d=16, Ng=9, blocks=())
+    out = _fwd(t, off, s)
+    f = bits_to_f64
+    for h in range(2):
+        ref = _sdpa(f(t["q_gen"])[0, :, h], f(t["k_gen"])[0, :, h], f(t["v_gen"])[0, :, h], s)
+        assert np.allclose(out["o_gen"][0, :, h], ref, atol=1e-13)
+    assert out["o_ref"].shape[1] == 0
+    t, off, s = _problem(rng, B=1, H=1, d=8, Ng=1, blocks=(2, 3))
+    out = _fwd(t, off, s)
+    K = np.concatenate([f(t["k_gen"])[0, :, 0], f(t["k_ref"])[0, :, 0]])
+    V = np.concatenate([f(t["v_gen"])[0, :, 0], f(t["v_ref"])[0, :, 0]])
+    assert np.allclose(out["o_gen"][0, :, 0], _sdpa(f(t["q_gen"])[0, :, 0], K, V, s), atol=1e-13)
+
+
+def test_cached_step_skips_ref_rows():
+    rng = np.random.default_rng(7)
+    t, off, s = _problem(rng)
+    a, b = _fwd(t, off, s, True), _fwd(t, off, s, False)
+    assert "o_ref" not in b and np.array_equal(a["o_gen"], b["o_gen"])
+
+
+# ----------------------------------------------------------------------------- symmetries
+def test_permutation_symmetries():
+    rng = np.random.default_rng(8)
+    blocks = (3, 4, 2)
+    t, off, s = _problem(rng, B=1, H=2, d=8, Ng=5, blocks=blocks, scale_q=2.0)
+    base = _fwd(t, off, s)
+    # (a) O_g invariant under ANY joint permutation of (K_r, V_r) rows, even across blocks
+    perm = rng.permutation(9)
+    t2 = dict(t); t2["k_ref"] = t["k_ref"][:, perm]; t2["v_ref"] = t["v_ref"][:, perm]
+    assert np.allclose(_fwd(t2, off, s)["o_gen"], base["o_gen"], atol=1e-14)
+    # (b) O_r equivariant under within-block permutations
+    perm = np.concatenate([off[j] + rng.permutation(b) for j, b in enumerate(blocks)])
+    t3 = dict(t)
+    for k in ("q_ref", "k_ref", "v_ref"):
+        t3[k] = t[k][:, perm]
+    o3 = _fwd(t3, off, s)
+    assert np.allclose(o3["o_ref"], base["o_ref"][:, perm], atol=1e-14)
+    assert np.allclose(o3["o_gen"], base["o_gen"], atol=1e-14)
+    # (c) reordering whole blocks: blocks (0,1,2) -> (2,0,1)
+    order = [2, 0, 1]
+    idx = np.concatenate([np.arange(off[j], off[j + 1]) for j in order])
+    off4 = np.concatenate([[0], np.cumsum([blocks[j] for j in order])])
+    t4 = dict(t)
+    for k in ("q_ref", "k_ref", "v_ref"):
+        t4[k] = t[k][:, idx]
+    o4 = _fwd(t4, off4, s)
+    assert np.allclose(o4["o_ref"], base["o_ref"][:, idx], atol=1e-14)
+    assert np.allclose(o4["o_gen"], base["o_gen"], atol=1e-14)
+
+
+# ----------------------------------------------------------------------------- brute force
+def _brute_force(t, off, s):
+    """Pure-Python per-element brute force (independent of numpy matmul / the oracle's structure)."""
+    f = bits_to_f64
+    qg, kg, vg, qr, kr, vr = (f(t[k]) for k in ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref"))
+    B, Ng, H, d = qg.shape
+    Nr = kr.shape[1]
+    bid = [next(k for k in range(len(off) - 1) if off[k] <= j < off[k + 1]) for j in range(Nr)]
+    O = np.zeros((B, Ng + Nr, H, d)); L = np.zeros((B, H, Ng + Nr))
+    for b in range(B):
+        for h in range(H):
+            for i in range(Ng + Nr):
+                q = qg[b, i, h] if i < Ng else qr[b, i - Ng, h]
+                keys = []
+                if i < Ng:
+                    keys += [(kg[b, j, h], vg[b, j, h]) for j in range(Ng)]
+                    keys += [(kr[b, j, h], vr[b, j, h]) for j in range(Nr)]
+                else:
+                    keys += [(kr[b, j, h], vr[b, j, h]) for j in range(Nr) if bid[j] == bid[i - Ng]]
+                sc = [s * sum(float(q[c]) * float(k[c]) for c in range(d)) for k, _ in keys]
+                mx = max(sc)
+                w = [math.exp(x - mx) for x in sc]
+                z = sum(w)
+                for c in range(d):
+                    O[b, i, h, c] = sum(wi * float(v[c]) for wi, (_, v) in zip(w, keys)) / z
+                L[b, h, i] = mx + math.log(z)
+    return O, L
+
+
+@pytest.mark.parametrize("seed,Ng,blocks,d", [(10, 4, (3, 1, 2), 4), (11, 1, (1,), 3), (12, 6, (2, 5), 8), (13, 3, (), 4)])
+def test_brute_force_tiny(seed, Ng, blocks, d):
+    rng = np.random.default_rng(seed)
+    t, off, s = _problem(rng, B=2, H=2, d=d, Ng=Ng, blocks=blocks, scale_q=2.0)
+    O, L = _brute_force(t, off, s)
+    out = _fwd(t, off, s)
+    assert np.allclose(out["o_gen"], O[:, :Ng], atol=1e-13) and np.allclose(out["lse_gen"], L[:, :, :Ng], atol=1e-13)
+    if blocks:
+        assert np.allclose(out["o_ref"], O[:, Ng:], atol=1e-13) and np.allclose(out["lse_ref"], L[:, :, Ng:], atol=1e-13)
+    n = Ng + sum(blocks)
+    oc, lc = c_oracle.forward_rows(t["q_gen"], t["k_gen"], t["v_gen"], t["q_ref"], t["k_ref"], t["v_ref"], off, s,
+                                   np.arange(n, dtype=np.int32))
+    assert np.allclose(oc, O, atol=1e-13) and np.allclose(lc, L, atol=1e-13)
+
+
+def test_numpy_vs_where_softmax_one_liner():
+    """The 4-line numpy `where(M, S, -inf)` softmax of SURVEY.md section 8c on the Tiny shape (1 head)."""
+    rng = np.random.default_rng(14)
+    t, off, s = _problem(rng, B=1, H=1, d=64, Ng=256, blocks=(128,) * 4, scale_q=1.0)
+    out = _fwd(t, off, s)
+    f = bits_to_f64
+    Q = np.concatenate([f(t["q_gen"])[0, :, 0], f(t["q_ref"])[0, :, 0]])
+    K = np.concatenate([f(t["k_gen"])[0, :, 0], f(t["k_ref"])[0, :, 0]])
+    V = np.concatenate([f(t["v_gen"])[0, :, 0], f(t["v_ref"])[0, :, 0]])
+    bid = np.concatenate([np.full(256, -1), np.repeat(np.arange(4), 128)])
+    M = (bid[:, None] == -1) | ((bid[:, None] == bid[None, :]) & (bid[None, :] >= 0))
+    S = np.where(M, s * Q @ K.T, -np.inf)
+    P = np.exp(S - S.max(1, keepdims=True)); P /= P.sum(1, keepdims=True)
+    O = P @ V
+    assert np.allclose(np.concatenate([out["o_gen"][0, :, 0], out["o_ref"][0, :, 0]]), O, atol=1e-13)
+    # C oracle: sampled rows + one full head agree with the numpy oracle
+    rows = np.array([0, 255, 256, 383, 384, 767], dtype=np.int32)
+    oc, _ = c_oracle.forward_rows(t["q_gen"], t["k_gen"], t["v_gen"], t["q_ref"], t["k_ref"], t["v_ref"], off, s, rows)
+    assert np.allclose(oc[0, :, 0], O[rows], atol=1e-13)
+    oh, lh = c_oracle.forward_head(t["q_gen"], t["k_gen"], t["v_gen"], t["q_ref"], t["k_ref"], t["v_ref"], off, s, 0, 0)
+    assert np.allclose(oh, O, atol=1e-13)
+    assert np.allclose(lh, np.log(np.exp(S - S.max(1, keepdims=True)).sum(1)) + S.max(1), atol=1e-12)
+
+
+# ----------------------------------------------------------------------------- backward
+def _bwd(t, off, s):
+    return sra_oracle.sra_backward(t["q_gen"], t["k_gen"], t["v_gen"], t["q_ref"], t["k_ref"], t["v_ref"],
+                                   t["do_gen"], t["do_ref"], off, s)
+
+
+def _loss(t, off, s):
+    """Scalar loss sum(dO o O) of the fp64 forward, as a function of fp64 inputs given directly."""
+    out = _fwd(t, off, s)
+    f = bits_to_f64
+    return float((f(t["do_gen"]) * out["o_gen"]).sum() + (f(t["do_ref"]) * out["o_ref"]).sum())
+
+
+def test_backward_torch_autograd():
+    """dQ/dK/dV equal torch fp64 autograd through an independently built masked attention."""
+    rng = np.random.default_rng(20)
+    blocks = (3, 1, 4)
+    t, off, s = _problem(rng, B=2, H=2, d=8, Ng=5, blocks=blocks, scale_q=2.0)
+    g = _bwd(t, off, s)
+    f = lambda k: torch.tensor(bits_to_f64(t[k]), requires_grad=True)
+    qg, kg, vg, qr, kr, vr = (f(k) for k in ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref"))
+    dog, dor = torch.tensor(bits_to_f64(t["do_gen"])), torch.tensor(bits_to_f64(t["do_ref"]))
+    bid = torch.tensor(np.repeat(np.arange(len(blocks)), blocks))
+    K = torch.cat([kg, kr], 1); V = torch.cat([vg, vr], 1)
+    Sg = s * torch.einsum("bihc,bjhc->bhij", qg, K)
+    Og = torch.einsum("bhij,bjhc->bihc", torch.softmax(Sg, -1), V)
+    Sr = s * torch.einsum("bihc,bjhc->bhij", qr, kr)
+    Sr = Sr.masked_fill(bid[:, None] != bid[None, :], float("-inf"))
+    Or = torch.einsum("bhij,bjhc->bihc", torch.softmax(Sr, -1), vr)
+    ((Og * dog).sum() + (Or * dor).sum()).backward()
+    for name, leaf in (("dq_gen", qg), ("dk_gen", kg), ("dv_gen", vg), ("dq_ref", qr), ("dk_ref", kr), ("dv_ref", vr)):
+        assert np.allclose(g[name], leaf.grad.numpy(), atol=1e-12), name
+    # C oracle backward (all rows / cols of each head) against the same autograd result
+    for b in range(2):
+        for h in range(2):
+            o, lse = c_oracle.forward_head(t["q_gen"], t["k_gen"], t["v_gen"], t["q_ref"], t["k_ref"], t["v_ref"], off, s, b, h)
+            dq, dk, dv = c_oracle.backward_head(t["q_gen"], t["k_gen"], t["v_gen"], t["q_ref"], t["k_ref"], t["v_ref"],
+                                                t["do_gen"], t["do_ref"], off, s, b, h, o, lse)
+            assert np.allclose(dq[:5], qg.grad.numpy()[b, :, h], atol=1e-12)
+            assert np.allclose(dq[5:], qr.grad.numpy()[b, :, h], atol=1e-12)
+            assert np.allclose(dk[:5], kg.grad.numpy()[b, :, h], atol=1e-12)
+            assert np.allclose(dk[5:], kr.grad.numpy()[b, :, h], atol=1e-12)
+            assert np.allclose(dv[:5], vg.grad.numpy()[b, :, h], atol=1e-12)
+            assert np.allclose(dv[5:], vr.grad.numpy()[b, :, h], atol=1e-12)
+            # subset of rows / cols is exact
+            rows = np.array([1, 6, 12], dtype=np.int32); cols = np.array([0, 5, 11], dtype=np.int32)
+            dq2, dk2, dv2 = c_oracle.backward_head(t["q_gen"], t["k_gen"], t["v_gen"], t["q_ref"], t["k_ref"], t["v_ref"],
+                                                   t["do_gen"], t["do_ref"], off, s, b, h, o, lse, rows, cols)
+            assert np.array_equal(dq2, dq[rows]) and np.array_equal(dk2, dk[cols]) and np.array_equal(dv2, dv[cols])
+
+
+def test_backward_finite_differences():
+    """Central differences of the fp64 forward loss sum(dO o O) w.r.t. bf16-representable perturbations.
+
+    Inputs are bf16 bit patterns, so the perturbation is applied on a private fp64 path:
+    masked_attention() is called directly with fp64 operands (eps = 1e-6)."""
+    rng = np.random.default_rng(21)
+    blocks = (2, 3)
+    Ng, Nr, d = 3, 5, 4
+    t, off, s = _problem(rng, B=1, H=1, d=d, Ng=Ng, blocks=blocks, scale_q=1.5)
+    g = _bwd(t, off, s)
+    f = bits_to_f64
+    Q = np.concatenate([f(t["q_gen"])[0, :, 0], f(t["q_ref"])[0, :, 0]])
+    K = np.concatenate([f(t["k_gen"])[0, :, 0], f(t["k_ref"])[0, :, 0]])
+    V = np.concatenate([f(t["v_gen"])[0, :, 0], f(t["v_ref"])[0, :, 0]])
+    dO = np.concatenate([f(t["do_gen"])[0, :, 0], f(t["do_ref"])[0, :, 0]])
+    M = sra_oracle.sra_mask(Ng, off)
+
+    def loss(Q, K, V):
+        O, _, _ = sra_oracle.masked_attention(Q, K, V, M, s)
+        return float((dO * O).sum())
+
+    eps = 1e-6
+    for X, names in ((Q, ("dq_gen", "dq_ref")), (K, ("dk_gen", "dk_ref")), (V, ("dv_gen", "dv_ref"))):
+        G = np.concatenate([g[names[0]][0, :, 0], g[names[1]][0, :, 0]])
+        for i in range(Ng + Nr):
+            for c in range(d):
+                Xp, Xm = X.copy(), X.copy()
+                Xp[i, c] += eps; Xm[i, c] -= eps
+                args_p = [Xp if Y is X else Y for Y in (Q, K, V)]
+                args_m = [Xm if Y is X else Y for Y in (Q, K, V)]
+                fd = (loss(*args_p) - loss(*args_m)) / (2 * eps)
+                assert abs(fd - G[i, c]) <= 1e-6 * max(1.0, abs(G[i, c])), (names, i, c, fd, G[i, c])
+
+
+def test_backward_invariants():
+    rng = np.random.default_rng(22)
+    blocks = (3, 2, 4)
+    t, off, s = _problem(rng, B=1, H=2, d=8, Ng=5, blocks=blocks, scale_q=2.0)
+    g = _bwd(t, off, s)
+    f = bits_to_f64
+    # sum_j dV_j = sum_i dO_i (rows of P sum to 1), over all G and R rows/cols
+    lhs = g["dv_gen"].sum(axis=1) + g["dv_ref"].sum(axis=1)
+    rhs = f(t["do_gen"]).sum(axis=1) + f(t["do_ref"]).sum(axis=1)
+    assert np.allclose(lhs, rhs, atol=1e-12)
+    # sum_j dS_ij = 0 per row  <=>  sum_j dS_ij K_j with K = const gives dQ = 0
+    t1 = dict(t)
+    t1["k_gen"] = to_bf16_bits(np.full((1, 5, 2, 8), 0.5)); t1["k_ref"] = to_bf16_bits(np.full((1, 9, 2, 8), 0.5))
+    g1 = _bwd(t1, off, s)
+    assert np.abs(g1["dq_gen"]).max() < 1e-14 and np.abs(g1["dq_ref"]).max() < 1e-14
+    # dK_g, dV_g independent of dO_r (R rows never see G keys)
+    t2 = dict(t); t2["do_ref"] = rand_bits(rng, t["do_ref"].shape, 100.0)
+    g2 = _bwd(t2, off, s)
+    assert np.array_equal(g2["dk_gen"], g["dk_gen"]) and np.array_equal(g2["dv_gen"], g["dv_gen"])
+    assert np.array_equal(g2["dq_gen"], g["dq_gen"])
+    # dK_r, dV_r of block j depend only on dO_g and dO_r[j]: perturb dO_r of block 1 only
+    t3 = dict(t); d3 = t["do_ref"].copy(); d3[:, off[1]:off[2]] = rand_bits(rng, d3[:, off[1]:off[2]].shape, 10.0)
+    t3["do_ref"] = d3
+    g3 = _bwd(t3, off, s)
+    for j in (0, 2):
+        sl = slice(off[j], off[j + 1])
+        assert np.array_equal(g3["dk_ref"][:, sl], g["dk_ref"][:, sl]) and np.array_equal(g3["dv_ref"][:, sl], g["dv_ref"][:, sl])
+    assert not np.allclose(g3["dk_ref"][:, off[1]:off[2]], g["dk_ref"][:, off[1]:off[2]])
