@@ -1,0 +1,145 @@
+/* sra.h - C ABI of the B200-native Sparse Reference Attention (SRA) library.
+ *
+ * SRA is the asymmetric self-attention of the VideoRef DiT of arxiv/paper_2606_13872:
+ *   "Generation tokens attend to all reference tokens ... while reference tokens only
+ *    self-attend"                                              (section 1)
+ *   structured sparsity, cost ~linear in reference length      (section 2.1)
+ *   reference K/V "computed once at the first denoising step and cached in GPU memory",
+ *   then concatenated with fresh generation K/V                (section 4.3)
+ *   references enter SFT training through SRA => backward      (section 3.3)
+ * The paper prints no equation; the mask reading:
+ *   rows/cols ordered [G ; R];  G row i sees every key of G u R;
+ *   R row i sees key j  iff  j in R and block(i) == block(j)  (blocks = contiguous ranges
+ *   given by ref_block_offsets, one block = one latent frame in the paper-shaped configs).
+ *   O = softmax(scale * Q K^T restricted to visible keys) V,  LSE = log sum exp (natural log).
+ *
+ * Conventions
+ *   - extern "C", plain pointers + sizes, no torch types.  Every function returns an int
+ *     status (0 = SRA_OK, <0 = error) and never throws / aborts.
+ *   - "device" pointers are CUDA device pointers on the ctx's device; "host" pointers are
+ *     ordinary host memory.  The caller owns every tensor; the library owns only sra_ctx
+ *     (resident reference-KV cache, tile schedule, fp32 backward workspace).
+ *   - Tensor layout: bf16, [batch, tokens, heads, head_dim], head_dim contiguous,
+ *     16-byte aligned base pointers.  LSE: fp32 [batch, heads, tokens].
+ *   - Calls are asynchronous on `cuda_stream` (a cudaStream_t passed as void*; NULL = legacy
+ *     default stream).  Argument / launch errors are returned synchronously; execution
+ *     faults surface at the caller's next synchronisation.
+ *   - One ctx is used from one thread at a time.  No CPU fallback exists: on a device that
+ *     is not sm_100 every compute entry point returns SRA_ERR_UNSUPPORTED.
+ */
+#ifndef SRA_H_
+#define SRA_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SRA_OK 0
+#define SRA_ERR_INVALID_ARG (-1)  /* NULL where required, bad sizes, bad offsets            */
+#define SRA_ERR_UNSUPPORTED (-2)  /* head_dim not in {64,128}; device is not sm_100         */
+#define SRA_ERR_CUDA (-3)         /* a CUDA runtime/driver call failed (see sra_last_error) */
+#define SRA_ERR_NO_REF_CACHE (-4) /* k_ref/v_ref NULL but sra_cache_reference_kv not called */
+#define SRA_ERR_OOM (-5)          /* device or host allocation failed                       */
+
+typedef struct sra_ctx sra_ctx;
+
+/* Problem statement (shapes from BASELINE.json configs). */
+typedef struct {
+  int32_t batch;                    /* B >= 1                                                       */
+  int32_t heads;                    /* H >= 1 (plain multi-head; the paper is silent on GQA)        */
+  int32_t head_dim;                 /* d in {64, 128}                                               */
+  int32_t n_gen;                    /* generation tokens per batch item (frames x tokens/frame) >=1 */
+  int32_t n_ref;                    /* reference tokens per batch item; 0 => plain self-attention   */
+  int32_t n_ref_blocks;             /* 0 iff n_ref == 0                                             */
+  const int32_t* ref_block_offsets; /* HOST, n_ref_blocks+1 ints: [0]=0, strictly increasing,       */
+                                    /* last = n_ref.  Copied at create.  NULL iff n_ref_blocks == 0 */
+  float softmax_scale;              /* <= 0 => 1/sqrt(head_dim)                                     */
+  int32_t device;                   /* CUDA ordinal, -1 = current device                            */
+} sra_config;
+
+/* Creates a context: validates the config, copies the block pattern, builds the tile
+ * schedule (work items never enumerate a masked tile), allocates the
+ * resident reference-KV cache (2 * B*n_ref*H*d bf16) and the backward workspace lazily.
+ * *out is set to NULL on failure. */
+int sra_create(const sra_config* cfg, sra_ctx** out);
+
+/* "reference KV tensors ... computed once at the first denoising step and
+ * cached in GPU memory".  k_ref / v_ref: DEVICE bf16 [B, n_ref, H, d] (post-projection,
+ * post-RoPE).  They are COPIED (re-laid head-major [B, H, n_ref, d]) into ctx-owned HBM by a
+ * CUDA kernel on `cuda_stream`; the cache stays valid until the next call or sra_destroy and
+ * is read by every later sra_forward whose k_ref/v_ref are NULL.  n_ref == 0 => no-op. */
+int sra_cache_reference_kv(sra_ctx* ctx, const void* k_ref, const void* v_ref, void* cuda_stream);
+
+typedef struct {
+  const void* q_gen; /* DEVICE bf16 [B, n_gen, H, d]                                              */
+  const void* k_gen; /* DEVICE bf16 [B, n_gen, H, d]                                              */
+  const void* v_gen; /* DEVICE bf16 [B, n_gen, H, d]                                              */
+  const void* q_ref; /* DEVICE bf16 [B, n_ref, H, d]; NULL => cached denoising step: R rows are   */
+                     /* skipped entirely                                           */
+  const void* k_ref; /* DEVICE bf16 [B, n_ref, H, d]; NULL => use the resident cache              */
+  const void* v_ref; /* (both NULL or both non-NULL; non-NULL = training, nothing cached)         */
+  void* o_gen;       /* out DEVICE bf16 [B, n_gen, H, d], fully overwritten                       */
+  void* o_ref;       /* out DEVICE bf16 [B, n_ref, H, d]; required iff q_ref != NULL              */
+  float* lse_gen;    /* out DEVICE fp32 [B, H, n_gen], natural log of the scaled scores; nullable */
+  float* lse_ref;    /* out DEVICE fp32 [B, H, n_ref]; nullable                                   */
+} sra_fwd_args;
+
+/* SRA forward: O_g = softmax(s Q_g [K_g;K_r]^T)[V_g;V_r] and, per
+ * reference block j, O_r[j] = softmax(s Q_r[j] K_r[j]^T) V_r[j].  bf16 in/out, fp32
+ * accumulation and softmax.  One kernel launch. */
+int sra_forward(sra_ctx* ctx, const sra_fwd_args* args, void* cuda_stream);
+
+typedef struct {
+  /* forward inputs, all required (training: nothing comes from the cache unless k_ref NULL) */
+  const void *q_gen, *k_gen, *v_gen; /* DEVICE bf16 [B, n_gen, H, d]                              */
+  const void *q_ref, *k_ref, *v_ref; /* DEVICE bf16 [B, n_ref, H, d]; q_ref NULL iff n_ref == 0;  */
+                                     /* k_ref/v_ref NULL => resident cache                        */
+  /* forward results */
+  const void *o_gen, *o_ref;         /* DEVICE bf16, as written by sra_forward                    */
+  const float *lse_gen, *lse_ref;    /* DEVICE fp32 [B, H, n], as written by sra_forward          */
+  /* upstream gradients */
+  const void *do_gen, *do_ref;       /* DEVICE bf16 [B, n, H, d]                                  */
+  /* outputs, bf16, same shapes as the corresponding inputs, fully overwritten */
+  void *dq_gen, *dk_gen, *dv_gen;
+  void *dq_ref, *dk_ref, *dv_ref;
+} sra_bwd_args;
+
+/* SRA backward (standard softmax-attention calculus under the same
+ * mask): D = rowsum(dO o O); P = exp(sQK^T - LSE); dV = P^T dO; dP = dO V^T;
+ * dS = P o (dP - D); dQ = s dS K; dK = s dS^T Q.  dK_r/dV_r receive contributions from all G
+ * rows and from the R rows of the same block. */
+int sra_backward(sra_ctx* ctx, const sra_bwd_args* args, void* cuda_stream);
+
+/* Frees the cache, workspace and schedule.  NULL-safe. */
+void sra_destroy(sra_ctx* ctx);
+
+/* Useful (unmasked) FLOPs of one call: 4*d*pairs*H*B forward, 2.5x that backward, with
+ * pairs = n_gen*(n_gen+n_ref) + (include_ref_rows ? sum_j b_j^2 : 0). */
+int sra_useful_flops(const sra_ctx* ctx, int include_ref_rows, int backward, double* out);
+
+/* Number of work items (CTAs) per (batch, head) the forward schedule enumerates for
+ * generation rows / reference rows, and the total key tiles they visit (for tests of a2). */
+int sra_schedule_info(const sra_ctx* ctx, int32_t* n_gen_items, int32_t* n_ref_items,
+                      int64_t* key_tiles_gen, int64_t* key_tiles_ref);
+
+/* Copies the forward schedule to HOST memory: up to `capacity` items of 8 int32 each
+ * {q_is_ref, q_row0, q_rows, seg0_is_ref, seg0_start, seg0_len, seg1_start, seg1_len}
+ * (seg1 is always the reference segment of a G item; len 0 = absent).  Returns the item
+ * count in *n_items.  Pure host logic - usable without a GPU. */
+int sra_schedule_copy(const sra_ctx* ctx, int32_t* items, int32_t capacity, int32_t* n_items);
+
+/* Device bytes held by the resident reference-KV cache (0 before the first cache call). */
+int64_t sra_cache_bytes(const sra_ctx* ctx);
+
+/* Kernels launched by this ctx since creation (bench.py's gpu_launches). */
+int64_t sra_launch_count(const sra_ctx* ctx);
+
+const char* sra_status_string(int status);
+const char* sra_last_error(const sra_ctx* ctx); /* "" if none; valid until the next call on ctx */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SRA_H_ */

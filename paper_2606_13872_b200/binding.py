@@ -1,0 +1,186 @@
+"""Thin ctypes binding of the C-ABI library declared in include/sra.h.
+
+Argument marshalling only: every step of the SRA path (reference-KV cache build, forward,
+backward) runs in the CUDA kernels of libsra_b200.so.  PyTorch is used for device memory and
+streams (`tensor.data_ptr()`, `torch.cuda.current_stream().cuda_stream`).  There is no CPU or
+PyTorch fallback: if the library is missing, importing this module raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsra_b200.so")
+
+SRA_OK = 0
+SRA_ERR_INVALID_ARG = -1
+SRA_ERR_UNSUPPORTED = -2
+SRA_ERR_CUDA = -3
+SRA_ERR_NO_REF_CACHE = -4
+SRA_ERR_OOM = -5
+
+EXPORTS = (
+    "sra_create", "sra_cache_reference_kv", "sra_forward", "sra_backward", "sra_destroy", "sra_useful_flops",
+    "sra_schedule_info", "sra_schedule_copy", "sra_cache_bytes", "sra_launch_count", "sra_status_string",
+    "sra_last_error",
+)
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        f"{LIB_PATH} not found: build it with `python -m paper_2606_13872_b200.build` "
+        "(the SRA path has no CPU fallback)")
+
+lib = ctypes.CDLL(LIB_PATH)
+
+
+class sra_config(ctypes.Structure):
+    _fields_ = [
+        ("batch", ctypes.c_int32), ("heads", ctypes.c_int32), ("head_dim", ctypes.c_int32),
+        ("n_gen", ctypes.c_int32), ("n_ref", ctypes.c_int32), ("n_ref_blocks", ctypes.c_int32),
+        ("ref_block_offsets", ctypes.POINTER(ctypes.c_int32)),
+        ("softmax_scale", ctypes.c_float), ("device", ctypes.c_int32),
+    ]
+
+
+class sra_fwd_args(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_void_p) for n in
+                ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref", "o_gen", "o_ref", "lse_gen", "lse_ref")]
+
+
+class sra_bwd_args(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_void_p) for n in
+                ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref", "o_gen", "o_ref", "lse_gen", "lse_ref",
+                 "do_gen", "do_ref", "dq_gen", "dk_gen", "dv_gen", "dq_ref", "dk_ref", "dv_ref")]
+
+
+_ctx_p = ctypes.c_void_p
+lib.sra_create.argtypes = [ctypes.POINTER(sra_config), ctypes.POINTER(_ctx_p)]
+lib.sra_create.restype = ctypes.c_int
+lib.sra_cache_reference_kv.argtypes = [_ctx_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+lib.sra_cache_reference_kv.restype = ctypes.c_int
+lib.sra_forward.argtypes = [_ctx_p, ctypes.POINTER(sra_fwd_args), ctypes.c_void_p]
+lib.sra_forward.restype = ctypes.c_int
+lib.sra_backward.argtypes = [_ctx_p, ctypes.POINTER(sra_bwd_args), ctypes.c_void_p]
+lib.sra_backward.restype = ctypes.c_int
+lib.sra_destroy.argtypes = [_ctx_p]
+lib.sra_destroy.restype = None
+lib.sra_useful_flops.argtypes = [_ctx_p, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
+lib.sra_useful_flops.restype = ctypes.c_int
+lib.sra_schedule_info.argtypes = [_ctx_p, ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32),
+                                  ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64)]
+lib.sra_schedule_info.restype = ctypes.c_int
+lib.sra_schedule_copy.argtypes = [_ctx_p, ctypes.POINTER(ctypes.c_int32), ctypes.c_int32,
+                                  ctypes.POINTER(ctypes.c_int32)]
+lib.sra_schedule_copy.restype = ctypes.c_int
+lib.sra_cache_bytes.argtypes = [_ctx_p]
+lib.sra_cache_bytes.restype = ctypes.c_int64
+lib.sra_launch_count.argtypes = [_ctx_p]
+lib.sra_launch_count.restype = ctypes.c_int64
+lib.sra_status_string.argtypes = [ctypes.c_int]
+lib.sra_status_string.restype = ctypes.c_char_p
+lib.sra_last_error.argtypes = [_ctx_p]
+lib.sra_last_error.restype = ctypes.c_char_p
+
+
+class SRAError(RuntimeError):
+    def __init__(self, status: int, detail: str = ""):
+        self.status = status
+        name = lib.sra_status_string(status).decode()
+        super().__init__(f"{name} ({status}){': ' + detail if detail else ''}")
+
+
+def _check(status: int, ctx=None):
+    if status != SRA_OK:
+        detail = lib.sra_last_error(ctx).decode() if ctx else ""
+        raise SRAError(status, detail)
+
+
+def _ptr(t) -> Optional[int]:
+    """Device pointer of a torch tensor (or None).  The tensor must be contiguous."""
+    if t is None:
+        return None
+    if not t.is_contiguous():
+        raise ValueError("SRA tensors must be contiguous [B, N, H, d]")
+    return t.data_ptr()
+
+
+def _stream(stream) -> Optional[int]:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream or None
+    if isinstance(stream, int):
+        return stream or None
+    return stream.cuda_stream or None
+
+
+# ----------------------------------------------------------------------------- same-name wrappers
+def sra_create(batch: int, heads: int, head_dim: int, n_gen: int, ref_block_offsets: Sequence[int],
+               softmax_scale: float = 0.0, device: int = -1) -> int:
+    """sra_create (include/sra.h).  Returns the opaque ctx handle (int)."""
+    off = [int(x) for x in ref_block_offsets] if len(ref_block_offsets) else [0]
+    n_blocks = len(off) - 1
+    arr = (ctypes.c_int32 * len(off))(*off)
+    cfg = sra_config(batch, heads, head_dim, n_gen, off[-1], n_blocks,
+                     arr if n_blocks > 0 else None, float(softmax_scale), device)
+    ctx = _ctx_p()
+    _check(lib.sra_create(ctypes.byref(cfg), ctypes.byref(ctx)))
+    return ctx.value
+
+
+def sra_destroy(ctx: Optional[int]) -> None:
+    lib.sra_destroy(ctx)
+
+
+def sra_cache_reference_kv(ctx: int, k_ref, v_ref, stream=None) -> None:
+    _check(lib.sra_cache_reference_kv(ctx, _ptr(k_ref), _ptr(v_ref), _stream(stream)), ctx)
+
+
+def sra_forward(ctx: int, q_gen, k_gen, v_gen, o_gen, q_ref=None, k_ref=None, v_ref=None, o_ref=None,
+                lse_gen=None, lse_ref=None, stream=None) -> None:
+    a = sra_fwd_args(_ptr(q_gen), _ptr(k_gen), _ptr(v_gen), _ptr(q_ref), _ptr(k_ref), _ptr(v_ref),
+                     _ptr(o_gen), _ptr(o_ref), _ptr(lse_gen), _ptr(lse_ref))
+    _check(lib.sra_forward(ctx, ctypes.byref(a), _stream(stream)), ctx)
+
+
+def sra_backward(ctx: int, *, q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, o_gen, o_ref, lse_gen, lse_ref,
+                 do_gen, do_ref, dq_gen, dk_gen, dv_gen, dq_ref, dk_ref, dv_ref, stream=None) -> None:
+    a = sra_bwd_args(*[_ptr(t) for t in (q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, o_gen, o_ref, lse_gen, lse_ref,
+                                         do_gen, do_ref, dq_gen, dk_gen, dv_gen, dq_ref, dk_ref, dv_ref)])
+    _check(lib.sra_backward(ctx, ctypes.byref(a), _stream(stream)), ctx)
+
+
+def sra_useful_flops(ctx: int, include_ref_rows: bool, backward: bool = False) -> float:
+    out = ctypes.c_double()
+    _check(lib.sra_useful_flops(ctx, int(include_ref_rows), int(backward), ctypes.byref(out)), ctx)
+    return out.value
+
+
+def sra_schedule_info(ctx: int):
+    a, b = ctypes.c_int32(), ctypes.c_int32()
+    c, d = ctypes.c_int64(), ctypes.c_int64()
+    _check(lib.sra_schedule_info(ctx, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c), ctypes.byref(d)), ctx)
+    return {"n_gen_items": a.value, "n_ref_items": b.value, "key_tiles_gen": c.value, "key_tiles_ref": d.value}
+
+
+def sra_schedule_copy(ctx: int):
+    """The forward work items as a list of dicts (host logic only; no GPU needed)."""
+    n = ctypes.c_int32()
+    _check(lib.sra_schedule_copy(ctx, None, 0, ctypes.byref(n)), ctx)
+    buf = (ctypes.c_int32 * (8 * max(n.value, 1)))()
+    _check(lib.sra_schedule_copy(ctx, buf, n.value, ctypes.byref(n)), ctx)
+    keys = ("q_is_ref", "q_row0", "q_rows", "seg0_is_ref", "seg0_start", "seg0_len", "seg1_start", "seg1_len")
+    return [dict(zip(keys, buf[8 * i:8 * i + 8])) for i in range(n.value)]
+
+
+def sra_cache_bytes(ctx: int) -> int:
+    return int(lib.sra_cache_bytes(ctx))
+
+
+def sra_launch_count(ctx: int) -> int:
+    return int(lib.sra_launch_count(ctx))
+
+
+def sra_last_error(ctx: int) -> str:
+    return lib.sra_last_error(ctx).decode()

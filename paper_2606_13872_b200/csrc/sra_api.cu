@@ -1,0 +1,368 @@
+// C-ABI implementation of include/sra.h: context, tile schedule (host), TMA tensor maps,
+// reference-KV cache build and kernel launches.  No CPU compute path exists here.
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "sra_ctx.h"
+
+using sra::BwdItem;
+using sra::FwdItem;
+using sra::kQRowsPerCta;
+using sra::kTile;
+
+
+namespace {
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (fn) return fn;
+  void* p = nullptr;
+  cudaDriverEntryPointQueryResult q;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+      q != cudaDriverEntryPointSuccess)
+    return nullptr;
+  fn = reinterpret_cast<EncodeTiledFn>(p);
+  return fn;
+}
+
+int fail(sra_ctx* ctx, int code, const std::string& msg) { return sra::ctx_fail(ctx, code, msg); }
+int fail_cuda(sra_ctx* ctx, cudaError_t e, const char* what) { return sra::ctx_fail_cuda(ctx, e, what); }
+
+}  // namespace
+
+namespace sra {
+
+int ctx_fail(sra_ctx* ctx, int code, const std::string& msg) {
+  if (ctx) ctx->err = msg;
+  return code;
+}
+int ctx_fail_cuda(sra_ctx* ctx, cudaError_t e, const char* what) {
+  return ctx_fail(ctx, SRA_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+// bf16 tensor map over a [B, N, H, d] (token-major) or [B, H, N, d] (head-major) tensor; box = box_rows x 64
+// columns, 128-byte swizzle, OOB rows read as zero.  Token-major coordinates: (c, h, n, b); head-major: (c, n, h, b).
+int make_tmap_bf16(sra_ctx* ctx, CUtensorMap* out, const void* ptr, int B, int N, int H, int d, bool head_major,
+                   int box_rows) {
+  EncodeTiledFn enc = get_encode_fn();
+  if (!enc) return fail(ctx, SRA_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
+  cuuint64_t dims[4], strides[3];
+  cuuint32_t box[4], estr[4] = {1, 1, 1, 1};
+  const cuuint64_t row = cuuint64_t(d) * 2;
+  if (head_major) {
+    dims[0] = d; dims[1] = N; dims[2] = H; dims[3] = B;
+    strides[0] = row; strides[1] = row * N; strides[2] = row * N * H;
+    box[0] = 64; box[1] = box_rows; box[2] = 1; box[3] = 1;
+  } else {
+    dims[0] = d; dims[1] = H; dims[2] = N; dims[3] = B;
+    strides[0] = row; strides[1] = row * H; strides[2] = row * H * N;
+    box[0] = 64; box[1] = 1; box[2] = box_rows; box[3] = 1;
+  }
+  CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(ptr), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(ctx, SRA_ERR_CUDA, "cuTensorMapEncodeTiled failed: " + std::to_string(int(r)));
+  return SRA_OK;
+}
+
+// [B, N, H, d] -> [B, H, N, d], 16 bytes per thread (a1: pure HBM copy, 2 * bytes of traffic).
+__global__ void relayout_head_major_kernel(const uint4* __restrict__ src0, const uint4* __restrict__ src1,
+                                           uint4* __restrict__ dst0, uint4* __restrict__ dst1, int N, int H, int vec,
+                                           size_t total) {
+  for (size_t i = blockIdx.x * size_t(blockDim.x) + threadIdx.x; i < total; i += size_t(gridDim.x) * blockDim.x) {
+    const int c = int(i % vec);
+    size_t t = i / vec;
+    const int hh = int(t % H);
+    t /= H;
+    const int n = int(t % N);
+    const size_t bb = t / N;
+    const size_t o = ((bb * H + hh) * size_t(N) + n) * vec + c;
+    dst0[o] = src0[i];
+    dst1[o] = src1[i];
+  }
+}
+
+}  // namespace sra
+
+// ------------------------------------------------------------------------------------------------ schedule
+static void build_schedule(sra_ctx* ctx) {
+  const int Ng = ctx->cfg.n_gen, Nr = ctx->cfg.n_ref;
+  ctx->fwd_items.clear();
+  // G slabs: every generation key tile, then every reference key tile.
+  for (int r0 = 0; r0 < Ng; r0 += kQRowsPerCta) {
+    FwdItem it{};
+    it.q_is_ref = 0; it.q_row0 = r0; it.q_rows = std::min(kQRowsPerCta, Ng - r0);
+    it.seg0_is_ref = 0; it.seg0_start = 0; it.seg0_len = Ng;
+    it.seg1_start = 0; it.seg1_len = Nr;
+    ctx->fwd_items.push_back(it);
+  }
+  ctx->n_gen_items = int(ctx->fwd_items.size());
+  // R slabs: only the keys of the slab's own block ("reference tokens only self-attend").
+  for (int j = 0; j + 1 < int(ctx->off.size()); ++j) {
+    const int s = ctx->off[j], e = ctx->off[j + 1];
+    for (int r0 = s; r0 < e; r0 += kQRowsPerCta) {
+      FwdItem it{};
+      it.q_is_ref = 1; it.q_row0 = r0; it.q_rows = std::min(kQRowsPerCta, e - r0);
+      it.seg0_is_ref = 1; it.seg0_start = s; it.seg0_len = e - s;
+      it.seg1_start = 0; it.seg1_len = 0;
+      ctx->fwd_items.push_back(it);
+    }
+  }
+  ctx->n_ref_items = int(ctx->fwd_items.size()) - ctx->n_gen_items;
+  // Backward: key tiles.  G key tiles are seen by all G queries; R key tiles of block j additionally by block j's
+  // R queries.  Tiles never straddle a block boundary.
+  ctx->bwd_items.clear();
+  for (int k0 = 0; k0 < Ng; k0 += kTile) {
+    BwdItem it{};
+    it.k_is_ref = 0; it.k_row0 = k0; it.k_rows = std::min(kTile, Ng - k0);
+    ctx->bwd_items.push_back(it);
+  }
+  for (int j = 0; j + 1 < int(ctx->off.size()); ++j) {
+    const int s = ctx->off[j], e = ctx->off[j + 1];
+    for (int k0 = s; k0 < e; k0 += kTile) {
+      BwdItem it{};
+      it.k_is_ref = 1; it.k_row0 = k0; it.k_rows = std::min(kTile, e - k0);
+      it.seg1_start = s; it.seg1_len = e - s;
+      ctx->bwd_items.push_back(it);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ C ABI
+extern "C" {
+
+const char* sra_status_string(int s) {
+  switch (s) {
+    case SRA_OK: return "SRA_OK";
+    case SRA_ERR_INVALID_ARG: return "SRA_ERR_INVALID_ARG";
+    case SRA_ERR_UNSUPPORTED: return "SRA_ERR_UNSUPPORTED";
+    case SRA_ERR_CUDA: return "SRA_ERR_CUDA";
+    case SRA_ERR_NO_REF_CACHE: return "SRA_ERR_NO_REF_CACHE";
+    case SRA_ERR_OOM: return "SRA_ERR_OOM";
+    default: return "SRA_ERR_UNKNOWN";
+  }
+}
+
+const char* sra_last_error(const sra_ctx* ctx) { return ctx ? ctx->err.c_str() : ""; }
+
+int sra_create(const sra_config* cfg, sra_ctx** out) {
+  if (!out) return SRA_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (!cfg) return SRA_ERR_INVALID_ARG;
+  if (cfg->batch < 1 || cfg->heads < 1 || cfg->n_gen < 1 || cfg->n_ref < 0 || cfg->n_ref_blocks < 0)
+    return SRA_ERR_INVALID_ARG;
+  if (cfg->head_dim != 64 && cfg->head_dim != 128) return SRA_ERR_UNSUPPORTED;
+  if ((cfg->n_ref == 0) != (cfg->n_ref_blocks == 0)) return SRA_ERR_INVALID_ARG;
+  if (cfg->n_ref_blocks > 0) {
+    if (!cfg->ref_block_offsets || cfg->ref_block_offsets[0] != 0) return SRA_ERR_INVALID_ARG;
+    for (int j = 0; j < cfg->n_ref_blocks; ++j)
+      if (cfg->ref_block_offsets[j + 1] <= cfg->ref_block_offsets[j]) return SRA_ERR_INVALID_ARG;
+    if (cfg->ref_block_offsets[cfg->n_ref_blocks] != cfg->n_ref) return SRA_ERR_INVALID_ARG;
+  }
+  if (cfg->heads > 65535 || cfg->batch > 65535) return SRA_ERR_INVALID_ARG;
+  sra_ctx* ctx = new (std::nothrow) sra_ctx();
+  if (!ctx) return SRA_ERR_OOM;
+  ctx->cfg = *cfg;
+  ctx->off.assign(1, 0);
+  for (int j = 0; j < cfg->n_ref_blocks; ++j) ctx->off.push_back(cfg->ref_block_offsets[j + 1]);
+  ctx->cfg.ref_block_offsets = nullptr;
+  ctx->scale = cfg->softmax_scale > 0.f ? cfg->softmax_scale : 1.0f / std::sqrt(float(cfg->head_dim));
+  build_schedule(ctx);
+
+  // Device discovery.  Without a usable CUDA device the ctx is host-only: the schedule can be inspected, every
+  // compute entry point fails with SRA_ERR_UNSUPPORTED (there is no CPU fallback).
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    (void)cudaGetLastError();
+    ctx->device = -1;
+    *out = ctx;
+    return SRA_OK;
+  }
+  int dev = cfg->device;
+  if (dev < 0 && cudaGetDevice(&dev) != cudaSuccess) dev = 0;
+  if (dev >= ndev) { delete ctx; return SRA_ERR_INVALID_ARG; }
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) { (void)cudaGetLastError(); delete ctx; return SRA_ERR_CUDA; }
+  ctx->device = dev;
+  ctx->sm100 = (prop.major == 10);
+  if (ctx->sm100) {
+    cudaSetDevice(dev);
+    cudaError_t e = cudaMalloc(&ctx->d_fwd_items, ctx->fwd_items.size() * sizeof(FwdItem));
+    if (e == cudaSuccess) e = cudaMemcpy(ctx->d_fwd_items, ctx->fwd_items.data(), ctx->fwd_items.size() * sizeof(FwdItem), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_bwd_items, ctx->bwd_items.size() * sizeof(BwdItem));
+    if (e == cudaSuccess) e = cudaMemcpy(ctx->d_bwd_items, ctx->bwd_items.data(), ctx->bwd_items.size() * sizeof(BwdItem), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); sra_destroy(ctx); return e == cudaErrorMemoryAllocation ? SRA_ERR_OOM : SRA_ERR_CUDA; }
+  }
+  *out = ctx;
+  return SRA_OK;
+}
+
+void sra_destroy(sra_ctx* ctx) {
+  if (!ctx) return;
+  if (ctx->device >= 0) {
+    cudaFree(ctx->d_fwd_items);
+    cudaFree(ctx->d_bwd_items);
+    cudaFree(ctx->cache_k);
+    cudaFree(ctx->cache_v);
+    cudaFree(ctx->ws_dq);
+    cudaFree(ctx->ws_delta);
+    (void)cudaGetLastError();
+  }
+  delete ctx;
+}
+
+static int check_device(sra_ctx* ctx) {
+  if (ctx->device < 0) return fail(ctx, SRA_ERR_UNSUPPORTED, "no CUDA device: this library has no CPU path");
+  if (!ctx->sm100) return fail(ctx, SRA_ERR_UNSUPPORTED, "device is not sm_100 (B200); kernels are sm_100a-only");
+  return SRA_OK;
+}
+
+int sra_cache_reference_kv(sra_ctx* ctx, const void* k_ref, const void* v_ref, void* cuda_stream) {
+  if (!ctx) return SRA_ERR_INVALID_ARG;
+  ctx->err.clear();
+  if (int rc = check_device(ctx)) return rc;
+  if (ctx->cfg.n_ref == 0) return SRA_OK;
+  if (!k_ref || !v_ref) return fail(ctx, SRA_ERR_INVALID_ARG, "k_ref / v_ref must be non-NULL");
+  const sra_config& c = ctx->cfg;
+  const size_t elems = size_t(c.batch) * c.n_ref * c.heads * c.head_dim;
+  if (!ctx->cache_k) {
+    cudaError_t e = cudaMalloc(&ctx->cache_k, elems * 2);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->cache_v, elems * 2);
+    if (e != cudaSuccess) {
+      (void)cudaGetLastError();
+      cudaFree(ctx->cache_k); ctx->cache_k = nullptr;
+      return fail(ctx, SRA_ERR_OOM, "reference-KV cache allocation failed");
+    }
+  }
+  const int vec = c.head_dim / 8;
+  const size_t total = elems / 8;
+  const int threads = 256;
+  const int blocks = int(std::min<size_t>((total + threads - 1) / threads, size_t(148) * 16));
+  sra::relayout_head_major_kernel<<<blocks, threads, 0, cudaStream_t(cuda_stream)>>>(
+      static_cast<const uint4*>(k_ref), static_cast<const uint4*>(v_ref), reinterpret_cast<uint4*>(ctx->cache_k),
+      reinterpret_cast<uint4*>(ctx->cache_v), c.n_ref, c.heads, vec, total);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "cache relayout launch");
+  ctx->launches += 1;
+  ctx->cache_valid = true;
+  return SRA_OK;
+}
+
+int sra_forward(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) {
+  if (!ctx) return SRA_ERR_INVALID_ARG;
+  ctx->err.clear();
+  if (!a) return fail(ctx, SRA_ERR_INVALID_ARG, "args is NULL");
+  if (int rc = check_device(ctx)) return rc;
+  const sra_config& c = ctx->cfg;
+  if (!a->q_gen || !a->k_gen || !a->v_gen || !a->o_gen) return fail(ctx, SRA_ERR_INVALID_ARG, "q_gen/k_gen/v_gen/o_gen required");
+  if ((a->k_ref == nullptr) != (a->v_ref == nullptr)) return fail(ctx, SRA_ERR_INVALID_ARG, "k_ref and v_ref must both be NULL or both non-NULL");
+  const bool with_ref_rows = a->q_ref != nullptr && c.n_ref > 0;
+  if (with_ref_rows && !a->o_ref) return fail(ctx, SRA_ERR_INVALID_ARG, "o_ref required when q_ref is given");
+  const bool use_cache = c.n_ref > 0 && a->k_ref == nullptr;
+  if (use_cache && !ctx->cache_valid) return fail(ctx, SRA_ERR_NO_REF_CACHE, "k_ref/v_ref NULL but sra_cache_reference_kv was never called");
+  const void* ptrs[] = {a->q_gen, a->k_gen, a->v_gen, a->q_ref, a->k_ref, a->v_ref, a->o_gen, a->o_ref};
+  for (const void* q : ptrs)
+    if (q && (reinterpret_cast<uintptr_t>(q) & 15)) return fail(ctx, SRA_ERR_INVALID_ARG, "tensor pointers must be 16-byte aligned");
+
+  CUtensorMap maps[6];
+  const int B = c.batch, H = c.heads, d = c.head_dim;
+  int rc;
+  if ((rc = sra::make_tmap_bf16(ctx, &maps[0], a->q_gen, B, c.n_gen, H, d, false, kTile))) return rc;
+  if ((rc = sra::make_tmap_bf16(ctx, &maps[1], a->k_gen, B, c.n_gen, H, d, false, kTile))) return rc;
+  if ((rc = sra::make_tmap_bf16(ctx, &maps[2], a->v_gen, B, c.n_gen, H, d, false, kTile))) return rc;
+  maps[3] = maps[0]; maps[4] = maps[1]; maps[5] = maps[2];  // placeholders when n_ref == 0 (never dereferenced)
+  if (c.n_ref > 0) {
+    if (with_ref_rows && (rc = sra::make_tmap_bf16(ctx, &maps[3], a->q_ref, B, c.n_ref, H, d, false, kTile))) return rc;
+    const void* kr = use_cache ? ctx->cache_k : a->k_ref;
+    const void* vr = use_cache ? ctx->cache_v : a->v_ref;
+    if ((rc = sra::make_tmap_bf16(ctx, &maps[4], kr, B, c.n_ref, H, d, use_cache, kTile))) return rc;
+    if ((rc = sra::make_tmap_bf16(ctx, &maps[5], vr, B, c.n_ref, H, d, use_cache, kTile))) return rc;
+  }
+  sra::FwdParams p{};
+  p.items = ctx->d_fwd_items;
+  p.n_items = ctx->n_gen_items + (with_ref_rows ? ctx->n_ref_items : 0);
+  p.heads = H; p.batch = B; p.n_gen = c.n_gen; p.n_ref = c.n_ref;
+  p.scale = ctx->scale;
+  p.scale_log2 = ctx->scale * 1.4426950408889634f;
+  p.o_gen = static_cast<__nv_bfloat16*>(a->o_gen);
+  p.o_ref = static_cast<__nv_bfloat16*>(a->o_ref);
+  p.lse_gen = a->lse_gen;
+  p.lse_ref = a->lse_ref;
+  p.ref_kv_head_major = use_cache ? 1 : 0;
+  cudaError_t e = (d == 128) ? sra::launch_fwd<128>(maps, p, cudaStream_t(cuda_stream))
+                             : sra::launch_fwd<64>(maps, p, cudaStream_t(cuda_stream));
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "sra_fwd_kernel launch");
+  ctx->launches += 1;
+  return SRA_OK;
+}
+
+int sra_backward(sra_ctx* ctx, const sra_bwd_args* a, void* cuda_stream) {
+  if (!ctx) return SRA_ERR_INVALID_ARG;
+  ctx->err.clear();
+  if (!a) return fail(ctx, SRA_ERR_INVALID_ARG, "args is NULL");
+  if (int rc = check_device(ctx)) return rc;
+  return sra::run_backward(ctx, a, cudaStream_t(cuda_stream));
+}
+
+int sra_useful_flops(const sra_ctx* ctx, int include_ref_rows, int backward, double* out) {
+  if (!ctx || !out) return SRA_ERR_INVALID_ARG;
+  const sra_config& c = ctx->cfg;
+  double pairs = double(c.n_gen) * (double(c.n_gen) + double(c.n_ref));
+  if (include_ref_rows)
+    for (size_t j = 0; j + 1 < ctx->off.size(); ++j) {
+      const double bsz = double(ctx->off[j + 1] - ctx->off[j]);
+      pairs += bsz * bsz;
+    }
+  *out = 4.0 * c.head_dim * pairs * c.heads * c.batch * (backward ? 2.5 : 1.0);
+  return SRA_OK;
+}
+
+int sra_schedule_info(const sra_ctx* ctx, int32_t* n_gen_items, int32_t* n_ref_items, int64_t* key_tiles_gen,
+                      int64_t* key_tiles_ref) {
+  if (!ctx) return SRA_ERR_INVALID_ARG;
+  int64_t tg = 0, tr = 0;
+  for (size_t i = 0; i < ctx->fwd_items.size(); ++i) {
+    const FwdItem& it = ctx->fwd_items[i];
+    const int64_t qt = (it.q_rows + kTile - 1) / kTile;
+    const int64_t t = qt * ((it.seg0_len + kTile - 1) / kTile + (it.seg1_len + kTile - 1) / kTile);
+    (it.q_is_ref ? tr : tg) += t;
+  }
+  if (n_gen_items) *n_gen_items = ctx->n_gen_items;
+  if (n_ref_items) *n_ref_items = ctx->n_ref_items;
+  if (key_tiles_gen) *key_tiles_gen = tg;
+  if (key_tiles_ref) *key_tiles_ref = tr;
+  return SRA_OK;
+}
+
+int sra_schedule_copy(const sra_ctx* ctx, int32_t* items, int32_t capacity, int32_t* n_items) {
+  if (!ctx || !n_items) return SRA_ERR_INVALID_ARG;
+  *n_items = int32_t(ctx->fwd_items.size());
+  if (items) {
+    const int n = std::min<int>(capacity, *n_items);
+    static_assert(sizeof(FwdItem) == 8 * sizeof(int32_t), "FwdItem layout is part of the ABI");
+    std::memcpy(items, ctx->fwd_items.data(), size_t(n) * sizeof(FwdItem));
+  }
+  return SRA_OK;
+}
+
+int64_t sra_cache_bytes(const sra_ctx* ctx) {
+  if (!ctx || !ctx->cache_k) return 0;
+  const sra_config& c = ctx->cfg;
+  return int64_t(2) * c.batch * c.n_ref * c.heads * c.head_dim * 2;
+}
+
+int64_t sra_launch_count(const sra_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+}  // extern "C"

@@ -1,0 +1,50 @@
+// Shared host/device definitions of the SRA CUDA path (work items, kernel parameters).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace sra {
+
+constexpr int kTile = 128;         // rows per MMA tile (UMMA M = 128; key tile N = 128)
+constexpr int kQRowsPerCta = 256;  // two ping-ponged Q tiles per CTA (forward)
+
+// Forward work item: a 256-row query slab and the (up to two) key
+// segments it may see.  G slab: seg0 = all generation keys, seg1 = all reference keys.
+// R slab of block j: seg0 = reference keys [off[j], off[j+1]), seg1 empty.
+struct FwdItem {
+  int32_t q_is_ref;     // 0: rows of Q_g / O_g, 1: rows of Q_r / O_r
+  int32_t q_row0;       // first row (token index inside its tensor)
+  int32_t q_rows;       // valid rows in this slab, 1..256
+  int32_t seg0_is_ref;  // which K/V tensors seg0 reads
+  int32_t seg0_start, seg0_len;
+  int32_t seg1_start, seg1_len;  // always reference K/V; len 0 = absent
+};
+
+// Backward work item: a 128-key tile and the (up to two) query segments that see it.
+// G key tile: seg0 = all generation queries.  R key tile of block j: seg0 = all generation
+// queries, seg1 = reference queries [off[j], off[j+1]).
+struct BwdItem {
+  int32_t k_is_ref;
+  int32_t k_row0;
+  int32_t k_rows;  // valid keys 1..128
+  int32_t seg1_start, seg1_len;  // reference-query segment (len 0 = absent)
+  int32_t pad[3];
+};
+
+struct FwdParams {
+  const FwdItem* items;
+  int32_t n_items;
+  int32_t heads, batch;
+  int32_t n_gen, n_ref;
+  float scale_log2;  // softmax_scale * log2(e)
+  float scale;       // softmax_scale
+  __nv_bfloat16* o_gen;
+  __nv_bfloat16* o_ref;
+  float* lse_gen;  // may be null
+  float* lse_ref;  // may be null
+  // coordinate order of the K/V reference tensor maps: 1 = head-major cache [B,H,N,d] => (c, n, h, b)
+  int32_t ref_kv_head_major;
+};
+
+}  // namespace sra

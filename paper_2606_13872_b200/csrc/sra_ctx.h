@@ -1,0 +1,44 @@
+// Private definition of sra_ctx (shared by the API and the backward driver).
+#pragma once
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/sra.h"
+#include "sra_common.h"
+
+struct sra_ctx {
+  sra_config cfg{};
+  std::vector<int32_t> off;  // n_ref_blocks + 1
+  float scale = 0.f;
+  int device = -1;       // -1: host-only context (no usable CUDA device)
+  bool sm100 = false;
+  std::vector<sra::FwdItem> fwd_items;  // G items first, then R items
+  int n_gen_items = 0, n_ref_items = 0;
+  std::vector<sra::BwdItem> bwd_items;
+  sra::FwdItem* d_fwd_items = nullptr;
+  sra::BwdItem* d_bwd_items = nullptr;
+  __nv_bfloat16* cache_k = nullptr;  // [B, H, n_ref, d]
+  __nv_bfloat16* cache_v = nullptr;
+  bool cache_valid = false;
+  // backward workspace (lazy)
+  float* ws_dq = nullptr;     // fp32 [B, H, n_gen + n_ref, d] accumulators
+  float* ws_delta = nullptr;  // fp32 [B, H, n_gen + n_ref]
+  size_t ws_dq_bytes = 0;
+  int64_t launches = 0;
+  std::string err;
+};
+
+namespace sra {
+int ctx_fail(sra_ctx* ctx, int code, const std::string& msg);
+int ctx_fail_cuda(sra_ctx* ctx, cudaError_t e, const char* what);
+int make_tmap_bf16(sra_ctx* ctx, CUtensorMap* out, const void* ptr, int B, int N, int H, int d, bool head_major,
+                   int box_rows);
+int make_tmap_f32(sra_ctx* ctx, CUtensorMap* out, const void* ptr, int B, int N, int H, int d, int box_rows);
+template <int D>
+cudaError_t launch_fwd(const CUtensorMap* maps, const FwdParams& p, cudaStream_t stream);
+int run_backward(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t stream);
+}  // namespace sra

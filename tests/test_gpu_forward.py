@@ -1,0 +1,138 @@
+"""-m gpu parity tests of the SRA forward: CUDA path (through the C ABI) vs the fp64 oracle.
+
+Contract tolerance (BASELINE.json north_star): bf16 I/O, fp32 accumulation, GPU vs oracle
+max-abs <= 2e-2 and mean-abs <= 2e-3; plus the self-imposed relative gate rel_l2 <= 1e-2
+(SURVEY.md 8c "tolerance bite": at paper sizes the absolute contract alone is nearly vacuous).
+LSE gate: max-abs <= 2e-3 (fp32 accumulation of O(1) numbers).
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_13872_b200 import inputs as sra_inputs
+from tests.gpu_util import bits, boundary_rows, gather_rows, oracle_forward_rows, run_gpu_forward
+from tests.util import assert_parity
+
+pytestmark = pytest.mark.gpu
+
+LSE_TOL = 2e-3
+
+
+def _full_parity(name, use_cache=True, dist=None, with_ref_rows=True):
+    w = sra_inputs.WORKLOADS[name]
+    if dist:
+        w = w.replace(dist=dist)
+    t = sra_inputs.make_inputs(w)
+    scale = 1.0 / math.sqrt(w.head_dim)
+    out = run_gpu_forward(w, t, use_cache=use_cache, with_ref_rows=with_ref_rows)
+    n = w.n_gen + (w.n_ref if with_ref_rows else 0)
+    rows = np.arange(n, dtype=np.int32)
+    o_ref, lse_ref = oracle_forward_rows(w, bits(t), rows, scale)
+    o_gpu, lse_gpu = gather_rows(out, w, rows)
+    m = assert_parity(o_gpu, o_ref, f"{name} O")
+    assert np.abs(lse_gpu - lse_ref).max() <= LSE_TOL, f"{name} LSE max err {np.abs(lse_gpu - lse_ref).max():.3e}"
+    return m
+
+
+@pytest.mark.parametrize("dist", ["A", "B", "peaked"])
+def test_tiny_full(dist):
+    """BASELINE.json configs[0]: B1 H4 d64, 256 gen + 4x128 ref, all rows, all heads."""
+    _full_parity("tiny", dist=dist)
+
+
+@pytest.mark.parametrize("use_cache", [True, False])
+def test_ragged_d128(use_cache):
+    """Non-uniform blocks (1, 130, 257, 64, 200), n_gen = 333, B2 H3: ragged tails everywhere."""
+    _full_parity("ragged", use_cache=use_cache)
+
+
+def test_ragged_d64_peaked():
+    _full_parity("ragged64")
+
+
+def test_mini480_full():
+    """Real 1560-token block structure, scaled down (H2, 2x1560 gen + 3x1560 ref), every row."""
+    _full_parity("mini480")
+
+
+def test_mini720_full():
+    _full_parity("mini720")
+
+
+def test_cached_step_skips_ref_rows():
+    """q_ref == NULL (PAPER.md:223 cached denoising step): only G rows are produced, one launch."""
+    w = sra_inputs.WORKLOADS["ragged"]
+    t = sra_inputs.make_inputs(w)
+    out = run_gpu_forward(w, t, use_cache=True, with_ref_rows=False)
+    assert "o_ref" not in out
+    rows = np.arange(w.n_gen, dtype=np.int32)
+    o_ref, _ = oracle_forward_rows(w, bits(t), rows, 1.0 / math.sqrt(w.head_dim))
+    assert_parity(out["o_gen"], o_ref, "cached-step O_g")
+    assert out["launches"] == 2  # cache build + one forward kernel
+
+
+def test_zero_ref_is_plain_self_attention():
+    """n_ref == 0 => full self-attention over G (north_star invariant), vs torch SDPA fp64 on CPU."""
+    w = sra_inputs.SRAWorkload("noref", 1, 2, 128, 300, (), "B", 3)
+    t = sra_inputs.make_inputs(w, names=("q_gen", "k_gen", "v_gen"))
+    out = run_gpu_forward(w, t)
+    q, k, v = (t[n].double().permute(0, 2, 1, 3) for n in ("q_gen", "k_gen", "v_gen"))
+    ref = torch.nn.functional.scaled_dot_product_attention(q, k, v).permute(0, 2, 1, 3).numpy()
+    assert_parity(out["o_gen"], ref, "zero-ref O_g")
+
+
+def test_mask_poison():
+    """huge finite values in K/V rows an R query must not see leave O_r unchanged."""
+    w = sra_inputs.WORKLOADS["ragged"]
+    t = sra_inputs.make_inputs(w)
+    base = run_gpu_forward(w, t, use_cache=False)
+    off = w.ref_block_offsets
+    j = 2  # poison everything except block j (and all generation K/V)
+    tp = {k: v.clone() for k, v in t.items()}
+    for name in ("k_gen", "v_gen"):
+        tp[name].fill_(1e4)
+    for name in ("k_ref", "v_ref"):
+        tp[name][:, :off[j]] = -1e4
+        tp[name][:, off[j + 1]:] = 1e4
+    pois = run_gpu_forward(w, tp, use_cache=False)
+    a = base["o_ref"][:, off[j]:off[j + 1]]
+    b = pois["o_ref"][:, off[j]:off[j + 1]]
+    assert np.array_equal(a, b), "R rows of block j changed when unseen keys/values were poisoned"
+    assert np.array_equal(base["lse_ref"][:, :, off[j]:off[j + 1]], pois["lse_ref"][:, :, off[j]:off[j + 1]])
+
+
+def test_group_indicator_mass():
+    """V[j] = e_{group(j)}: O rows are probability mass per group; masked groups must be exactly 0."""
+    w = sra_inputs.WORKLOADS["ragged"]
+    t = sra_inputs.make_inputs(w)
+    off = w.ref_block_offsets
+    t["v_gen"].zero_()
+    t["v_ref"].zero_()
+    t["v_gen"][..., 0] = 1.0
+    for j in range(len(off) - 1):
+        t["v_ref"][:, off[j]:off[j + 1], :, 1 + j] = 1.0
+    out = run_gpu_forward(w, t, use_cache=True)
+    ng = len(off)  # groups: G + blocks
+    og = out["o_gen"][..., :ng]
+    assert np.abs(og.sum(-1) - 1.0).max() <= 1e-2
+    for j in range(len(off) - 1):
+        orf = out["o_ref"][:, off[j]:off[j + 1]]
+        assert np.abs(orf[..., 1 + j] - 1.0).max() <= 8e-3  # bf16 output rounding of ~1
+        others = np.delete(orf[..., :ng], 1 + j, axis=-1)
+        assert np.all(others == 0.0), "probability mass leaked to a masked group"
+
+
+def test_480p_sampled_rows():
+    """BASELINE.json configs[1] at full size, launch configuration of bench.py; sampled rows vs oracle."""
+    w = sra_inputs.WORKLOADS["480p"].replace(dist="B")
+    t = sra_inputs.make_inputs(w)
+    out = run_gpu_forward(w, t, use_cache=True)
+    rows = boundary_rows(w, n_random=16)
+    o_ref, lse_ref = oracle_forward_rows(w, bits(t), rows, 1.0 / math.sqrt(w.head_dim))
+    o_gpu, lse_gpu = gather_rows(out, w, rows)
+    assert_parity(o_gpu, o_ref, "480p sampled O")
+    assert np.abs(lse_gpu - lse_ref).max() <= LSE_TOL
+    # property at any size: every output finite
+    assert np.isfinite(out["o_gen"]).all() and np.isfinite(out["o_ref"]).all()
