@@ -91,6 +91,26 @@ typedef struct {
  * accumulation and softmax.  One kernel launch. */
 int sra_forward(sra_ctx* ctx, const sra_fwd_args* args, void* cuda_stream);
 
+
+typedef struct {
+  const void* q_gen; /* HOST bf16 [B, n_gen, H, d] (pinned memory recommended: the copies are async) */
+  const void* k_gen; /* HOST bf16 [B, n_gen, H, d]                                                 */
+  const void* v_gen; /* HOST bf16 [B, n_gen, H, d]                                                 */
+  const void* q_ref; /* HOST bf16 [B, n_ref, H, d] or NULL (cached denoising step)                 */
+  void* o_gen;       /* out HOST bf16 [B, n_gen, H, d]                                             */
+  void* o_ref;       /* out HOST bf16 [B, n_ref, H, d]; required iff q_ref != NULL                 */
+  float* lse_gen;    /* out HOST fp32 [B, H, n_gen]; nullable                                      */
+  float* lse_ref;    /* out HOST fp32 [B, H, n_ref]; nullable                                      */
+} sra_fwd_host_args;
+
+/* End-to-end form of one denoising step (fresh generation Q/K/V arrive each step,
+ * the reference K/V come from the resident cache): every pointer is a HOST pointer.  Enqueues on
+ * `cuda_stream` the host->device copies of q/k/v into ctx-owned staging buffers (allocated on first
+ * use, freed by sra_destroy), the same forward kernel as sra_forward, and the device->host copies of
+ * the outputs.  The results are valid after the caller synchronises the stream.  Requires the
+ * resident cache when n_ref > 0 (SRA_ERR_NO_REF_CACHE otherwise). */
+int sra_forward_host(sra_ctx* ctx, const sra_fwd_host_args* args, void* cuda_stream);
+
 typedef struct {
   /* forward inputs, all required (training: nothing comes from the cache unless k_ref NULL) */
   const void *q_gen, *k_gen, *v_gen; /* DEVICE bf16 [B, n_gen, H, d]                              */

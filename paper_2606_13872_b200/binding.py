@@ -22,7 +22,7 @@ SRA_ERR_NO_REF_CACHE = -4
 SRA_ERR_OOM = -5
 
 EXPORTS = (
-    "sra_create", "sra_cache_reference_kv", "sra_forward", "sra_backward", "sra_destroy", "sra_useful_flops",
+    "sra_create", "sra_cache_reference_kv", "sra_forward", "sra_forward_host", "sra_backward", "sra_destroy", "sra_useful_flops",
     "sra_schedule_info", "sra_schedule_copy", "sra_cache_bytes", "sra_launch_count", "sra_status_string",
     "sra_last_error",
 )
@@ -49,6 +49,11 @@ class sra_fwd_args(ctypes.Structure):
                 ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref", "o_gen", "o_ref", "lse_gen", "lse_ref")]
 
 
+class sra_fwd_host_args(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_void_p) for n in
+                ("q_gen", "k_gen", "v_gen", "q_ref", "o_gen", "o_ref", "lse_gen", "lse_ref")]
+
+
 class sra_bwd_args(ctypes.Structure):
     _fields_ = [(n, ctypes.c_void_p) for n in
                 ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref", "o_gen", "o_ref", "lse_gen", "lse_ref",
@@ -62,6 +67,8 @@ lib.sra_cache_reference_kv.argtypes = [_ctx_p, ctypes.c_void_p, ctypes.c_void_p,
 lib.sra_cache_reference_kv.restype = ctypes.c_int
 lib.sra_forward.argtypes = [_ctx_p, ctypes.POINTER(sra_fwd_args), ctypes.c_void_p]
 lib.sra_forward.restype = ctypes.c_int
+lib.sra_forward_host.argtypes = [_ctx_p, ctypes.POINTER(sra_fwd_host_args), ctypes.c_void_p]
+lib.sra_forward_host.restype = ctypes.c_int
 lib.sra_backward.argtypes = [_ctx_p, ctypes.POINTER(sra_bwd_args), ctypes.c_void_p]
 lib.sra_backward.restype = ctypes.c_int
 lib.sra_destroy.argtypes = [_ctx_p]
@@ -142,6 +149,22 @@ def sra_forward(ctx: int, q_gen, k_gen, v_gen, o_gen, q_ref=None, k_ref=None, v_
     a = sra_fwd_args(_ptr(q_gen), _ptr(k_gen), _ptr(v_gen), _ptr(q_ref), _ptr(k_ref), _ptr(v_ref),
                      _ptr(o_gen), _ptr(o_ref), _ptr(lse_gen), _ptr(lse_ref))
     _check(lib.sra_forward(ctx, ctypes.byref(a), _stream(stream)), ctx)
+
+
+def _host_ptr(t) -> Optional[int]:
+    """Host pointer of a CPU torch tensor (or None).  Must be contiguous; pin it for async copies."""
+    if t is None:
+        return None
+    if t.device.type != "cpu" or not t.is_contiguous():
+        raise ValueError("sra_forward_host takes contiguous CPU tensors")
+    return t.data_ptr()
+
+
+def sra_forward_host(ctx: int, q_gen, k_gen, v_gen, o_gen, q_ref=None, o_ref=None, lse_gen=None, lse_ref=None,
+                     stream=None) -> None:
+    """sra_forward_host (include/sra.h): HOST tensors in/out, reference K/V from the resident cache."""
+    a = sra_fwd_host_args(*[_host_ptr(t) for t in (q_gen, k_gen, v_gen, q_ref, o_gen, o_ref, lse_gen, lse_ref)])
+    _check(lib.sra_forward_host(ctx, ctypes.byref(a), _stream(stream)), ctx)
 
 
 def sra_backward(ctx: int, *, q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, o_gen, o_ref, lse_gen, lse_ref,

@@ -218,6 +218,7 @@ void sra_destroy(sra_ctx* ctx) {
     cudaFree(ctx->cache_v);
     cudaFree(ctx->ws_dq);
     cudaFree(ctx->ws_delta);
+    for (void* s : ctx->stage) cudaFree(s);
     (void)cudaGetLastError();
   }
   delete ctx;
@@ -305,6 +306,47 @@ int sra_forward(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) {
                              : sra::launch_fwd<64>(maps, p, cudaStream_t(cuda_stream));
   if (e != cudaSuccess) return fail_cuda(ctx, e, "sra_fwd_kernel launch");
   ctx->launches += 1;
+  return SRA_OK;
+}
+
+int sra_forward_host(sra_ctx* ctx, const sra_fwd_host_args* a, void* cuda_stream) {
+  if (!ctx) return SRA_ERR_INVALID_ARG;
+  ctx->err.clear();
+  if (!a) return fail(ctx, SRA_ERR_INVALID_ARG, "args is NULL");
+  if (int rc = check_device(ctx)) return rc;
+  const sra_config& c = ctx->cfg;
+  if (!a->q_gen || !a->k_gen || !a->v_gen || !a->o_gen) return fail(ctx, SRA_ERR_INVALID_ARG, "q_gen/k_gen/v_gen/o_gen required");
+  const bool with_ref_rows = a->q_ref != nullptr && c.n_ref > 0;
+  if (with_ref_rows && !a->o_ref) return fail(ctx, SRA_ERR_INVALID_ARG, "o_ref required when q_ref is given");
+  if (c.n_ref > 0 && !ctx->cache_valid) return fail(ctx, SRA_ERR_NO_REF_CACHE, "sra_forward_host reads reference K/V from the resident cache");
+  const size_t row = size_t(c.heads) * c.head_dim * 2;
+  const size_t gen_bytes = size_t(c.batch) * c.n_gen * row, ref_bytes = size_t(c.batch) * c.n_ref * row;
+  const size_t lse_gen_bytes = size_t(c.batch) * c.heads * c.n_gen * 4, lse_ref_bytes = size_t(c.batch) * c.heads * c.n_ref * 4;
+  const size_t want[8] = {gen_bytes, gen_bytes, gen_bytes, gen_bytes, with_ref_rows ? ref_bytes : 0,
+                          with_ref_rows ? ref_bytes : 0, a->lse_gen ? lse_gen_bytes : 0,
+                          (with_ref_rows && a->lse_ref) ? lse_ref_bytes : 0};
+  for (int i = 0; i < 8; ++i)
+    if (want[i] && !ctx->stage[i]) {
+      cudaError_t e = cudaMalloc(&ctx->stage[i], want[i]);
+      if (e != cudaSuccess) { (void)cudaGetLastError(); ctx->stage[i] = nullptr; return fail(ctx, SRA_ERR_OOM, "staging buffer allocation failed"); }
+    }
+  cudaStream_t st = cudaStream_t(cuda_stream);
+  cudaError_t e = cudaMemcpyAsync(ctx->stage[0], a->q_gen, gen_bytes, cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->stage[1], a->k_gen, gen_bytes, cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->stage[2], a->v_gen, gen_bytes, cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess && with_ref_rows) e = cudaMemcpyAsync(ctx->stage[4], a->q_ref, ref_bytes, cudaMemcpyHostToDevice, st);
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "host->device copy");
+  sra_fwd_args d{};
+  d.q_gen = ctx->stage[0]; d.k_gen = ctx->stage[1]; d.v_gen = ctx->stage[2]; d.o_gen = ctx->stage[3];
+  if (with_ref_rows) { d.q_ref = ctx->stage[4]; d.o_ref = ctx->stage[5]; }
+  d.lse_gen = a->lse_gen ? static_cast<float*>(ctx->stage[6]) : nullptr;
+  d.lse_ref = (with_ref_rows && a->lse_ref) ? static_cast<float*>(ctx->stage[7]) : nullptr;
+  if (int rc = sra_forward(ctx, &d, cuda_stream)) return rc;
+  e = cudaMemcpyAsync(a->o_gen, ctx->stage[3], gen_bytes, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess && with_ref_rows) e = cudaMemcpyAsync(a->o_ref, ctx->stage[5], ref_bytes, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess && d.lse_gen) e = cudaMemcpyAsync(a->lse_gen, d.lse_gen, lse_gen_bytes, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess && d.lse_ref) e = cudaMemcpyAsync(a->lse_ref, d.lse_ref, lse_ref_bytes, cudaMemcpyDeviceToHost, st);
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "device->host copy");
   return SRA_OK;
 }
 

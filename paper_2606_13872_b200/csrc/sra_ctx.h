@@ -28,6 +28,8 @@ struct sra_ctx {
   float* ws_dq = nullptr;     // fp32 [B, H, n_gen + n_ref, d] accumulators
   float* ws_delta = nullptr;  // fp32 [B, H, n_gen + n_ref]
   size_t ws_dq_bytes = 0;
+  // host-buffer staging of sra_forward_host (lazy): q,k,v,o gen; q,o ref; lse gen/ref
+  void* stage[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
   int64_t launches = 0;
   std::string err;
 };

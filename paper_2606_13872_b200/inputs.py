@@ -120,3 +120,20 @@ def bf16_bits(x: torch.Tensor):
     """The raw bf16 bit patterns of `x` as a numpy uint16 array (what the oracle consumes)."""
     assert x.dtype == torch.bfloat16 and x.device.type == "cpu"
     return x.contiguous().view(torch.int16).numpy().view("uint16")
+
+
+def make_tensor_device(w: SRAWorkload, tensor: str, device, step: int = 0, seed_offset: int = 0,
+                       n_tokens: Optional[int] = None) -> torch.Tensor:
+    """Same distribution and seeding rule as `make_tensor`, drawn by the DEVICE generator (bench.py at
+    full size: 720p tensors are 0.4 G elements each, too slow to draw on the host every run).  The byte
+    values differ from the CPU recipe; anything checked against the oracle copies these buffers back."""
+    k = TENSOR_ORDER.index(tensor)
+    is_gen = tensor.endswith("_gen")
+    n = n_tokens if n_tokens is not None else (w.n_gen if is_gen else w.n_ref)
+    seed = w.seed + seed_offset + k + (1000 * step if is_gen else 0)
+    g = torch.Generator(device).manual_seed(seed)
+    x = torch.randn(w.batch, n, w.heads, w.head_dim, generator=g, dtype=torch.float32, device=device)
+    scale = 1.0 if tensor.startswith("do_") else w.elem_scale(tensor)
+    if scale != 1.0:
+        x.mul_(scale)
+    return x.to(torch.bfloat16)

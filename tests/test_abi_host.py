@@ -1,0 +1,135 @@
+"""-m "not gpu": the C-ABI library loads, exports every symbol include/sra.h declares, validates its
+arguments, and its host-side tile schedule covers exactly the unmasked pairs of the
+explicit SRA mask.  No compute entry point is exercised here beyond its "no device" error path."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from oracle import sra_oracle
+from paper_2606_13872_b200 import binding as B
+from paper_2606_13872_b200 import inputs as sra_inputs
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared_symbols():
+    src = open(os.path.join(ROOT, "include", "sra.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(sra_[a-z_]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported():
+    names = _declared_symbols()
+    assert {"sra_create", "sra_cache_reference_kv", "sra_forward", "sra_backward", "sra_destroy"} <= set(names)
+    for n in names:
+        assert hasattr(B.lib, n), f"{n} declared in include/sra.h but not exported by libsra_b200.so"
+    assert set(names) == set(B.EXPORTS), (names, B.EXPORTS)
+
+
+def test_status_strings():
+    assert B.lib.sra_status_string(0) == b"SRA_OK"
+    assert B.lib.sra_status_string(-4) == b"SRA_ERR_NO_REF_CACHE"
+    assert B.lib.sra_status_string(-99) == b"SRA_ERR_UNKNOWN"
+
+
+@pytest.mark.parametrize("kw,status", [
+    (dict(head_dim=96), B.SRA_ERR_UNSUPPORTED),
+    (dict(batch=0), B.SRA_ERR_INVALID_ARG),
+    (dict(n_gen=0), B.SRA_ERR_INVALID_ARG),
+    (dict(ref_block_offsets=[0, 5, 5]), B.SRA_ERR_INVALID_ARG),
+    (dict(ref_block_offsets=[1, 5]), B.SRA_ERR_INVALID_ARG),
+    (dict(ref_block_offsets=[0, 7, 3]), B.SRA_ERR_INVALID_ARG),
+])
+def test_create_rejects_bad_configs(kw, status):
+    base = dict(batch=1, heads=2, head_dim=64, n_gen=10, ref_block_offsets=[0, 4, 9])
+    base.update(kw)
+    with pytest.raises(B.SRAError) as e:
+        B.sra_create(**base)
+    assert e.value.status == status
+
+
+def test_null_handling():
+    assert B.lib.sra_create(None, None) == B.SRA_ERR_INVALID_ARG
+    B.sra_destroy(None)  # NULL-safe
+    assert B.lib.sra_forward(None, None, None) == B.SRA_ERR_INVALID_ARG
+    assert B.lib.sra_backward(None, None, None) == B.SRA_ERR_INVALID_ARG
+    assert B.lib.sra_forward_host(None, None, None) == B.SRA_ERR_INVALID_ARG
+    assert B.lib.sra_cache_bytes(None) == 0
+
+
+def _covered_pairs(items, n_gen, n_ref):
+    """Pair-coverage count matrix implied by the schedule: rows/cols [G ; R]."""
+    n = n_gen + n_ref
+    C = np.zeros((n, n), dtype=np.int32)
+    for it in items:
+        r0 = it["q_row0"] + (n_gen if it["q_is_ref"] else 0)
+        rows = slice(r0, r0 + it["q_rows"])
+        s0 = it["seg0_start"] + (n_gen if it["seg0_is_ref"] else 0)
+        C[rows, s0:s0 + it["seg0_len"]] += 1
+        if it["seg1_len"]:
+            s1 = it["seg1_start"] + n_gen
+            C[rows, s1:s1 + it["seg1_len"]] += 1
+    return C
+
+
+@pytest.mark.parametrize("n_gen,blocks", [(256, (128,) * 4), (333, (1, 130, 257, 64, 200)), (1, (3,)), (700, ()),
+                                          (300, (77, 128, 129, 5)), (513, (600,))])
+def test_schedule_covers_exactly_the_mask(n_gen, blocks):
+    """Every unmasked (query, key) pair is covered exactly once; no masked pair is ever scheduled
+    ("eliminating redundant computation among tokens that do not require mutual interaction")."""
+    off = [0]
+    for b in blocks:
+        off.append(off[-1] + b)
+    ctx = B.sra_create(1, 1, 64, n_gen, off)
+    try:
+        items = B.sra_schedule_copy(ctx)
+        C = _covered_pairs(items, n_gen, off[-1])
+        M = sra_oracle.sra_mask(n_gen, off)
+        assert np.array_equal(C, M.astype(np.int32))
+        info = B.sra_schedule_info(ctx)
+        assert info["n_gen_items"] + info["n_ref_items"] == len(items)
+        for it in items:
+            assert 1 <= it["q_rows"] <= 256
+    finally:
+        B.sra_destroy(ctx)
+
+
+@pytest.mark.parametrize("name", ["tiny", "480p", "720p", "sweep40s", "train"])
+def test_useful_flops_closed_form(name):
+    """sra_useful_flops = 4 d pairs H B with pairs = N_g (N_g + N_r) + sum b_j^2 (tests/golden/pairs.txt)."""
+    w = sra_inputs.WORKLOADS[name]
+    ctx = B.sra_create(w.batch, w.heads, w.head_dim, w.n_gen, w.ref_block_offsets)
+    try:
+        pairs_g = w.n_gen * (w.n_gen + w.n_ref)
+        pairs_r = sum(b * b for b in w.ref_block_sizes)
+        f = 4.0 * w.head_dim * w.heads * w.batch
+        assert B.sra_useful_flops(ctx, True) == pytest.approx(f * (pairs_g + pairs_r), rel=1e-12)
+        assert B.sra_useful_flops(ctx, False) == pytest.approx(f * pairs_g, rel=1e-12)
+        assert B.sra_useful_flops(ctx, True, backward=True) == pytest.approx(2.5 * f * (pairs_g + pairs_r), rel=1e-12)
+        info = B.sra_schedule_info(ctx)
+        # tile counts: G slabs visit ceil(Ng/128)+ceil(Nr/128) key tiles per 128-row q tile
+        qt = -(-w.n_gen // 128)
+        assert info["key_tiles_gen"] == qt * (-(-w.n_gen // 128) + -(-w.n_ref // 128))
+    finally:
+        B.sra_destroy(ctx)
+
+
+def test_no_device_means_unsupported_not_fallback():
+    """On a box without a CUDA device every compute entry point must fail loudly (no CPU path)."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("CUDA device present")
+    ctx = B.sra_create(1, 1, 64, 8, [0, 4])
+    try:
+        a = B.sra_fwd_args()
+        assert B.lib.sra_forward(ctx, ctypes.byref(a), None) in (B.SRA_ERR_UNSUPPORTED, B.SRA_ERR_INVALID_ARG)
+        dummy = ctypes.c_void_p(16)
+        assert B.lib.sra_cache_reference_kv(ctx, dummy, dummy, None) == B.SRA_ERR_UNSUPPORTED
+        assert b"no CUDA device" in B.lib.sra_last_error(ctx)
+        bw = B.sra_bwd_args()
+        assert B.lib.sra_backward(ctx, ctypes.byref(bw), None) == B.SRA_ERR_UNSUPPORTED
+    finally:
+        B.sra_destroy(ctx)
