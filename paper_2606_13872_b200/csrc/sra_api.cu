@@ -218,6 +218,7 @@ void sra_destroy(sra_ctx* ctx) {
     cudaFree(ctx->cache_v);
     cudaFree(ctx->ws_dq);
     cudaFree(ctx->ws_delta);
+    cudaFree(ctx->ws_lse2);
     for (void* s : ctx->stage) cudaFree(s);
     (void)cudaGetLastError();
   }

@@ -47,4 +47,24 @@ struct FwdParams {
   int32_t ref_kv_head_major;
 };
 
+constexpr int kBwdQTile = 64;  // query rows per backward iteration (keys per CTA = kTile)
+
+struct BwdParams {
+  const BwdItem* items;
+  int32_t n_items;
+  int32_t heads, batch;
+  int32_t n_gen, n_ref;
+  int32_t n_pad;       // row length of the [G ; R]-concatenated fp32 workspaces (multiple of 64)
+  float scale_log2;    // softmax_scale * log2(e)
+  float scale;         // softmax_scale
+  const float* lse2;   // ws [B*H][n_pad]: LSE * log2(e)           (written by the preprocess kernel)
+  const float* delta;  // ws [B*H][n_pad]: D_i = sum_c dO_ic O_ic  (written by the preprocess kernel)
+  float* dq_ws;        // ws [B*H][n_pad][d] fp32 dQ accumulators (zeroed before the launch)
+  __nv_bfloat16* dk_gen;
+  __nv_bfloat16* dv_gen;
+  __nv_bfloat16* dk_ref;
+  __nv_bfloat16* dv_ref;
+  int32_t ref_kv_head_major;
+};
+
 }  // namespace sra

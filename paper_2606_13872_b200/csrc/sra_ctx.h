@@ -25,8 +25,9 @@ struct sra_ctx {
   __nv_bfloat16* cache_v = nullptr;
   bool cache_valid = false;
   // backward workspace (lazy)
-  float* ws_dq = nullptr;     // fp32 [B, H, n_gen + n_ref, d] accumulators
-  float* ws_delta = nullptr;  // fp32 [B, H, n_gen + n_ref]
+  float* ws_dq = nullptr;     // fp32 [B*H, n_pad, d] dQ accumulators
+  float* ws_delta = nullptr;  // fp32 [B*H, n_pad]   D_i
+  float* ws_lse2 = nullptr;   // fp32 [B*H, n_pad]   LSE_i * log2(e)
   size_t ws_dq_bytes = 0;
   // host-buffer staging of sra_forward_host (lazy): q,k,v,o gen; q,o ref; lse gen/ref
   void* stage[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
@@ -39,7 +40,8 @@ int ctx_fail(sra_ctx* ctx, int code, const std::string& msg);
 int ctx_fail_cuda(sra_ctx* ctx, cudaError_t e, const char* what);
 int make_tmap_bf16(sra_ctx* ctx, CUtensorMap* out, const void* ptr, int B, int N, int H, int d, bool head_major,
                    int box_rows);
-int make_tmap_f32(sra_ctx* ctx, CUtensorMap* out, const void* ptr, int B, int N, int H, int d, int box_rows);
+template <int D>
+cudaError_t launch_bwd(const CUtensorMap* maps, const BwdParams& p, cudaStream_t stream);
 template <int D>
 cudaError_t launch_fwd(const CUtensorMap* maps, const FwdParams& p, cudaStream_t stream);
 int run_backward(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t stream);

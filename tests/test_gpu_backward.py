@@ -1,0 +1,131 @@
+"""-m gpu parity tests of the SRA backward: CUDA path through the C ABI vs
+the fp64 oracle, per (batch, head), every row and column.
+
+Contract tolerance (BASELINE.json north_star): bf16 I/O, fp32 accumulation, GPU vs oracle max-abs <= 2e-2 and
+mean-abs <= 2e-3, plus the self-imposed relative gate rel_l2 <= 1e-2 per gradient tensor.
+The GPU backward consumes the GPU forward's own O (bf16) and LSE (fp32), as a training step would.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import c_oracle
+from paper_2606_13872_b200 import inputs as sra_inputs
+from tests.gpu_util import bits
+from tests.util import assert_parity
+
+pytestmark = pytest.mark.gpu
+
+GRADS = ("dq_gen", "dk_gen", "dv_gen", "dq_ref", "dk_ref", "dv_ref")
+
+
+def run_gpu_fwd_bwd(w, t, use_cache=False, scale=0.0):
+    """Forward (with LSE) then backward of workload `w` on cuda:0.  Returns dict of fp32 numpy gradients."""
+    from paper_2606_13872_b200 import binding as B
+    dev = torch.device("cuda:0")
+    g = {k: v.to(dev) for k, v in t.items()}
+    has_ref = w.n_ref > 0
+    ctx = B.sra_create(w.batch, w.heads, w.head_dim, w.n_gen, w.ref_block_offsets, scale)
+    try:
+        o_gen = torch.empty_like(g["q_gen"])
+        lse_gen = torch.empty((w.batch, w.heads, w.n_gen), device=dev)
+        o_ref = torch.empty_like(g["q_ref"]) if has_ref else None
+        lse_ref = torch.empty((w.batch, w.heads, w.n_ref), device=dev) if has_ref else None
+        if has_ref and use_cache:
+            B.sra_cache_reference_kv(ctx, g["k_ref"], g["v_ref"])
+        kr = None if (use_cache or not has_ref) else g["k_ref"]
+        vr = None if (use_cache or not has_ref) else g["v_ref"]
+        B.sra_forward(ctx, g["q_gen"], g["k_gen"], g["v_gen"], o_gen, q_ref=g.get("q_ref") if has_ref else None,
+                      k_ref=kr, v_ref=vr, o_ref=o_ref, lse_gen=lse_gen, lse_ref=lse_ref)
+        outs = {}
+        for n in GRADS:
+            if n.endswith("_ref") and not has_ref:
+                outs[n] = None
+            else:
+                outs[n] = torch.full_like(g["q_gen" if n.endswith("_gen") else "q_ref"], float("nan"))
+        B.sra_backward(ctx, q_gen=g["q_gen"], k_gen=g["k_gen"], v_gen=g["v_gen"],
+                       q_ref=g["q_ref"] if has_ref else None, k_ref=kr, v_ref=vr, o_gen=o_gen, o_ref=o_ref,
+                       lse_gen=lse_gen, lse_ref=lse_ref, do_gen=g["do_gen"], do_ref=g["do_ref"] if has_ref else None,
+                       **outs)
+        torch.cuda.synchronize()
+        return {n: (v.float().cpu().numpy() if v is not None else None) for n, v in outs.items()}
+    finally:
+        B.sra_destroy(ctx)
+
+
+def oracle_grads(w, tb, b, h, scale):
+    args = [tb.get(k) for k in ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref")]
+    o, lse = c_oracle.forward_head(*args, w.ref_block_offsets, scale, b, h)
+    return c_oracle.backward_head(*args, tb["do_gen"], tb.get("do_ref"), w.ref_block_offsets, scale, b, h, o, lse)
+
+
+def _check(w, got, tb, heads=None, what=""):
+    scale = 1.0 / math.sqrt(w.head_dim)
+    Ng = w.n_gen
+    ms = {}
+    for b in range(w.batch):
+        for h in (heads if heads is not None else range(w.heads)):
+            dq, dk, dv = oracle_grads(w, tb, b, h, scale)
+            for name, ref in (("dq", dq), ("dk", dk), ("dv", dv)):
+                parts = [got[name + "_gen"][b, :, h]]
+                if w.n_ref > 0:
+                    parts.append(got[name + "_ref"][b, :, h])
+                ms[(b, h, name)] = assert_parity(np.concatenate(parts, axis=0), ref, f"{what} b{b} h{h} {name}")
+                # generation and reference parts separately (a wrong R part can hide in a joint norm)
+                assert_parity(parts[0], ref[:Ng], f"{what} b{b} h{h} {name}_gen")
+                if w.n_ref > 0:
+                    assert_parity(parts[1], ref[Ng:], f"{what} b{b} h{h} {name}_ref")
+    return ms
+
+
+@pytest.mark.parametrize("use_cache", [False, True])
+def test_ragged_backward(use_cache):
+    """Non-uniform blocks (1, 130, 257, 64, 200), n_gen = 333, B2 H3 d128: ragged tails in every tile class."""
+    w = sra_inputs.WORKLOADS["ragged"]
+    t = sra_inputs.make_inputs(w, with_grad=True)
+    got = run_gpu_fwd_bwd(w, t, use_cache=use_cache)
+    _check(w, got, bits(t), what=f"ragged cache={use_cache}")
+
+
+def test_zero_ref_backward():
+    """n_ref == 0: plain self-attention backward vs torch fp64 autograd (library routine)."""
+    w = sra_inputs.SRAWorkload("noref", 1, 2, 128, 300, (), "B", 3)
+    t = sra_inputs.make_inputs(w, names=("q_gen", "k_gen", "v_gen", "do_gen"))
+    got = run_gpu_fwd_bwd(w, t)
+    q, k, v = (t[n].double().permute(0, 2, 1, 3).requires_grad_(True) for n in ("q_gen", "k_gen", "v_gen"))
+    o = torch.nn.functional.scaled_dot_product_attention(q, k, v)
+    (o * t["do_gen"].double().permute(0, 2, 1, 3)).sum().backward()
+    for name, leaf in (("dq_gen", q), ("dk_gen", k), ("dv_gen", v)):
+        assert_parity(got[name], leaf.grad.permute(0, 2, 1, 3).numpy(), f"zero-ref {name}")
+
+
+def test_mini_train_backward():
+    """Real 1560-token block structure scaled down (B2 H2, 1860 gen + 2x1560 ref, dist B as configs[4])."""
+    w = sra_inputs.WORKLOADS["mini_train"]
+    t = sra_inputs.make_inputs(w, with_grad=True)
+    got = run_gpu_fwd_bwd(w, t)
+    _check(w, got, bits(t), what="mini_train")
+
+
+def test_backward_mask_poison():
+    """a huge dO_r must leave dK_g, dV_g, dQ_g bit-identical (R rows never see G keys), and
+    dK_r/dV_r of blocks other than the perturbed one bit-identical up to the dQ-independent parts."""
+    w = sra_inputs.WORKLOADS["ragged"]
+    t = sra_inputs.make_inputs(w, with_grad=True)
+    base = run_gpu_fwd_bwd(w, t)
+    off = w.ref_block_offsets
+    tp = {k: v.clone() for k, v in t.items()}
+    j = 2
+    tp["do_ref"][:, off[j]:off[j + 1]] *= 1000.0
+    pois = run_gpu_fwd_bwd(w, tp)
+    for name in ("dk_gen", "dv_gen"):
+        assert np.array_equal(base[name], pois[name]), f"{name} changed when dO_r was perturbed"
+    for jj in range(len(off) - 1):
+        if jj == j:
+            continue
+        sl = slice(off[jj], off[jj + 1])
+        for name in ("dk_ref", "dv_ref"):
+            assert np.array_equal(base[name][:, sl], pois[name][:, sl]), f"{name} block {jj} changed"
+    assert not np.array_equal(base["dv_ref"][:, off[j]:off[j + 1]], pois["dv_ref"][:, off[j]:off[j + 1]])
