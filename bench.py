@@ -400,12 +400,181 @@ def bench_ours(args, w):
         dist.destroy_process_group()
 
 
+def bench_train(args, w):
+    """--mode train (BASELINE.json configs[4]): one step = sra_forward (fresh reference K/V, LSE written) +
+    sra_backward (a6 + a7 + a8) on the workload; value = useful fwd+bwd TFLOP/s (3.5 x forward FLOPs)."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2606_13872_b200 import binding as B
+    from paper_2606_13872_b200 import dp
+    from paper_2606_13872_b200 import inputs as I
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the SRA path has no CPU fallback")
+    if w.head_dim != 128 or w.n_ref == 0:
+        raise SystemExit("bench.py --mode train: needs head_dim 128 and a reference (configs[4] shape)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    peaks, peaks_kind = load_peaks()
+    b0, _ = dp.shard_batch(w.batch, world, rank)
+    seed_off = dp.unit_seed(0, b0)
+    t = {n: I.make_tensor_device(w, n, dev, seed_offset=seed_off) for n in I.TENSOR_ORDER}
+    o_gen, o_ref = torch.empty_like(t["q_gen"]), torch.empty_like(t["q_ref"])
+    lse_gen = torch.empty((w.batch, w.heads, w.n_gen), device=dev, dtype=torch.float32)
+    lse_ref = torch.empty((w.batch, w.heads, w.n_ref), device=dev, dtype=torch.float32)
+    grads = {n: torch.empty_like(t["q_gen" if n.endswith("_gen") else "q_ref"])
+             for n in ("dq_gen", "dk_gen", "dv_gen", "dq_ref", "dk_ref", "dv_ref")}
+    ctx = B.sra_create(w.batch, w.heads, w.head_dim, w.n_gen, w.ref_block_offsets)
+    B.sra_set_kernel_timing(ctx, True)
+    fl_f, fl_b = useful_flops(w), useful_flops(w, backward=True)
+    assert abs(B.sra_useful_flops(ctx, True, True) - fl_b) <= 1e-6 * fl_b
+
+    def fwd():
+        B.sra_forward(ctx, t["q_gen"], t["k_gen"], t["v_gen"], o_gen, q_ref=t["q_ref"], k_ref=t["k_ref"],
+                      v_ref=t["v_ref"], o_ref=o_ref, lse_gen=lse_gen, lse_ref=lse_ref)
+
+    def bwd():
+        B.sra_backward(ctx, q_gen=t["q_gen"], k_gen=t["k_gen"], v_gen=t["v_gen"], q_ref=t["q_ref"], k_ref=t["k_ref"],
+                       v_ref=t["v_ref"], o_gen=o_gen, o_ref=o_ref, lse_gen=lse_gen, lse_ref=lse_ref,
+                       do_gen=t["do_gen"], do_ref=t["do_ref"], **grads)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        fwd(); bwd()
+    barrier()
+    launches0 = B.sra_launch_count(ctx)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    k_ms = {k: [] for k in ("fwd", "bwd_pre", "bwd_main", "bwd_fin")}
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        fwd(); bwd()
+    e1.record()
+    barrier()
+    # per-kernel device times of the LAST timed step (the library brackets each launch with CUDA events on the
+    # launching stream; reading them earlier would synchronise inside the timed loop)
+    for k, which in (("fwd", B.KERNEL_FWD), ("bwd_pre", B.KERNEL_BWD_PREPROCESS), ("bwd_main", B.KERNEL_BWD_MAIN),
+                     ("bwd_fin", B.KERNEL_BWD_DQ_FINALIZE)):
+        k_ms[k].append(B.sra_kernel_time_ms(ctx, which))
+    clocks = sampler.stop() if rank == 0 else None
+    launches = B.sra_launch_count(ctx) - launches0
+    elapsed_ms = dp.max_over_ranks(e0.elapsed_time(e1), dev)
+    total_fl = dp.sum_over_ranks((fl_f + fl_b) * args.steps, dev)
+    value = total_fl / (elapsed_ms * 1e-3) / 1e12
+
+    parity = None
+    if rank == 0 and world == 1 and args.train_parity:
+        parity = train_parity(w, t, grads, dev)
+    B.sra_destroy(ctx)
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    km = {k: statistics.mean(v) for k, v in k_ms.items()}
+    achieved = fl_b / (km["bwd_main"] * 1e-3) / 1e12
+    peak = peaks["bf16_tflops_sustained"]
+    roofline = {
+        "bound": "tensor", "kernel": "sra_bwd_kernel<128>", "achieved": achieved, "peak": peak, "unit": UNIT,
+        "frac": achieved / peak,
+        "peak_kind": f"{peaks_kind} cuBLAS bf16, sustained (kernel timed inside a seconds-long step loop)",
+        "frac_of_burst": achieved / peaks["bf16_tflops"], "peak_burst": peaks["bf16_tflops"],
+        "frac_of_nominal": achieved / NOMINAL_BF16_TFLOPS, "peak_nominal": NOMINAL_BF16_TFLOPS,
+        "kernel_ms": km["bwd_main"], "algorithmic_flops_per_launch": fl_b,
+        "traffic": (load_traffic_all().get(w.name, {}) or {}).get("sra_bwd_kernel_dram_bytes"),
+        "kernel_ms_all": km,
+        "fwd_kernel": {"achieved": fl_f / (km["fwd"] * 1e-3) / 1e12, "frac": fl_f / (km["fwd"] * 1e-3) / 1e12 / peak,
+                       "kernel_ms": km["fwd"], "algorithmic_flops_per_launch": fl_f},
+    }
+    cfg = config_of(w, args)
+    cfg["step"] = "sra_forward (fresh reference K/V, LSE) + sra_backward (preprocess + main + dQ finalise): one DiT attention layer fwd+bwd"
+    out = {
+        "metric": "sra_train_useful_tflops", "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "bf16", "data": "synthetic", "config": cfg,
+        "pct_of_peak": {"measured_sustained": 100 * value / world / peaks["bf16_tflops_sustained"],
+                        "measured_burst": 100 * value / world / peaks["bf16_tflops"],
+                        "nominal_2250": 100 * value / world / NOMINAL_BF16_TFLOPS},
+        "e2e": None, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": None,
+        "parity": parity,
+    }
+    print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def train_parity(w, t, grads, dev, b=0, h=0, n_rows=48, n_cols=48):
+    """Backward parity at full size (slow: the oracle needs the forward of EVERY row of one (b, h) - ~1 TFLOP of
+    fp64 - before it can give dK/dV of sampled keys): sampled query rows for dQ, sampled key columns for dK/dV."""
+    import numpy as np
+    from oracle import c_oracle
+    from paper_2606_13872_b200 import inputs as I
+    c_oracle.build()
+    t0 = time.perf_counter()
+    bits = {n: I.bf16_bits(t[n][b:b + 1, :, h:h + 1].contiguous().cpu()) for n in I.TENSOR_ORDER}
+    args6 = [bits[k] for k in ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref")]
+    scale = 1.0 / math.sqrt(w.head_dim)
+    o, lse = c_oracle.forward_head(*args6, w.ref_block_offsets, scale, 0, 0)
+    rng = np.random.default_rng(1)
+    n = w.n_gen + w.n_ref
+    off = w.ref_block_offsets
+    edge = [0, 63, 64, 127, 128, w.n_gen - 1, w.n_gen, w.n_gen + off[1] - 1, w.n_gen + off[1], n - 1]
+    rows = np.asarray(sorted(set(edge) | set(int(x) for x in rng.integers(0, n, n_rows))), dtype=np.int32)
+    cols = np.asarray(sorted(set(edge) | set(int(x) for x in rng.integers(0, n, n_cols))), dtype=np.int32)
+    dq, dk, dv = c_oracle.backward_head(*args6, bits["do_gen"], bits["do_ref"], off, scale, 0, 0, o, lse, rows=rows,
+                                        cols=cols)
+    res = {"b": b, "h": h, "rows": int(len(rows)), "cols": int(len(cols)), "oracle_seconds": time.perf_counter() - t0,
+           "tolerance": {"max_abs": MAX_ABS_TOL, "mean_abs": MEAN_ABS_TOL, "rel_l2": REL_L2_TOL}}
+    ok = True
+    for name, ref, idx in (("dq", dq, rows), ("dk", dk, cols), ("dv", dv, cols)):
+        gi = idx[idx < w.n_gen]
+        ri = idx[idx >= w.n_gen] - w.n_gen
+        got = np.concatenate([grads[name + "_gen"][b, :, h][torch_index(gi, dev)].float().cpu().numpy(),
+                              grads[name + "_ref"][b, :, h][torch_index(ri, dev)].float().cpu().numpy()], axis=0)
+        diff = np.abs(got - ref)
+        rel = float(np.linalg.norm(got - ref) / max(np.linalg.norm(ref), 1e-300))
+        res[name] = {"max_abs": float(diff.max()), "mean_abs": float(diff.mean()), "rel_l2": rel}
+        ok = ok and bool(np.isfinite(got).all() and diff.max() <= MAX_ABS_TOL and diff.mean() <= MEAN_ABS_TOL
+                         and rel <= REL_L2_TOL)
+    res["ok"] = ok
+    return res
+
+
+def torch_index(idx, dev):
+    import torch
+    return torch.as_tensor(idx, device=dev).long()
+
+
+def load_traffic_all():
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return json.load(f)
+    except Exception:
+        return {}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="720p")
+    ap.add_argument("--workload", default=None, help="default: 720p (--mode fwd), train (--mode train)")
+    ap.add_argument("--mode", default="fwd", choices=["fwd", "train"],
+                    help="fwd: the BASELINE metric (forward layer); train: configs[4] forward + backward")
+    ap.add_argument("--train-parity", action="store_true",
+                    help="--mode train: also check dQ/dK/dV of one (batch, head) against the oracle (minutes of CPU)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-oracle", action="store_true", help="skip the cpu_baseline / parity legs")
     ap.add_argument("--oracle-rows", type=int, default=192, help="generation rows in the oracle sample")
@@ -413,7 +582,7 @@ def main():
     if args.warmup < 3 and args.impl == "ours":
         log("note: W < 3 warm-up steps breaks the timing rules; use --warmup >= 3 for a reportable number")
     from paper_2606_13872_b200 import inputs as I
-    w = I.WORKLOADS[args.workload]
+    w = I.WORKLOADS[args.workload or ("train" if args.mode == "train" else "720p")]
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if world != args.gpus and world > 1:
         log(f"note: --gpus {args.gpus} but WORLD_SIZE={world}; using WORLD_SIZE")
@@ -421,6 +590,8 @@ def main():
         if int(os.environ.get("RANK", "0")) != 0:
             return
         bench_reference(args, w)
+    elif args.mode == "train":
+        bench_train(args, w)
     else:
         bench_ours(args, w)
 

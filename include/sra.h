@@ -153,6 +153,19 @@ int sra_schedule_copy(const sra_ctx* ctx, int32_t* items, int32_t capacity, int3
 /* Device bytes held by the resident reference-KV cache (0 before the first cache call). */
 int64_t sra_cache_bytes(const sra_ctx* ctx);
 
+/* Optional per-kernel device timing (bench.py's roofline leg): when enabled, every launch is bracketed by
+ * CUDA events recorded on the launching stream.  sra_kernel_time_ms returns the duration of the LAST launch
+ * of kernel `which` (it synchronises on that launch's end event); SRA_ERR_INVALID_ARG if timing is off or the
+ * kernel has not been launched since it was switched on. */
+#define SRA_KERNEL_CACHE_RELAYOUT 0 /* a1 */
+#define SRA_KERNEL_FWD 1            /* a3-a5 */
+#define SRA_KERNEL_BWD_PREPROCESS 2 /* a6 */
+#define SRA_KERNEL_BWD_MAIN 3       /* a7 */
+#define SRA_KERNEL_BWD_DQ_FINALIZE 4 /* a8 */
+#define SRA_NUM_KERNELS 5
+int sra_set_kernel_timing(sra_ctx* ctx, int enable);
+int sra_kernel_time_ms(sra_ctx* ctx, int which, float* ms);
+
 /* Kernels launched by this ctx since creation (bench.py's gpu_launches). */
 int64_t sra_launch_count(const sra_ctx* ctx);
 

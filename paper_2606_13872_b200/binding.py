@@ -24,7 +24,7 @@ SRA_ERR_OOM = -5
 EXPORTS = (
     "sra_create", "sra_cache_reference_kv", "sra_forward", "sra_forward_host", "sra_backward", "sra_destroy", "sra_useful_flops",
     "sra_schedule_info", "sra_schedule_copy", "sra_cache_bytes", "sra_launch_count", "sra_status_string",
-    "sra_last_error",
+    "sra_last_error", "sra_set_kernel_timing", "sra_kernel_time_ms",
 )
 
 if not os.path.exists(LIB_PATH):
@@ -85,6 +85,10 @@ lib.sra_cache_bytes.argtypes = [_ctx_p]
 lib.sra_cache_bytes.restype = ctypes.c_int64
 lib.sra_launch_count.argtypes = [_ctx_p]
 lib.sra_launch_count.restype = ctypes.c_int64
+lib.sra_set_kernel_timing.argtypes = [_ctx_p, ctypes.c_int]
+lib.sra_set_kernel_timing.restype = ctypes.c_int
+lib.sra_kernel_time_ms.argtypes = [_ctx_p, ctypes.c_int, ctypes.POINTER(ctypes.c_float)]
+lib.sra_kernel_time_ms.restype = ctypes.c_int
 lib.sra_status_string.argtypes = [ctypes.c_int]
 lib.sra_status_string.restype = ctypes.c_char_p
 lib.sra_last_error.argtypes = [_ctx_p]
@@ -199,6 +203,19 @@ def sra_schedule_copy(ctx: int):
 
 def sra_cache_bytes(ctx: int) -> int:
     return int(lib.sra_cache_bytes(ctx))
+
+
+KERNEL_CACHE_RELAYOUT, KERNEL_FWD, KERNEL_BWD_PREPROCESS, KERNEL_BWD_MAIN, KERNEL_BWD_DQ_FINALIZE = range(5)
+
+
+def sra_set_kernel_timing(ctx: int, enable: bool) -> None:
+    _check(lib.sra_set_kernel_timing(ctx, int(enable)), ctx)
+
+
+def sra_kernel_time_ms(ctx: int, which: int) -> float:
+    ms = ctypes.c_float()
+    _check(lib.sra_kernel_time_ms(ctx, int(which), ctypes.byref(ms)), ctx)
+    return ms.value
 
 
 def sra_launch_count(ctx: int) -> int:

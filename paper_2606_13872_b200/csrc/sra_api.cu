@@ -220,6 +220,9 @@ void sra_destroy(sra_ctx* ctx) {
     cudaFree(ctx->ws_delta);
     cudaFree(ctx->ws_lse2);
     for (void* s : ctx->stage) cudaFree(s);
+    for (auto& e : ctx->ev)
+      for (cudaEvent_t x : e)
+        if (x) cudaEventDestroy(x);
     (void)cudaGetLastError();
   }
   delete ctx;
@@ -252,10 +255,14 @@ int sra_cache_reference_kv(sra_ctx* ctx, const void* k_ref, const void* v_ref, v
   const size_t total = elems / 8;
   const int threads = 256;
   const int blocks = int(std::min<size_t>((total + threads - 1) / threads, size_t(148) * 16));
-  sra::relayout_head_major_kernel<<<blocks, threads, 0, cudaStream_t(cuda_stream)>>>(
-      static_cast<const uint4*>(k_ref), static_cast<const uint4*>(v_ref), reinterpret_cast<uint4*>(ctx->cache_k),
-      reinterpret_cast<uint4*>(ctx->cache_v), c.n_ref, c.heads, vec, total);
-  cudaError_t e = cudaGetLastError();
+  cudaError_t e;
+  {
+    sra::KernelTimer kt(ctx, SRA_KERNEL_CACHE_RELAYOUT, cudaStream_t(cuda_stream));
+    sra::relayout_head_major_kernel<<<blocks, threads, 0, cudaStream_t(cuda_stream)>>>(
+        static_cast<const uint4*>(k_ref), static_cast<const uint4*>(v_ref), reinterpret_cast<uint4*>(ctx->cache_k),
+        reinterpret_cast<uint4*>(ctx->cache_v), c.n_ref, c.heads, vec, total);
+    e = cudaGetLastError();
+  }
   if (e != cudaSuccess) return fail_cuda(ctx, e, "cache relayout launch");
   ctx->launches += 1;
   ctx->cache_valid = true;
@@ -303,8 +310,12 @@ int sra_forward(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) {
   p.lse_gen = a->lse_gen;
   p.lse_ref = a->lse_ref;
   p.ref_kv_head_major = use_cache ? 1 : 0;
-  cudaError_t e = (d == 128) ? sra::launch_fwd<128>(maps, p, cudaStream_t(cuda_stream))
-                             : sra::launch_fwd<64>(maps, p, cudaStream_t(cuda_stream));
+  cudaError_t e;
+  {
+    sra::KernelTimer kt(ctx, SRA_KERNEL_FWD, cudaStream_t(cuda_stream));
+    e = (d == 128) ? sra::launch_fwd<128>(maps, p, cudaStream_t(cuda_stream))
+                   : sra::launch_fwd<64>(maps, p, cudaStream_t(cuda_stream));
+  }
   if (e != cudaSuccess) return fail_cuda(ctx, e, "sra_fwd_kernel launch");
   ctx->launches += 1;
   return SRA_OK;
@@ -404,6 +415,29 @@ int64_t sra_cache_bytes(const sra_ctx* ctx) {
   if (!ctx || !ctx->cache_k) return 0;
   const sra_config& c = ctx->cfg;
   return int64_t(2) * c.batch * c.n_ref * c.heads * c.head_dim * 2;
+}
+
+int sra_set_kernel_timing(sra_ctx* ctx, int enable) {
+  if (!ctx) return SRA_ERR_INVALID_ARG;
+  ctx->err.clear();
+  if (int rc = check_device(ctx)) return rc;
+  if (enable && !ctx->ev[0][0]) {
+    for (auto& e : ctx->ev)
+      for (cudaEvent_t& x : e)
+        if (cudaEventCreate(&x) != cudaSuccess) return fail(ctx, SRA_ERR_CUDA, "cudaEventCreate failed");
+  }
+  ctx->timing = enable != 0;
+  for (bool& r : ctx->ev_recorded) r = false;
+  return SRA_OK;
+}
+
+int sra_kernel_time_ms(sra_ctx* ctx, int which, float* ms) {
+  if (!ctx || !ms || which < 0 || which >= SRA_NUM_KERNELS) return SRA_ERR_INVALID_ARG;
+  if (!ctx->timing || !ctx->ev_recorded[which]) return fail(ctx, SRA_ERR_INVALID_ARG, "kernel timing is off or the kernel was not launched");
+  cudaError_t e = cudaEventSynchronize(ctx->ev[which][1]);
+  if (e == cudaSuccess) e = cudaEventElapsedTime(ms, ctx->ev[which][0], ctx->ev[which][1]);
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaEventElapsedTime");
+  return SRA_OK;
 }
 
 int64_t sra_launch_count(const sra_ctx* ctx) { return ctx ? ctx->launches : 0; }

@@ -549,6 +549,7 @@ int run_backward(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t stream) {
     const size_t rows = size_t(B) * n_cat * H;
     const int threads = 256;
     const int blocks = int(std::min<size_t>((rows * 32 + threads - 1) / threads, size_t(148) * 32));
+    KernelTimer kt(ctx, SRA_KERNEL_BWD_PREPROCESS, stream);
     sra_bwd_preprocess_kernel<128><<<blocks, threads, 0, stream>>>(
         static_cast<const __nv_bfloat16*>(a->o_gen), static_cast<const __nv_bfloat16*>(a->do_gen), a->lse_gen,
         static_cast<const __nv_bfloat16*>(a->o_ref), static_cast<const __nv_bfloat16*>(a->do_ref), a->lse_ref,
@@ -583,13 +584,18 @@ int run_backward(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t stream) {
   p.dk_gen = static_cast<__nv_bfloat16*>(a->dk_gen); p.dv_gen = static_cast<__nv_bfloat16*>(a->dv_gen);
   p.dk_ref = static_cast<__nv_bfloat16*>(a->dk_ref); p.dv_ref = static_cast<__nv_bfloat16*>(a->dv_ref);
   p.ref_kv_head_major = use_cache ? 1 : 0;
-  if ((e = launch_bwd<128>(m, p, stream)) != cudaSuccess) return ctx_fail_cuda(ctx, e, "sra_bwd_kernel launch");
+  {
+    KernelTimer kt(ctx, SRA_KERNEL_BWD_MAIN, stream);
+    e = launch_bwd<128>(m, p, stream);
+  }
+  if (e != cudaSuccess) return ctx_fail_cuda(ctx, e, "sra_bwd_kernel launch");
   ctx->launches += 1;
 
   {  // a8
     const size_t total = size_t(B) * H * n_cat * (d / 8);
     const int threads = 256;
     const int blocks = int(std::min<size_t>((total + threads - 1) / threads, size_t(148) * 32));
+    KernelTimer kt(ctx, SRA_KERNEL_BWD_DQ_FINALIZE, stream);
     sra_bwd_dq_finalize_kernel<128><<<blocks, threads, 0, stream>>>(ctx->ws_dq, static_cast<__nv_bfloat16*>(a->dq_gen),
                                                                    static_cast<__nv_bfloat16*>(a->dq_ref), B, H, c.n_gen,
                                                                    c.n_ref, n_pad, ctx->scale);

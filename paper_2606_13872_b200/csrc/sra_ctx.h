@@ -32,10 +32,29 @@ struct sra_ctx {
   // host-buffer staging of sra_forward_host (lazy): q,k,v,o gen; q,o ref; lse gen/ref
   void* stage[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
   int64_t launches = 0;
+  // optional per-kernel timing (sra_set_kernel_timing)
+  bool timing = false;
+  cudaEvent_t ev[SRA_NUM_KERNELS][2] = {};
+  bool ev_recorded[SRA_NUM_KERNELS] = {};
   std::string err;
 };
 
 namespace sra {
+// Brackets one kernel launch with CUDA events on its stream when ctx->timing is on.
+struct KernelTimer {
+  sra_ctx* ctx;
+  int id;
+  cudaStream_t stream;
+  KernelTimer(sra_ctx* c, int which, cudaStream_t s) : ctx(c), id(which), stream(s) {
+    if (ctx->timing) cudaEventRecord(ctx->ev[id][0], stream);
+  }
+  ~KernelTimer() {
+    if (ctx->timing) {
+      cudaEventRecord(ctx->ev[id][1], stream);
+      ctx->ev_recorded[id] = true;
+    }
+  }
+};
 int ctx_fail(sra_ctx* ctx, int code, const std::string& msg);
 int ctx_fail_cuda(sra_ctx* ctx, cudaError_t e, const char* what);
 int make_tmap_bf16(sra_ctx* ctx, CUtensorMap* out, const void* ptr, int B, int N, int H, int d, bool head_major,
