@@ -193,6 +193,29 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* r) {
 }
 
 // ------------------------------------------------------------------ misc
+// True in exactly one lane of a fully converged warp.  Unlike `lane == 0`, ptxas knows the guarded
+// region is single-lane, so uniform-datapath instructions (UTCHMMA, UTMALDG) are emitted without a
+// per-lane serialisation loop.
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "elect.sync _|p, 0xffffffff;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t"
+      "}"
+      : "=r"(pred));
+  return pred != 0;
+}
+// 64-bit shared-memory matrix descriptor from a precomputed low word (address and LBO fields) and the
+// constant high word (SBO, version, swizzle); stepping along K or to another stage is one 32-bit add.
+__host__ __device__ constexpr uint32_t desc_hi_sw128(uint32_t sbo_bytes) {
+  return ((sbo_bytes >> 4) & 0x3FFF) | (1u << 14) | (2u << 29);
+}
+__device__ __forceinline__ uint32_t desc_lo(uint32_t smem_addr, uint32_t lbo_bytes) {
+  return ((smem_addr >> 4) & 0x3FFF) | (((lbo_bytes >> 4) & 0x3FFF) << 16);
+}
+__device__ __forceinline__ uint64_t desc64(uint32_t lo, uint32_t hi) { return (uint64_t(hi) << 32) | lo; }
 template <int N>
 __device__ __forceinline__ void reg_inc() {
   asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N));
@@ -205,6 +228,58 @@ __device__ __forceinline__ float ex2(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
+}
+// Packed fp32 pairs (sm_100 FFMA2 / FADD2): one issue slot for two lanes of work.
+__device__ __forceinline__ uint64_t pack2(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void unpack2(uint64_t v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+__device__ __forceinline__ uint64_t sub2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+__device__ __forceinline__ uint64_t mul2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+// 2^x for a pair, on the FMA/ALU pipes instead of MUFU (x <= ~100; x is clamped at -125 so the
+// exponent arithmetic cannot wrap).  Round-to-nearest split x = n + r, r in [-0.5, 0.5]; degree-3
+// minimax polynomial for 2^r (max rel. error 7.5e-5, far below the bf16 rounding of P), then n is
+// added into the exponent field.  The magic constant 1.5 * 2^23 leaves n in the low mantissa bits
+// of x + magic, and (bits << 23) drops everything but n.
+__device__ __forceinline__ void ex2_emu2(uint64_t x, float& p0, float& p1) {
+  float x0, x1;
+  unpack2(x, x0, x1);
+  x0 = fmaxf(x0, -125.0f);
+  x1 = fmaxf(x1, -125.0f);
+  const uint64_t xc = pack2(x0, x1);
+  const uint64_t magic = pack2(12582912.0f, 12582912.0f);
+  const uint64_t xr = add2(xc, magic);
+  const uint64_t r = sub2(xc, sub2(xr, magic));
+  uint64_t p = fma2(pack2(0.05517149344086647f, 0.05517149344086647f), r, pack2(0.24261094629764557f, 0.24261094629764557f));
+  p = fma2(p, r, pack2(0.6932609677314758f, 0.6932609677314758f));
+  p = fma2(p, r, pack2(0.9999280571937561f, 0.9999280571937561f));
+  float q0, q1, n0, n1;
+  unpack2(p, q0, q1);
+  unpack2(xr, n0, n1);
+  p0 = __int_as_float(__float_as_int(q0) + (__float_as_int(n0) << 23));
+  p1 = __int_as_float(__float_as_int(q1) + (__float_as_int(n1) << 23));
 }
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
   uint32_t r;
@@ -221,6 +296,11 @@ __device__ __forceinline__ float4 ld_shared_f4(uint32_t addr) {
 }
 __device__ __forceinline__ void st_shared_f32(uint32_t addr, float v) {
   asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
+}
+__device__ __forceinline__ float ld_shared_f32(uint32_t addr) {
+  float v;
+  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr) : "memory");
+  return v;
 }
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");

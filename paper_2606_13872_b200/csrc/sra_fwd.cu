@@ -18,6 +18,14 @@
 
 namespace sra {
 
+// Of every 8 column pairs of a score tile, this many take their exp2 on the FMA/ALU pipes
+// (ex2_emu2) instead of MUFU: per key tile the two MMAs and the 16 K MUFU exponentials need the
+// same number of SM cycles, so without the split the softmax sits on the critical path.
+#ifndef SRA_FWD_EMU
+#define SRA_FWD_EMU 3
+#endif
+constexpr int kEmuPairsPer8 = SRA_FWD_EMU;
+
 template <int D>
 struct FwdCfg {
   static constexpr int kTileBytes = kTile * D * 2;          // one Q/K/V tile in smem
@@ -25,7 +33,8 @@ struct FwdCfg {
   static constexpr int kBoxBytes = kTile * 128;              // 16 KB
   static constexpr int kStages = (D == 128) ? 5 : 10;        // K/V ring depth (tiles)
   static constexpr int kNumBars = 1 + 2 * kStages + 6;
-  static constexpr int kSmemBytes = 1024 /*align slack*/ + (2 + kStages) * kTileBytes + kNumBars * 8 + 16;
+  static constexpr int kXchBytes = 2 * 2 * kTile * 4;       // (slot, half, row) floats swapped by the two threads of a row
+  static constexpr int kSmemBytes = (2 + kStages) * kTileBytes + kNumBars * 8 + 16 + kXchBytes;
   static constexpr int kTmemCols = 512;
   static constexpr int kThreads = 384;
 };
@@ -49,8 +58,9 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
                    const __grid_constant__ CUtensorMap tm_k_ref, const __grid_constant__ CUtensorMap tm_v_ref,
                    const FwdParams p) {
   using C = FwdCfg<D>;
-  extern __shared__ uint8_t smem_raw[];
-  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  extern __shared__ __align__(1024) uint8_t smem_raw[];  // 128-byte-swizzled tiles need 1024-byte alignment
+  const uint32_t smem_base = smem_u32(smem_raw);
+  if ((smem_base & 1023u) != 0) __trap();
   const uint32_t sQ = smem_base;                         // 2 tiles
   const uint32_t sKV = smem_base + 2 * C::kTileBytes;    // kStages tiles
   const uint32_t sBar = sKV + C::kStages * C::kTileBytes;
@@ -61,6 +71,7 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
   const uint32_t bar_p_full = bar_s_full + 16;
   const uint32_t bar_o_full = bar_p_full + 16;
   const uint32_t s_tmem_ptr = bar_o_full + 16;
+  const uint32_t sXch = s_tmem_ptr + 16;
   uint32_t* tmem_ptr_generic = reinterpret_cast<uint32_t*>(smem_raw + (s_tmem_ptr - smem_u32(smem_raw)));
 
   const int warp = threadIdx.x >> 5;
@@ -82,7 +93,7 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
     }
     for (int i = 0; i < 2; ++i) {
       mbar_init(bar_s_full + 8 * i, 1);
-      mbar_init(bar_p_full + 8 * i, 128);
+      mbar_init(bar_p_full + 8 * i, 256);
       mbar_init(bar_o_full + 8 * i, 1);
     }
     fence_mbar_init();
@@ -100,53 +111,54 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
   const uint32_t tS0 = tmem, tO0 = tmem + 256;
 
   if (warp < 8) {
-    // ======================================================= softmax warpgroups
+    // ======================================================= softmax warps
+    // Warps w and w + 4 sit on the same SM sub-partition and own the same 32 TMEM lanes (query rows);
+    // warp w takes key columns [0, 64) of every score tile, warp w + 4 columns [64, 128), for BOTH Q
+    // tiles in turn.  Two warps per sub-partition work on one tile at a time, so the hardware scheduler
+    // interleaves their MUFU / FMA / ALU streams (one warp alone issues its exp2 back to back and leaves
+    // the other pipes idle), and the softmax of a tile takes about half as long, which is what bounds the
+    // S -> P -> PV -> QK dependency ring of that tile.
     reg_inc<224>();
-    const int i = warp >> 2;  // Q tile of this warpgroup
-    if (i < n_qt) {
-      const uint32_t lane_off = uint32_t((warp & 3) * 32) << 16;
-      const uint32_t tS = tS0 + i * 128 + lane_off;
-      const uint32_t tO = tO0 + i * D + lane_off;
-      const float sl2 = p.scale_log2;
-      float m_ref = -INFINITY;  // reference max of the raw scores (lazily updated)
-      float l = 0.f;            // running sum of exp2((s - m_ref) * sl2)
-      for (int j = 0; j < n_kv; ++j) {
-        const int n_valid = (j < n0) ? min(kTile, item.seg0_len - j * kTile) : min(kTile, item.seg1_len - (j - n0) * kTile);
-        mbar_wait(bar_s_full + 8 * i, j & 1);
-        tc_fence_after();
-        uint32_t s[4][32];
+    const int hh = warp >> 2;  // column half
+    const int row_in_tile = (warp & 3) * 32 + lane;
+    const uint32_t lane_off = uint32_t((warp & 3) * 32) << 16;
+    const float sl2 = p.scale_log2;
+    // Online softmax with a *lagging* lazy rescale.  m_ref is the reference max the exponentials are
+    // taken against; it is stale on purpose: P = exp2((s - m_ref) * sl2) is exact for any m_ref (bf16 and
+    // fp32 keep their relative precision), so a tile never waits for its own row max before its first
+    // exp2.  The tile max mt is reduced alongside the exponentials (FMNMX3 in the shadow of MUFU) and
+    // only (a) moves m_ref at the start of a later tile once it leads by more than 2^8 (O and l are
+    // rescaled then), (b) forces a second, exact pass over this tile when it leads by more than 2^64
+    // (always on the first tile, where m_ref = -inf; otherwise only for adversarial score jumps).
+    float m_ref[2] = {-INFINITY, -INFINITY};
+    float m_seen[2] = {-INFINITY, -INFINITY};  // max raw score over the tiles processed so far
+    float l[2] = {0.f, 0.f};                   // this thread's half of sum exp2((s - m_ref) * sl2)
+    uint32_t slot = 0;                         // exchange-buffer parity, toggles at every named barrier
+    // One float per (slot, half, row): the two threads of a row swap their half-row maxima (and, at the
+    // end, their half-row sums) across a 64-thread named barrier (one per pair of warps).  A slot is rewritten two barriers later.
+    auto exchange = [&](float mine) -> float {
+      st_shared_f32(sXch + ((slot * 2 + hh) * kTile + row_in_tile) * 4, mine);
+      tc_fence_before();
+      named_bar_sync(1 + (warp & 3), 64);  // only the two warps of this row group: pass counts differ between groups
+      tc_fence_after();
+      const float other = ld_shared_f32(sXch + ((slot * 2 + (hh ^ 1)) * kTile + row_in_tile) * 4);
+      slot ^= 1;
+      return other;
+    };
+    for (int j = 0; j < n_kv; ++j) {
+      const int n_valid = (j < n0) ? min(kTile, item.seg0_len - j * kTile) : min(kTile, item.seg1_len - (j - n0) * kTile);
+      const int n_valid_h = n_valid - 64 * hh;  // valid columns of this thread's 64-column half (may be <= 0)
 #pragma unroll
-        for (int c = 0; c < 4; ++c) tmem_ld32(tS + c * 32, s[c]);
-        tmem_wait_ld();
-        if (n_valid < kTile) {
+      for (int i = 0; i < 2; ++i) {
+        if (i < n_qt) {
+          const uint32_t tS = tS0 + i * 128 + lane_off;
+          const uint32_t tO = tO0 + i * D + lane_off + hh * (D / 2);
+          auto rescale_to = [&](float m_new) {
+            const float alpha = ex2((m_ref[i] - m_new) * sl2);
+            m_ref[i] = m_new;
+            l[i] *= alpha;
 #pragma unroll
-          for (int c = 0; c < 4; ++c)
-#pragma unroll
-            for (int k = 0; k < 32; ++k)
-              if (c * 32 + k >= n_valid) s[c][k] = 0xff800000u;  // -inf
-        }
-        float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
-#pragma unroll
-        for (int k = 0; k < 32; ++k) {
-          mx0 = fmaxf(mx0, __uint_as_float(s[0][k]));
-          mx1 = fmaxf(mx1, __uint_as_float(s[1][k]));
-          mx2 = fmaxf(mx2, __uint_as_float(s[2][k]));
-          mx3 = fmaxf(mx3, __uint_as_float(s[3][k]));
-        }
-        const float m_tile = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
-        if (j == 0) {
-          m_ref = m_tile;
-        } else {
-          // Lazy rescale: keep the stale reference max while the new max exceeds it by < 2^8.
-          const bool need = (m_tile - m_ref) * sl2 > 8.0f;
-          if (__any_sync(0xffffffffu, need)) {
-            const float m_new = fmaxf(m_ref, m_tile);
-            const float alpha = ex2((m_ref - m_new) * sl2);
-            m_ref = m_new;
-            l *= alpha;
-            // s_full(j) completed => every earlier MMA, including O_i += P_i V_{j-1}, is complete.
-#pragma unroll
-            for (int c = 0; c < D / 32; ++c) {
+            for (int c = 0; c < D / 64; ++c) {  // this thread's half of the O_i row
               uint32_t o[32];
               tmem_ld32(tO + c * 32, o);
               tmem_wait_ld();
@@ -154,62 +166,129 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
               for (int k = 0; k < 32; ++k) o[k] = __float_as_uint(__uint_as_float(o[k]) * alpha);
               tmem_st32(tO + c * 32, o);
             }
+            tmem_wait_st();
+          };
+          mbar_wait(bar_s_full + 8 * i, j & 1);
+          tc_fence_after();
+          // s_full(j) completed => every earlier MMA, including O_i += P_i V_{j-1}, is complete.
+          if (j > 0 && __any_sync(0xffffffffu, (m_seen[i] - m_ref[i]) * sl2 > 8.0f)) rescale_to(fmaxf(m_ref[i], m_seen[i]));
+          uint32_t pk[2][16];
+          float l_tile = 0.f, mt = -INFINITY;
+#pragma unroll 1
+          for (int pass = 0; pass < 2; ++pass) {
+            // The half row streams through two 32-column register buffers: the tcgen05.ld of the second
+            // chunk is in flight while the first is exponentiated.
+            uint32_t s[2][32];
+            const float neg_m = -m_ref[i] * sl2;
+            const uint64_t sl2_2 = pack2(sl2, sl2), neg_m2 = pack2(neg_m, neg_m);
+            uint64_t la = pack2(0.f, 0.f), lb = pack2(0.f, 0.f);
+            float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+            tmem_ld32(tS + hh * 64, s[0]);
+#pragma unroll
+            for (int c = 0; c < 2; ++c) {
+              tmem_wait_ld();
+              if (c == 0) tmem_ld32(tS + hh * 64 + 32, s[1]);
+              uint32_t(&sc)[32] = s[c];
+              if (n_valid < kTile) {
+#pragma unroll
+                for (int k = 0; k < 32; ++k)
+                  if (c * 32 + k >= n_valid_h) sc[k] = 0xff800000u;  // -inf
+              }
+#pragma unroll
+              for (int k = 0; k < 16; ++k) {
+                const float s0 = __uint_as_float(sc[2 * k]), s1 = __uint_as_float(sc[2 * k + 1]);
+                mx[k & 3] = fmaxf(mx[k & 3], fmaxf(s0, s1));
+                // x = s * scale * log2(e) - m_ref * scale * log2(e) for a pair of columns (one FFMA2)
+                const uint64_t x = fma2(pack2(s0, s1), sl2_2, neg_m2);
+                float p0, p1;
+                if (((k * kEmuPairsPer8) & 7) < kEmuPairsPer8) {
+                  ex2_emu2(x, p0, p1);  // FMA/ALU pipes
+                } else {
+                  float x0, x1;
+                  unpack2(x, x0, x1);
+                  p0 = ex2(x0);  // MUFU
+                  p1 = ex2(x1);
+                }
+                if (k & 1) lb = add2(lb, pack2(p0, p1)); else la = add2(la, pack2(p0, p1));
+                pk[c][k] = pack_bf16(p0, p1);
+              }
+            }
+            float l0, l1, l2, l3;
+            unpack2(la, l0, l1);
+            unpack2(lb, l2, l3);
+            l_tile = (l0 + l1) + (l2 + l3);
+            // Full-row tile max = max of the two halves.  The barrier also orders every tcgen05.ld of S_i
+            // (both halves) before any tcgen05.st of P_i, which overwrites columns [0, 64) of S_i.
+            const float mt_h = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3]));
+            mt = fmaxf(mt_h, exchange(mt_h));
+            // exact unless the tile leads m_ref by more than 2^64 (or m_ref is still -inf); the decision is
+            // the same in both warps of a row (same mt, same m_ref)
+            if (pass == 1 || !__any_sync(0xffffffffu, !((mt - m_ref[i]) * sl2 <= 64.0f))) break;
+            const float m_new = fmaxf(m_ref[i], mt);
+            if (j > 0) rescale_to(m_new); else m_ref[i] = m_new;
+          }
+          m_seen[i] = fmaxf(m_seen[i], mt);
+          l[i] += l_tile;
+          if (n_valid < kTile) {
+            // the emulated exp2 returns ~2^-125 (not 0) for a masked column: force P = 0 exactly
+#pragma unroll
+            for (int c = 0; c < 2; ++c)
+#pragma unroll
+              for (int k = 0; k < 16; ++k) {
+                const int col = c * 32 + 2 * k;
+                if (col >= n_valid_h) pk[c][k] = 0u;
+                else if (col + 1 >= n_valid_h) pk[c][k] &= 0xffffu;
+              }
+          }
+          // P_i: bf16 pairs; this half's 64 keys are columns [32 hh, 32 hh + 32) of the S_i region
+#pragma unroll
+          for (int c = 0; c < 2; ++c) tmem_st16(tS + hh * 32 + c * 16, pk[c]);
+          tmem_wait_st();
+          tc_fence_before();
+          mbar_arrive(bar_p_full + 8 * i);
+        }
+      }
+    }
+    // ---------------------------------------------------- epilogue (a5): O / l -> bf16, LSE
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+      if (i < n_qt) {
+        const uint32_t tO = tO0 + i * D + lane_off + hh * (D / 2);
+        mbar_wait(bar_o_full + 8 * i, 0);
+        tc_fence_after();
+        const float l_row = l[i] + exchange(l[i]);
+        const int row = i * kTile + row_in_tile;
+        const bool valid = row < item.q_rows;
+        const int n_tok = item.q_is_ref ? p.n_ref : p.n_gen;
+        const int grow = item.q_row0 + row;
+        __nv_bfloat16* obase = item.q_is_ref ? p.o_ref : p.o_gen;
+        uint4* orow = reinterpret_cast<uint4*>(obase + ((size_t(b) * n_tok + grow) * p.heads + h) * D + hh * (D / 2));
+        const float inv_l = 1.0f / l_row;
+#pragma unroll
+        for (int c = 0; c < D / 64; ++c) {
+          uint32_t o[32];
+          tmem_ld32(tO + c * 32, o);
+          tmem_wait_ld();
+          if (valid) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              uint4 v;
+              v.x = pack_bf16(__uint_as_float(o[8 * q + 0]) * inv_l, __uint_as_float(o[8 * q + 1]) * inv_l);
+              v.y = pack_bf16(__uint_as_float(o[8 * q + 2]) * inv_l, __uint_as_float(o[8 * q + 3]) * inv_l);
+              v.z = pack_bf16(__uint_as_float(o[8 * q + 4]) * inv_l, __uint_as_float(o[8 * q + 5]) * inv_l);
+              v.w = pack_bf16(__uint_as_float(o[8 * q + 6]) * inv_l, __uint_as_float(o[8 * q + 7]) * inv_l);
+              orow[c * 4 + q] = v;
+            }
           }
         }
-        const float neg_m = -m_ref * sl2;
-        float l0 = 0.f, l1 = 0.f;
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-          uint32_t pk[16];
-#pragma unroll
-          for (int k = 0; k < 16; ++k) {
-            const float p0 = ex2(fmaf(__uint_as_float(s[c][2 * k]), sl2, neg_m));
-            const float p1 = ex2(fmaf(__uint_as_float(s[c][2 * k + 1]), sl2, neg_m));
-            l0 += p0;
-            l1 += p1;
-            pk[k] = pack_bf16(p0, p1);
-          }
-          tmem_st16(tS + c * 16, pk);  // P_i: bf16 pairs, columns [16c, 16c+16) of S_i
-        }
-        l += l0 + l1;
-        tmem_wait_st();
+        float* lse = item.q_is_ref ? p.lse_ref : p.lse_gen;
+        if (lse != nullptr && valid && hh == 0) lse[(size_t(b) * p.heads + h) * n_tok + grow] = m_ref[i] * p.scale + __logf(l_row);
         tc_fence_before();
-        mbar_arrive(bar_p_full + 8 * i);
       }
-      // ---------------------------------------------------- epilogue (a5): O / l -> bf16, LSE
-      mbar_wait(bar_o_full + 8 * i, 0);
-      tc_fence_after();
-      const int row = i * kTile + (warp & 3) * 32 + lane;
-      const bool valid = row < item.q_rows;
-      const int n_tok = item.q_is_ref ? p.n_ref : p.n_gen;
-      const int grow = item.q_row0 + row;
-      __nv_bfloat16* obase = item.q_is_ref ? p.o_ref : p.o_gen;
-      uint4* orow = reinterpret_cast<uint4*>(obase + ((size_t(b) * n_tok + grow) * p.heads + h) * D);
-      const float inv_l = 1.0f / l;
-#pragma unroll
-      for (int c = 0; c < D / 32; ++c) {
-        uint32_t o[32];
-        tmem_ld32(tO + c * 32, o);
-        tmem_wait_ld();
-        if (valid) {
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            uint4 v;
-            v.x = pack_bf16(__uint_as_float(o[8 * q + 0]) * inv_l, __uint_as_float(o[8 * q + 1]) * inv_l);
-            v.y = pack_bf16(__uint_as_float(o[8 * q + 2]) * inv_l, __uint_as_float(o[8 * q + 3]) * inv_l);
-            v.z = pack_bf16(__uint_as_float(o[8 * q + 4]) * inv_l, __uint_as_float(o[8 * q + 5]) * inv_l);
-            v.w = pack_bf16(__uint_as_float(o[8 * q + 6]) * inv_l, __uint_as_float(o[8 * q + 7]) * inv_l);
-            orow[c * 4 + q] = v;
-          }
-        }
-      }
-      float* lse = item.q_is_ref ? p.lse_ref : p.lse_gen;
-      if (lse != nullptr && valid) lse[(size_t(b) * p.heads + h) * n_tok + grow] = m_ref * p.scale + __logf(l);
-      tc_fence_before();
     }
   } else {
     reg_dec<56>();
-    if (warp == 9 && lane == 0) {
+    if (warp == 9 && elect_one()) {
       // ===================================================== TMA loader
       const CUtensorMap* tq = item.q_is_ref ? &tm_q_ref : &tm_q_gen;
       mbar_arrive_expect_tx(bar_q_full, n_qt * C::kTileBytes);
@@ -230,24 +309,27 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
           load_tile<D>(sKV + s * C::kTileBytes, tm, bar_kv_full + 8 * s, row, h, b, hm);
         }
       }
-    } else if (warp == 8 && lane == 0) {
+    } else if (warp == 8 && elect_one()) {
       // ===================================================== MMA issuer
       constexpr uint32_t idesc_qk = make_idesc_bf16(kTile, kTile, 0, 0);
       constexpr uint32_t idesc_pv = make_idesc_bf16(kTile, D, 0, 1);
+      // Descriptor low words: Q/K tiles are K-major (LBO unused), V is MN-major (LBO = one 64-column box).
+      constexpr uint32_t kDescHi = desc_hi_sw128(1024);
+      constexpr uint32_t kStageStep = C::kTileBytes >> 4;
+      const uint32_t q_lo = desc_lo(sQ, 16), k_lo = desc_lo(sKV, 16), v_lo = desc_lo(sKV, C::kBoxBytes);
       auto issue_qk = [&](int i, int stage) {
-        const uint32_t q = sQ + i * C::kTileBytes, k = sKV + stage * C::kTileBytes;
+        const uint32_t q = q_lo + i * kStageStep, k = k_lo + stage * kStageStep;
 #pragma unroll
         for (int kk = 0; kk < D / 16; ++kk) {
-          const uint32_t off = (kk / 4) * C::kBoxBytes + (kk % 4) * 32;
-          umma_ss(tS0 + i * 128, make_smem_desc_sw128(q + off, 16, 1024), make_smem_desc_sw128(k + off, 16, 1024),
-                  idesc_qk, kk > 0);
+          const uint32_t off = ((kk / 4) * C::kBoxBytes + (kk % 4) * 32) >> 4;
+          umma_ss(tS0 + i * 128, desc64(q + off, kDescHi), desc64(k + off, kDescHi), idesc_qk, kk > 0);
         }
       };
       auto issue_pv = [&](int i, int stage, bool acc) {
-        const uint32_t v = sKV + stage * C::kTileBytes;
+        const uint32_t v = v_lo + stage * kStageStep;
 #pragma unroll
         for (int kk = 0; kk < kTile / 16; ++kk)
-          umma_ts(tO0 + i * D, tS0 + i * 128 + kk * 8, make_smem_desc_sw128(v + kk * 2048, C::kBoxBytes, 1024), idesc_pv,
+          umma_ts(tO0 + i * D, tS0 + i * 128 + kk * 8, desc64(v + kk * (2048 >> 4), kDescHi), idesc_pv,
                   (acc || kk > 0) ? 1u : 0u);
       };
       auto stage_of = [&](int it) { return it % C::kStages; };
