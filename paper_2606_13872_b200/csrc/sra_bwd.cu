@@ -30,15 +30,13 @@ struct BwdCfg {
   static constexpr int kQBytes = kQT * D * 2;           // Q_i or dO_i tile
   static constexpr int kQBoxBytes = kQT * 128;
   static constexpr int kBoxes = D / 64;
-  static constexpr int kStages = 3;
+  static constexpr int kStages = 4;
   static constexpr int kStageBytes = 2 * kQBytes;       // Q_i + dO_i
   static constexpr int kDsBytes = kTile * kQT * 2;      // dS^T tile [128 keys][64 queries] bf16, x2 buffers
-  static constexpr int kDqBytes = kQT * D * 4;          // dQ staging tile [64 queries][D] fp32
   static constexpr int kVecBytes = kStages * 2 * kQT * 4;  // lse2[64] + delta[64] per stage
   static constexpr int kNumBars = 1 + 2 * kStages + 2 + 1 + 2 + 2 + 2 + 2 + 1;
-  static constexpr int kSmemBytes = 1024 + 2 * kKBytes + kStages * kStageBytes + 2 * kDsBytes + kDqBytes + kVecBytes +
-                                    kNumBars * 8 + 16;
-  static constexpr int kThreads = 384;
+  static constexpr int kSmemBytes = 2 * kKBytes + kStages * kStageBytes + 2 * kDsBytes + kVecBytes + kNumBars * 8 + 16;
+  static constexpr int kThreads = 512;  // 2 compute warpgroups, 1 dQ warpgroup, MMA + TMA warps (+2 idle)
   // TMEM columns
   static constexpr int kColS = 0, kColDP = 128, kColDQ = 192, kColDV = 256, kColDK = 256 + D;
 };
@@ -85,14 +83,14 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
   using C = BwdCfg<D>;
   constexpr int QT = C::kQT;
   constexpr int ST = C::kStages;
-  extern __shared__ uint8_t smem_raw[];
-  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  extern __shared__ __align__(1024) uint8_t smem_raw[];  // 128-byte-swizzled tiles need 1024-byte alignment
+  const uint32_t smem_base = smem_u32(smem_raw);
+  if ((smem_base & 1023u) != 0) __trap();
   const uint32_t sK = smem_base;
   const uint32_t sV = sK + C::kKBytes;
   const uint32_t sStage = sV + C::kKBytes;                      // [ST] x {Q_i, dO_i}
   const uint32_t sDs = sStage + ST * C::kStageBytes;            // [2] dS^T
-  const uint32_t sDq = sDs + 2 * C::kDsBytes;                   // dQ staging tile
-  const uint32_t sVec = sDq + C::kDqBytes;                      // [ST] x {lse2[64], delta[64]}
+  const uint32_t sVec = sDs + 2 * C::kDsBytes;                  // [ST] x {lse2[64], delta[64]}
   const uint32_t sBar = sVec + C::kVecBytes;
   const uint32_t bar_kv_full = sBar;
   const uint32_t bar_q_full = sBar + 8;                         // [ST]
@@ -126,8 +124,8 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
     }
     for (int i = 0; i < 2; ++i) {
       mbar_init(bar_s_full + 8 * i, 1);
-      mbar_init(bar_p_full + 8 * i, 128);
-      mbar_init(bar_ds_full + 8 * i, 128);
+      mbar_init(bar_p_full + 8 * i, 256);
+      mbar_init(bar_ds_full + 8 * i, 256);
       mbar_init(bar_ds_empty + 8 * i, 1);
     }
     mbar_init(bar_dp_full, 1);
@@ -136,53 +134,59 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
     mbar_init(bar_acc_full, 1);
     fence_mbar_init();
   }
-  if (warp == 9 && lane == 0) {
+  if (warp == 13 && lane == 0) {
     tma_prefetch_desc(&tm_q_gen);
     tma_prefetch_desc(&tm_do_gen);
     tma_prefetch_desc(item.k_is_ref ? &tm_k_ref : &tm_k_gen);
     tma_prefetch_desc(item.k_is_ref ? &tm_v_ref : &tm_v_gen);
   }
-  if (warp == 8) tmem_alloc(s_tmem_ptr, 512);
+  if (warp == 12) tmem_alloc(s_tmem_ptr, 512);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = *tmem_ptr_generic;
 
-  if (warp < 4) {
-    // ================================================= compute warpgroup: P^T and dS^T (thread = key)
-    reg_inc<224>();
-    const int key = warp * 32 + lane;
+  if (warp < 8) {
+    // ================================================= two compute warpgroups: P^T and dS^T (thread = key)
+    // Warps w and w + 4 sit on the same SM sub-partition and own the same 32 TMEM lanes (keys); warp w takes
+    // queries [0, 32) of every 64-query tile, warp w + 4 queries [32, 64).  Two warps per sub-partition let
+    // the scheduler overlap one warp's MUFU / tcgen05.ld / barrier latencies with the other's arithmetic, and
+    // halve the time each tile spends in this stage of the S -> P -> dV / dP -> dS -> dK, dQ ring.
+    const int ch = warp >> 2;  // query half
+    const int key = (warp & 3) * 32 + lane;
     const bool key_valid = key < item.k_rows;
-    const uint32_t lane_off = uint32_t(warp * 32) << 16;
+    const uint32_t lane_off = uint32_t((warp & 3) * 32) << 16;
     const float sl2 = p.scale_log2;
     for (int it = 0; it < n_it; ++it) {
       const int bf = it & 1, s = it % ST;
       const uint32_t tS = tmem + lane_off + C::kColS + bf * QT;
       const uint32_t tDP = tmem + lane_off + C::kColDP;
-      const uint32_t vec = sVec + s * (2 * QT * 4);
+      const uint32_t vec = sVec + s * (2 * QT * 4) + ch * 32 * 4;
       mbar_wait(bar_q_full + 8 * s, (it / ST) & 1);  // acquire the loader's lse2 / delta writes
       mbar_wait(bar_s_full + 8 * bf, (it >> 1) & 1);
       tc_fence_after();
-      uint32_t sv[2][32];
-      tmem_ld32(tS, sv[0]);
-      tmem_ld32(tS + 32, sv[1]);
+      uint32_t sv[32];
+      tmem_ld32(tS + ch * 32, sv);
       tmem_wait_ld();
-      float pf[QT];
+      float pf[32];
 #pragma unroll
-      for (int c = 0; c < 2; ++c)
-#pragma unroll
-        for (int q4 = 0; q4 < 8; ++q4) {
-          const float4 l = ld_shared_f4(vec + (c * 32 + q4 * 4) * 4);
-          pf[c * 32 + q4 * 4 + 0] = ex2(fmaf(__uint_as_float(sv[c][q4 * 4 + 0]), sl2, -l.x));
-          pf[c * 32 + q4 * 4 + 1] = ex2(fmaf(__uint_as_float(sv[c][q4 * 4 + 1]), sl2, -l.y));
-          pf[c * 32 + q4 * 4 + 2] = ex2(fmaf(__uint_as_float(sv[c][q4 * 4 + 2]), sl2, -l.z));
-          pf[c * 32 + q4 * 4 + 3] = ex2(fmaf(__uint_as_float(sv[c][q4 * 4 + 3]), sl2, -l.w));
-        }
+      for (int q4 = 0; q4 < 8; ++q4) {
+        const float4 l = ld_shared_f4(vec + (q4 * 4) * 4);
+        pf[q4 * 4 + 0] = ex2(fmaf(__uint_as_float(sv[q4 * 4 + 0]), sl2, -l.x));
+        pf[q4 * 4 + 1] = ex2(fmaf(__uint_as_float(sv[q4 * 4 + 1]), sl2, -l.y));
+        pf[q4 * 4 + 2] = ex2(fmaf(__uint_as_float(sv[q4 * 4 + 2]), sl2, -l.z));
+        pf[q4 * 4 + 3] = ex2(fmaf(__uint_as_float(sv[q4 * 4 + 3]), sl2, -l.w));
+      }
       {
-        uint32_t pk[32];
+        uint32_t pk[16];
 #pragma unroll
-        for (int k = 0; k < 32; ++k) pk[k] = pack_bf16(pf[2 * k], pf[2 * k + 1]);
-        tmem_st32(tS, pk);  // P^T: bf16 pairs in the first 32 columns of S[bf]
+        for (int k = 0; k < 16; ++k) pk[k] = pack_bf16(pf[2 * k], pf[2 * k + 1]);
+        // P^T: bf16 pairs in the first 32 columns of S[bf]; both halves have finished their tcgen05.ld of
+        // columns [0, 32) only once the half-0 warp is here, and half 1 writes columns [16, 32): order them
+        tc_fence_before();
+        named_bar_sync(1 + (warp & 3), 64);
+        tc_fence_after();
+        tmem_st16(tS + ch * 16, pk);
       }
       tmem_wait_st();
       tc_fence_before();
@@ -190,13 +194,12 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
 
       mbar_wait(bar_dp_full, it & 1);
       tc_fence_after();
-      tmem_ld32(tDP, sv[0]);
-      tmem_ld32(tDP + 32, sv[1]);
+      tmem_ld32(tDP + ch * 32, sv);
       tmem_wait_ld();
       mbar_wait(bar_ds_empty + 8 * bf, ((it >> 1) & 1) ^ 1);  // dK / dQ MMAs of iteration it-2 have read sDs[bf]
       const uint32_t ds_row = sDs + bf * C::kDsBytes + key * 128;
 #pragma unroll
-      for (int c = 0; c < 8; ++c) {  // 16-byte chunk c = queries [8c, 8c+8)
+      for (int c = 0; c < 4; ++c) {  // 16-byte chunk 4 ch + c = queries [32 ch + 8c, 32 ch + 8c + 8)
         const float4 d0 = ld_shared_f4(vec + QT * 4 + (c * 8) * 4);
         const float4 d1 = ld_shared_f4(vec + QT * 4 + (c * 8 + 4) * 4);
         const float dl[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
@@ -204,29 +207,29 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
           const int q = c * 8 + 2 * k;
-          float a = pf[q] * (__uint_as_float(sv[q >> 5][q & 31]) - dl[2 * k]);
-          float bb = pf[q + 1] * (__uint_as_float(sv[(q + 1) >> 5][(q + 1) & 31]) - dl[2 * k + 1]);
+          float a = pf[q] * (__uint_as_float(sv[q]) - dl[2 * k]);
+          float bb = pf[q + 1] * (__uint_as_float(sv[q + 1]) - dl[2 * k + 1]);
           if (!key_valid) { a = 0.f; bb = 0.f; }
           w[k] = pack_bf16(a, bb);
         }
-        st_shared_v4(ds_row + ((c ^ (key & 7)) << 4), w[0], w[1], w[2], w[3]);
+        st_shared_v4(ds_row + (((ch * 4 + c) ^ (key & 7)) << 4), w[0], w[1], w[2], w[3]);
       }
       fence_proxy_async_smem();
       tc_fence_before();
       mbar_arrive(bar_ds_full + 8 * bf);
     }
-    // ---------------------------------------------------- epilogue: dV (lanes = keys)
+    // ---------------------------------------------------- epilogue: dV (lanes = keys), this warp's D/2 columns
     mbar_wait(bar_acc_full, 0);
     tc_fence_after();
     {
       const int n_tok = item.k_is_ref ? p.n_ref : p.n_gen;
       const int grow = item.k_row0 + key;
       __nv_bfloat16* base = item.k_is_ref ? p.dv_ref : p.dv_gen;
-      uint4* orow = reinterpret_cast<uint4*>(base + ((size_t(b) * n_tok + grow) * p.heads + h) * D);
+      uint4* orow = reinterpret_cast<uint4*>(base + ((size_t(b) * n_tok + grow) * p.heads + h) * D + ch * (D / 2));
 #pragma unroll
-      for (int c = 0; c < D / 32; ++c) {
+      for (int c = 0; c < D / 64; ++c) {
         uint32_t o[32];
-        tmem_ld32(tmem + lane_off + C::kColDV + c * 32, o);
+        tmem_ld32(tmem + lane_off + C::kColDV + ch * (D / 2) + c * 32, o);
         tmem_wait_ld();
         if (key_valid) {
 #pragma unroll
@@ -242,13 +245,11 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
       }
     }
     tc_fence_before();
-  } else if (warp < 8) {
+  } else if (warp < 12) {
     // ================================================= reduce warpgroup: dQ^T drain (thread = d), then dK epilogue
-    reg_inc<224>();
-    const int wq = warp - 4;
+    const int wq = warp - 8;
     const int drow = wq * 32 + lane;  // TMEM lane = d index (dQ^T), later = key index (dK)
     const uint32_t lane_off = uint32_t(wq * 32) << 16;
-    const bool issuer = (threadIdx.x == 128);
     for (int it = 0; it < n_it; ++it) {
       const QTile qt = q_tile_of(it, n0, item, p.n_gen);
       mbar_wait(bar_dq_full, it & 1);
@@ -259,21 +260,16 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
       tmem_wait_ld();
       tc_fence_before();
       mbar_arrive(bar_dq_empty);
-      if (issuer) tma_wait_group_read<0>();  // the previous reduce-add has finished reading the staging tile
-      named_bar_sync(1, 128);
-      // staging tile [64 queries][D] fp32 row-major: for a fixed query the warp writes 32 consecutive floats
+      // dQ_it^T leaves the SM straight from registers: for a fixed query the 32 lanes of a warp hold 32
+      // consecutive d, so each red.global.add.f32 is one coalesced 128-byte reduction into the fp32
+      // workspace (no shared-memory staging: the kernel is bound by shared-memory bandwidth).
+      float* dq_row = p.dq_ws + (size_t(bh) * p.n_pad + qt.cat0) * D + drow;
 #pragma unroll
       for (int x = 0; x < 2; ++x)
 #pragma unroll
-        for (int c = 0; c < 32; ++c) st_shared_f32(sDq + ((x * 32 + c) * D + drow) * 4, __uint_as_float(r[x][c]));
-      fence_proxy_async_smem();
-      named_bar_sync(1, 128);
-      if (issuer) {
-        bulk_reduce_add_f32(p.dq_ws + (size_t(bh) * p.n_pad + qt.cat0) * D, sDq, uint32_t(qt.valid) * D * 4);
-        tma_commit_group();
-      }
+        for (int c = 0; c < 32; ++c)
+          if (x * 32 + c < qt.valid) red_add_f32(dq_row + (x * 32 + c) * D, __uint_as_float(r[x][c]));
     }
-    if (issuer) tma_wait_group<0>();
     // ---------------------------------------------------- epilogue: dK = scale * acc (lanes = keys)
     mbar_wait(bar_acc_full, 0);
     tc_fence_after();
@@ -305,8 +301,7 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
     }
     tc_fence_before();
   } else {
-    reg_dec<56>();
-    if (warp == 9) {
+    if (warp == 13) {
       // ================================================= loader: K/V once, then the {Q_i, dO_i, lse2, delta} ring
       const bool k_hm = item.k_is_ref && p.ref_kv_head_major;
       if (lane == 0) {
@@ -336,38 +331,45 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
                            qt.row0, h, b, false);
         }
       }
-    } else if (warp == 8 && lane == 0) {
+    } else if (warp == 12 && elect_one()) {
       // ================================================= MMA issuer
       constexpr uint32_t idesc_st = make_idesc_bf16(kTile, QT, 0, 0);   // S^T, dP^T : [128 x 64], K = d
       constexpr uint32_t idesc_acc = make_idesc_bf16(kTile, D, 0, 1);   // dV, dK    : [128 x D],  K = 64 queries
       constexpr uint32_t idesc_dq = make_idesc_bf16(D, QT, 1, 1);       // dQ^T      : [D x 64],    K = 128 keys
       const uint32_t tS0 = tmem + C::kColS, tDP = tmem + C::kColDP, tDQ = tmem + C::kColDQ;
       const uint32_t tDV = tmem + C::kColDV, tDK = tmem + C::kColDK;
-      // [128 x 64] = A[128 keys][d] (K-major) * B[64 queries][d]^T (K-major)
-      auto issue_kq = [&](uint32_t d_tmem, uint32_t a_tile, uint32_t b_tile) {
+      // Descriptor low words (start address, LBO); stepping along K or to another stage is one 32-bit add.
+      constexpr uint32_t kHi = desc_hi_sw128(1024);
+      const uint32_t k_km = desc_lo(sK, 16), v_km = desc_lo(sV, 16);             // K, V as K-major A operands
+      const uint32_t k_mn = desc_lo(sK, C::kKBoxBytes);                          // K as MN-major A operand (dQ^T)
+      const uint32_t st_km = desc_lo(sStage, 16);                                // Q_i / dO_i as K-major B operands
+      const uint32_t st_mn = desc_lo(sStage, C::kQBoxBytes);                     // Q_i / dO_i as MN-major B operands
+      const uint32_t ds_km = desc_lo(sDs, 16), ds_mn = desc_lo(sDs, C::kDsBytes);
+      // [128 x 64] = A[128 keys][d] (K-major) * B[64 queries][d]^T (K-major); b_off = byte offset inside sStage
+      auto issue_kq = [&](uint32_t d_tmem, uint32_t a_lo, uint32_t b_off) {
 #pragma unroll
         for (int kk = 0; kk < D / 16; ++kk)
-          umma_ss(d_tmem, make_smem_desc_sw128(a_tile + (kk / 4) * C::kKBoxBytes + (kk % 4) * 32, 16, 1024),
-                  make_smem_desc_sw128(b_tile + (kk / 4) * C::kQBoxBytes + (kk % 4) * 32, 16, 1024), idesc_st, kk > 0);
+          umma_ss(d_tmem, desc64(a_lo + (((kk / 4) * C::kKBoxBytes + (kk % 4) * 32) >> 4), kHi),
+                  desc64(st_km + ((b_off + (kk / 4) * C::kQBoxBytes + (kk % 4) * 32) >> 4), kHi), idesc_st, kk > 0);
       };
       mbar_wait(bar_kv_full, 0);
       mbar_wait(bar_q_full, 0);
       tc_fence_after();
-      issue_kq(tS0, sK, sStage);
+      issue_kq(tS0, k_km, 0);
       umma_commit(bar_s_full);
-      issue_kq(tDP, sV, sStage + C::kQBytes);
+      issue_kq(tDP, v_km, C::kQBytes);
       umma_commit(bar_dp_full);
       for (int it = 0; it < n_it; ++it) {
         const int bf = it & 1, s = it % ST;
-        const uint32_t sQ = sStage + s * C::kStageBytes, sDO = sQ + C::kQBytes;
-        const uint32_t ds = sDs + bf * C::kDsBytes;
+        const uint32_t oQ = s * C::kStageBytes, oDO = oQ + C::kQBytes;  // byte offsets inside sStage
+        const uint32_t ods = bf * C::kDsBytes;
         const bool more = it + 1 < n_it;
         const int s1 = (it + 1) % ST;
-        const uint32_t sQ1 = sStage + s1 * C::kStageBytes;
+        const uint32_t oQ1 = s1 * C::kStageBytes;
         if (more) {
           mbar_wait(bar_q_full + 8 * s1, ((it + 1) / ST) & 1);
           tc_fence_after();
-          issue_kq(tS0 + (bf ^ 1) * QT, sK, sQ1);  // S^T(it+1); its buffer held P^T(it-1), consumed by dV(it-1)
+          issue_kq(tS0 + (bf ^ 1) * QT, k_km, oQ1);  // S^T(it+1); its buffer held P^T(it-1), consumed by dV(it-1)
           umma_commit(bar_s_full + 8 * (bf ^ 1));
         }
         // dV += P^T(it) dO_it : A = P^T from TMEM (16 queries = 8 columns per step), B = dO_it [queries][d] MN-major
@@ -375,26 +377,25 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
         tc_fence_after();
 #pragma unroll
         for (int kk = 0; kk < QT / 16; ++kk)
-          umma_ts(tDV, tS0 + bf * QT + kk * 8, make_smem_desc_sw128(sDO + kk * 2048, C::kQBoxBytes, 1024), idesc_acc,
+          umma_ts(tDV, tS0 + bf * QT + kk * 8, desc64(st_mn + ((oDO + kk * 2048) >> 4), kHi), idesc_acc,
                   (it > 0 || kk > 0) ? 1u : 0u);
         mbar_wait(bar_ds_full + 8 * bf, (it >> 1) & 1);  // dS^T(it) in smem; dP^T(it) has been read out of TMEM
         tc_fence_after();
         if (more) {
-          issue_kq(tDP, sV, sQ1 + C::kQBytes);  // dP^T(it+1)
+          issue_kq(tDP, v_km, oQ1 + C::kQBytes);  // dP^T(it+1)
           umma_commit(bar_dp_full);
         }
         // dK += dS^T(it) Q_it : A = dS^T [keys][queries] K-major (one 128-byte box), B = Q_it [queries][d] MN-major
 #pragma unroll
         for (int kk = 0; kk < QT / 16; ++kk)
-          umma_ss(tDK, make_smem_desc_sw128(ds + kk * 32, 16, 1024), make_smem_desc_sw128(sQ + kk * 2048, C::kQBoxBytes, 1024),
+          umma_ss(tDK, desc64(ds_km + ((ods + kk * 32) >> 4), kHi), desc64(st_mn + ((oQ + kk * 2048) >> 4), kHi),
                   idesc_acc, (it > 0 || kk > 0) ? 1u : 0u);
         // dQ_it^T = K^T dS^T(it) : A = K [keys][d] MN-major, B = dS^T [keys][queries] MN-major, K = 128 keys
         mbar_wait(bar_dq_empty, (it & 1) ^ 1);
         tc_fence_after();
 #pragma unroll
         for (int kk = 0; kk < kTile / 16; ++kk)
-          umma_ss(tDQ, make_smem_desc_sw128(sK + kk * 2048, C::kKBoxBytes, 1024),
-                  make_smem_desc_sw128(ds + kk * 2048, C::kDsBytes, 1024), idesc_dq, kk > 0);
+          umma_ss(tDQ, desc64(k_mn + ((kk * 2048) >> 4), kHi), desc64(ds_mn + ((ods + kk * 2048) >> 4), kHi), idesc_dq, kk > 0);
         umma_commit(bar_dq_full);
         umma_commit(bar_q_empty + 8 * s);
         umma_commit(bar_ds_empty + 8 * bf);
@@ -403,7 +404,7 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
     }
   }
   __syncthreads();
-  if (warp == 8) {
+  if (warp == 12) {
     tc_fence_after();
     tmem_dealloc(tmem, 512);
   }
