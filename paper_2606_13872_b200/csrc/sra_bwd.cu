@@ -9,10 +9,12 @@
 //         dV  += P^T dO_i       [keys x d]         A = P^T (bf16) from TMEM, aliasing S[i&1]
 //         dK  += dS^T Q_i       [keys x d]         A = dS^T (bf16) from shared memory
 //         dQ_i^T = K^T dS^T     [d x queries]      A = K (MN-major), B = dS^T (MN-major), -> TMEM dQ
-//       with P^T = exp2(S^T * scale*log2e - LSE*log2e) and dS^T = P^T o (dP^T - D) computed by one warpgroup
-//       (thread = key = TMEM lane).  dQ_i^T is drained by a second warpgroup (thread = d = TMEM lane) through
-//       shared memory into the fp32 workspace [B*H][n_pad][d] with a bulk reduce-add (many key tiles add into
-//       the same query rows; the summation order is not deterministic - SURVEY.md 8c A13).
+//       with P^T = exp2(S^T * scale*log2e - LSE*log2e) formed by one warpgroup and dS^T = P^T o (dP^T - D) by a
+//       second one (thread = key = TMEM lane; the two are pipeline stages of consecutive tiles).  dQ_i^T is
+//       drained by a third warpgroup (thread = d = TMEM lane) straight from registers into the fp32 workspace
+//       [B*H][n_pad][d] with coalesced red.global.add.f32 (many key tiles add into the same query rows; the
+//       summation order is not deterministic - SURVEY.md 8c A13).  The L2 reduction rate (~2.8 TB/s measured)
+//       is what bounds this kernel: 32 KB of fp32 partial dQ per (key tile, query tile) pair of 10.5 MFLOP.
 //   a8  sra_bwd_dq_finalize_kernel  workspace * scale -> bf16 dQ [B, N, H, d]
 //
 // TMEM columns (D = 128): S0 @0 (64), S1 @64 (64), dP @128 (64), dQ^T @192 (64), dV @256 (128), dK @384 (128).
@@ -36,7 +38,7 @@ struct BwdCfg {
   static constexpr int kVecBytes = kStages * 2 * kQT * 4;  // lse2[64] + delta[64] per stage
   static constexpr int kNumBars = 1 + 2 * kStages + 2 + 1 + 2 + 2 + 2 + 2 + 1;
   static constexpr int kSmemBytes = 2 * kKBytes + kStages * kStageBytes + 2 * kDsBytes + kVecBytes + kNumBars * 8 + 16;
-  static constexpr int kThreads = 512;  // 2 compute warpgroups, 1 dQ warpgroup, MMA + TMA warps (+2 idle)
+  static constexpr int kThreads = 512;  // P, dS and dQ warpgroups, MMA + TMA warps (+2 idle)
   // TMEM columns
   static constexpr int kColS = 0, kColDP = 128, kColDQ = 192, kColDV = 256, kColDK = 256 + D;
 };
@@ -124,8 +126,8 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
     }
     for (int i = 0; i < 2; ++i) {
       mbar_init(bar_s_full + 8 * i, 1);
-      mbar_init(bar_p_full + 8 * i, 256);
-      mbar_init(bar_ds_full + 8 * i, 256);
+      mbar_init(bar_p_full + 8 * i, 128);
+      mbar_init(bar_ds_full + 8 * i, 128);
       mbar_init(bar_ds_empty + 8 * i, 1);
     }
     mbar_init(bar_dp_full, 1);
@@ -146,90 +148,57 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
   tc_fence_after();
   const uint32_t tmem = *tmem_ptr_generic;
 
-  if (warp < 8) {
-    // ================================================= two compute warpgroups: P^T and dS^T (thread = key)
-    // Warps w and w + 4 sit on the same SM sub-partition and own the same 32 TMEM lanes (keys); warp w takes
-    // queries [0, 32) of every 64-query tile, warp w + 4 queries [32, 64).  Two warps per sub-partition let
-    // the scheduler overlap one warp's MUFU / tcgen05.ld / barrier latencies with the other's arithmetic, and
-    // halve the time each tile spends in this stage of the S -> P -> dV / dP -> dS -> dK, dQ ring.
-    const int ch = warp >> 2;  // query half
-    const int key = (warp & 3) * 32 + lane;
+  if (warp < 4) {
+    // ================================================= P warpgroup: P^T = exp2(S^T * sl2 - LSE * log2e) (thread = key)
+    // The elementwise work of a tile is split into two pipeline stages on two warpgroups (this one and the
+    // dS warpgroup below), so each SM sub-partition always has warps in different phases (MUFU-bound exp2
+    // here, FMA/LSU-bound dS there, tcgen05.ld round trips in both) and a tile's P^T is ready for dV while
+    // the previous tile's dS^T is still being formed.
+    const int key = warp * 32 + lane;
     const bool key_valid = key < item.k_rows;
-    const uint32_t lane_off = uint32_t((warp & 3) * 32) << 16;
+    const uint32_t lane_off = uint32_t(warp * 32) << 16;
     const float sl2 = p.scale_log2;
     for (int it = 0; it < n_it; ++it) {
       const int bf = it & 1, s = it % ST;
       const uint32_t tS = tmem + lane_off + C::kColS + bf * QT;
-      const uint32_t tDP = tmem + lane_off + C::kColDP;
-      const uint32_t vec = sVec + s * (2 * QT * 4) + ch * 32 * 4;
-      mbar_wait(bar_q_full + 8 * s, (it / ST) & 1);  // acquire the loader's lse2 / delta writes
+      const uint32_t vec = sVec + s * (2 * QT * 4);
+      mbar_wait(bar_q_full + 8 * s, (it / ST) & 1);  // acquire the loader's lse2 writes
       mbar_wait(bar_s_full + 8 * bf, (it >> 1) & 1);
       tc_fence_after();
-      uint32_t sv[32];
-      tmem_ld32(tS + ch * 32, sv);
+      uint32_t sv[2][32];
+      tmem_ld32(tS, sv[0]);
+      tmem_ld32(tS + 32, sv[1]);
       tmem_wait_ld();
-      float pf[32];
+      uint32_t pk[32];
 #pragma unroll
-      for (int q4 = 0; q4 < 8; ++q4) {
-        const float4 l = ld_shared_f4(vec + (q4 * 4) * 4);
-        pf[q4 * 4 + 0] = ex2(fmaf(__uint_as_float(sv[q4 * 4 + 0]), sl2, -l.x));
-        pf[q4 * 4 + 1] = ex2(fmaf(__uint_as_float(sv[q4 * 4 + 1]), sl2, -l.y));
-        pf[q4 * 4 + 2] = ex2(fmaf(__uint_as_float(sv[q4 * 4 + 2]), sl2, -l.z));
-        pf[q4 * 4 + 3] = ex2(fmaf(__uint_as_float(sv[q4 * 4 + 3]), sl2, -l.w));
-      }
-      {
-        uint32_t pk[16];
+      for (int c = 0; c < 2; ++c)
 #pragma unroll
-        for (int k = 0; k < 16; ++k) pk[k] = pack_bf16(pf[2 * k], pf[2 * k + 1]);
-        // P^T: bf16 pairs in the first 32 columns of S[bf]; both halves have finished their tcgen05.ld of
-        // columns [0, 32) only once the half-0 warp is here, and half 1 writes columns [16, 32): order them
-        tc_fence_before();
-        named_bar_sync(1 + (warp & 3), 64);
-        tc_fence_after();
-        tmem_st16(tS + ch * 16, pk);
-      }
+        for (int q4 = 0; q4 < 8; ++q4) {
+          const float4 l = ld_shared_f4(vec + (c * 32 + q4 * 4) * 4);
+          const float p0 = ex2(fmaf(__uint_as_float(sv[c][q4 * 4 + 0]), sl2, -l.x));
+          const float p1 = ex2(fmaf(__uint_as_float(sv[c][q4 * 4 + 1]), sl2, -l.y));
+          const float p2 = ex2(fmaf(__uint_as_float(sv[c][q4 * 4 + 2]), sl2, -l.z));
+          const float p3 = ex2(fmaf(__uint_as_float(sv[c][q4 * 4 + 3]), sl2, -l.w));
+          pk[c * 16 + q4 * 2 + 0] = pack_bf16(p0, p1);
+          pk[c * 16 + q4 * 2 + 1] = pack_bf16(p2, p3);
+        }
+      tmem_st32(tS, pk);  // P^T: bf16 pairs in the first 32 columns of S[bf]
       tmem_wait_st();
       tc_fence_before();
       mbar_arrive(bar_p_full + 8 * bf);
-
-      mbar_wait(bar_dp_full, it & 1);
-      tc_fence_after();
-      tmem_ld32(tDP + ch * 32, sv);
-      tmem_wait_ld();
-      mbar_wait(bar_ds_empty + 8 * bf, ((it >> 1) & 1) ^ 1);  // dK / dQ MMAs of iteration it-2 have read sDs[bf]
-      const uint32_t ds_row = sDs + bf * C::kDsBytes + key * 128;
-#pragma unroll
-      for (int c = 0; c < 4; ++c) {  // 16-byte chunk 4 ch + c = queries [32 ch + 8c, 32 ch + 8c + 8)
-        const float4 d0 = ld_shared_f4(vec + QT * 4 + (c * 8) * 4);
-        const float4 d1 = ld_shared_f4(vec + QT * 4 + (c * 8 + 4) * 4);
-        const float dl[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
-        uint32_t w[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          const int q = c * 8 + 2 * k;
-          float a = pf[q] * (__uint_as_float(sv[q]) - dl[2 * k]);
-          float bb = pf[q + 1] * (__uint_as_float(sv[q + 1]) - dl[2 * k + 1]);
-          if (!key_valid) { a = 0.f; bb = 0.f; }
-          w[k] = pack_bf16(a, bb);
-        }
-        st_shared_v4(ds_row + (((ch * 4 + c) ^ (key & 7)) << 4), w[0], w[1], w[2], w[3]);
-      }
-      fence_proxy_async_smem();
-      tc_fence_before();
-      mbar_arrive(bar_ds_full + 8 * bf);
     }
-    // ---------------------------------------------------- epilogue: dV (lanes = keys), this warp's D/2 columns
+    // ---------------------------------------------------- epilogue: dV (lanes = keys)
     mbar_wait(bar_acc_full, 0);
     tc_fence_after();
     {
       const int n_tok = item.k_is_ref ? p.n_ref : p.n_gen;
       const int grow = item.k_row0 + key;
       __nv_bfloat16* base = item.k_is_ref ? p.dv_ref : p.dv_gen;
-      uint4* orow = reinterpret_cast<uint4*>(base + ((size_t(b) * n_tok + grow) * p.heads + h) * D + ch * (D / 2));
+      uint4* orow = reinterpret_cast<uint4*>(base + ((size_t(b) * n_tok + grow) * p.heads + h) * D);
 #pragma unroll
-      for (int c = 0; c < D / 64; ++c) {
+      for (int c = 0; c < D / 32; ++c) {
         uint32_t o[32];
-        tmem_ld32(tmem + lane_off + C::kColDV + ch * (D / 2) + c * 32, o);
+        tmem_ld32(tmem + lane_off + C::kColDV + c * 32, o);
         tmem_wait_ld();
         if (key_valid) {
 #pragma unroll
@@ -245,6 +214,51 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
       }
     }
     tc_fence_before();
+  } else if (warp < 8) {
+    // ================================================= dS warpgroup: dS^T = P^T o (dP^T - D) (thread = key)
+    // P^T is read back from TMEM as the bf16 the dV MMA consumes (S[bf] is not overwritten before the
+    // MMA issuer has seen ds_full of this tile).
+    const int wk = warp - 4;
+    const int key = wk * 32 + lane;
+    const bool key_valid = key < item.k_rows;
+    const uint32_t lane_off = uint32_t(wk * 32) << 16;
+    for (int it = 0; it < n_it; ++it) {
+      const int bf = it & 1, s = it % ST;
+      const uint32_t tP = tmem + lane_off + C::kColS + bf * QT;
+      const uint32_t tDP = tmem + lane_off + C::kColDP;
+      const uint32_t vec = sVec + s * (2 * QT * 4) + QT * 4;  // delta[64]
+      mbar_wait(bar_q_full + 8 * s, (it / ST) & 1);  // acquire the loader's delta writes
+      mbar_wait(bar_p_full + 8 * bf, (it >> 1) & 1);
+      mbar_wait(bar_dp_full, it & 1);
+      tc_fence_after();
+      uint32_t pb[32], dp[2][32];
+      tmem_ld32(tP, pb);
+      tmem_ld32(tDP, dp[0]);
+      tmem_ld32(tDP + 32, dp[1]);
+      tmem_wait_ld();
+      mbar_wait(bar_ds_empty + 8 * bf, ((it >> 1) & 1) ^ 1);  // dK / dQ MMAs of iteration it-2 have read sDs[bf]
+      const uint32_t ds_row = sDs + bf * C::kDsBytes + key * 128;
+#pragma unroll
+      for (int c = 0; c < 8; ++c) {  // 16-byte chunk c = queries [8c, 8c+8)
+        const float4 d0 = ld_shared_f4(vec + (c * 8) * 4);
+        const float4 d1 = ld_shared_f4(vec + (c * 8 + 4) * 4);
+        const float dl[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
+        uint32_t w[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const int q = c * 8 + 2 * k;
+          const uint32_t pp = pb[q >> 1];
+          float a = __uint_as_float(pp << 16) * (__uint_as_float(dp[q >> 5][q & 31]) - dl[2 * k]);
+          float bb = __uint_as_float(pp & 0xffff0000u) * (__uint_as_float(dp[(q + 1) >> 5][(q + 1) & 31]) - dl[2 * k + 1]);
+          if (!key_valid) { a = 0.f; bb = 0.f; }
+          w[k] = pack_bf16(a, bb);
+        }
+        st_shared_v4(ds_row + ((c ^ (key & 7)) << 4), w[0], w[1], w[2], w[3]);
+      }
+      fence_proxy_async_smem();
+      tc_fence_before();
+      mbar_arrive(bar_ds_full + 8 * bf);
+    }
   } else if (warp < 12) {
     // ================================================= reduce warpgroup: dQ^T drain (thread = d), then dK epilogue
     const int wq = warp - 8;
