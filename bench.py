@@ -565,14 +565,90 @@ def load_traffic_all():
         return {}
 
 
+def bench_short(args, w):
+    """--mode short (north_star "cache-bound short-query cases", SURVEY.md 8d auxiliary sweep): cached denoising
+    steps of a few generation rows against the resident reference cache.  Arithmetic intensity ~ N_g FLOP/B is
+    below the ridge (~250 FLOP/B) for N_g <= 256, so the step is judged on HBM GB/s: algorithmic bytes = the
+    resident K/V cache + the step's q/k/v in + o out (+ LSE), over the device time of sra_fwd_kernel + the merge of
+    the key-split partials.  Four rotating sets of generation tensors; the cache alone (>= 0.4 GB) exceeds L2."""
+    import torch
+    from paper_2606_13872_b200 import binding as B
+    from paper_2606_13872_b200 import inputs as I
+    if int(os.environ.get("WORLD_SIZE", "1")) != 1:
+        raise SystemExit("bench.py --mode short is a single-GPU diagnostic")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the SRA path has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    peaks, peaks_kind = load_peaks()
+    ref = {n: I.make_tensor_device(w, n, dev) for n in ("k_ref", "v_ref")}
+    sets = [{n: I.make_tensor_device(w, n, dev, step=s) for n in ("q_gen", "k_gen", "v_gen")} for s in range(4)]
+    o_gen = torch.empty_like(sets[0]["q_gen"])
+    lse_gen = torch.empty((w.batch, w.heads, w.n_gen), device=dev, dtype=torch.float32)
+    ctx = B.sra_create(w.batch, w.heads, w.head_dim, w.n_gen, w.ref_block_offsets)
+    B.sra_set_kernel_timing(ctx, True)
+    B.sra_cache_reference_kv(ctx, ref["k_ref"], ref["v_ref"])
+    n_split, _ = B.sra_split_schedule_copy(ctx)
+    fl = useful_flops(w, include_ref_rows=False)
+    row = w.heads * w.head_dim * 2
+    alg_bytes = B.sra_cache_bytes(ctx) + 4 * w.batch * w.n_gen * row + w.batch * w.heads * w.n_gen * 4
+
+    def step(i):
+        g = sets[i % 4]
+        B.sra_forward(ctx, g["q_gen"], g["k_gen"], g["v_gen"], o_gen, lse_gen=lse_gen)
+
+    for i in range(max(args.warmup, 3)):
+        step(i)
+    torch.cuda.synchronize()
+    launches0 = B.sra_launch_count(ctx)
+    sampler = ClockSampler(0)
+    sampler.start()
+    k_ms = []
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(args.steps):
+        step(i)
+    e1.record()
+    torch.cuda.synchronize()
+    elapsed_ms = e0.elapsed_time(e1)
+    for i in range(min(args.steps, 8)):  # per-kernel device times, one step at a time (reading them synchronises)
+        step(i)
+        ms = B.sra_kernel_time_ms(ctx, B.KERNEL_FWD)
+        if n_split > 1:
+            ms += B.sra_kernel_time_ms(ctx, B.KERNEL_FWD_MERGE)
+        k_ms.append(ms)
+    clocks = sampler.stop()
+    launches = B.sra_launch_count(ctx) - launches0
+    B.sra_destroy(ctx)
+    kernel_ms = statistics.median(k_ms)
+    achieved = alg_bytes / (kernel_ms * 1e-3) / 1e9
+    cfg = config_of(w, args)
+    cfg["step"] = "sra_forward, cached denoising step (q_ref = k_ref = v_ref = NULL): G rows against gen K/V + resident reference cache"
+    cfg["n_split"] = n_split
+    out = {
+        "metric": "sra_short_query_cache_gbs", "value": alg_bytes * args.steps / (elapsed_ms * 1e-3) / 1e9, "unit": "GB/s",
+        "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": elapsed_ms / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": cfg, "useful_tflops": fl * args.steps / (elapsed_ms * 1e-3) / 1e12, "e2e": None,
+        "gpu_launches": int(launches), "clocks": clocks,
+        "roofline": {"bound": "hbm", "kernel": "sra_fwd_kernel<128>" + (" + sra_fwd_merge_kernel<128>" if n_split > 1 else ""),
+                     "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
+                     "peak_kind": f"{peaks_kind} copy bandwidth", "kernel_ms": kernel_ms,
+                     "algorithmic_bytes_per_launch": alg_bytes, "traffic": None},
+        "cpu_baseline": None, "parity": None,
+    }
+    print(json.dumps(out), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default=None, help="default: 720p (--mode fwd), train (--mode train)")
-    ap.add_argument("--mode", default="fwd", choices=["fwd", "train"],
-                    help="fwd: the BASELINE metric (forward layer); train: configs[4] forward + backward")
+    ap.add_argument("--mode", default="fwd", choices=["fwd", "train", "short"],
+                    help="fwd: the BASELINE metric (forward layer); train: configs[4] forward + backward; "
+                         "short: cache-bound short-query cached steps (--workload short128|short512|short2048), HBM roofline")
     ap.add_argument("--train-parity", action="store_true",
                     help="--mode train: also check dQ/dK/dV of one (batch, head) against the oracle (minutes of CPU)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
@@ -582,7 +658,7 @@ def main():
     if args.warmup < 3 and args.impl == "ours":
         log("note: W < 3 warm-up steps breaks the timing rules; use --warmup >= 3 for a reportable number")
     from paper_2606_13872_b200 import inputs as I
-    w = I.WORKLOADS[args.workload or ("train" if args.mode == "train" else "720p")]
+    w = I.WORKLOADS[args.workload or {"train": "train", "short": "short128"}.get(args.mode, "720p")]
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if world != args.gpus and world > 1:
         log(f"note: --gpus {args.gpus} but WORLD_SIZE={world}; using WORLD_SIZE")
@@ -592,6 +668,8 @@ def main():
         bench_reference(args, w)
     elif args.mode == "train":
         bench_train(args, w)
+    elif args.mode == "short":
+        bench_short(args, w)
     else:
         bench_ours(args, w)
 

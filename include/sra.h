@@ -150,6 +150,15 @@ int sra_schedule_info(const sra_ctx* ctx, int32_t* n_gen_items, int32_t* n_ref_i
  * count in *n_items.  Pure host logic - usable without a GPU. */
 int sra_schedule_copy(const sra_ctx* ctx, int32_t* items, int32_t capacity, int32_t* n_items);
 
+/* Short-query schedules (north_star "cache-bound short-query cases"): when a context has fewer generation
+ * slabs than about two per SM, sra_create cuts every generation slab into *n_split key ranges of whole
+ * 128-key tiles; each range runs as its own CTA, writes an fp32 partial (O_s, LSE_s) into a ctx-owned
+ * workspace, and a merge kernel combines them (O = sum_s exp(LSE_s - LSE) O_s).  *n_split == 1 means the
+ * plain schedule of sra_schedule_copy is launched.  With `items` non-NULL the LAUNCHED list is copied
+ * (same 8-int32 layout; q_is_ref bit 0 = reference rows, bits 8.. = split index + 1, 0 for unsplit items):
+ * n_gen_items * n_split split slabs, then the reference items.  Pure host logic - usable without a GPU. */
+int sra_split_schedule_copy(const sra_ctx* ctx, int32_t* n_split, int32_t* items, int32_t capacity, int32_t* n_items);
+
 /* Device bytes held by the resident reference-KV cache (0 before the first cache call). */
 int64_t sra_cache_bytes(const sra_ctx* ctx);
 
@@ -162,7 +171,8 @@ int64_t sra_cache_bytes(const sra_ctx* ctx);
 #define SRA_KERNEL_BWD_PREPROCESS 2 /* a6 */
 #define SRA_KERNEL_BWD_MAIN 3       /* a7 */
 #define SRA_KERNEL_BWD_DQ_FINALIZE 4 /* a8 */
-#define SRA_NUM_KERNELS 5
+#define SRA_KERNEL_FWD_MERGE 5       /* a5': merge of key-split partials (short-query schedules only) */
+#define SRA_NUM_KERNELS 6
 int sra_set_kernel_timing(sra_ctx* ctx, int enable);
 int sra_kernel_time_ms(sra_ctx* ctx, int which, float* ms);
 

@@ -24,7 +24,7 @@ SRA_ERR_OOM = -5
 EXPORTS = (
     "sra_create", "sra_cache_reference_kv", "sra_forward", "sra_forward_host", "sra_backward", "sra_destroy", "sra_useful_flops",
     "sra_schedule_info", "sra_schedule_copy", "sra_cache_bytes", "sra_launch_count", "sra_status_string",
-    "sra_last_error", "sra_set_kernel_timing", "sra_kernel_time_ms",
+    "sra_last_error", "sra_set_kernel_timing", "sra_kernel_time_ms", "sra_split_schedule_copy",
 )
 
 if not os.path.exists(LIB_PATH):
@@ -78,6 +78,9 @@ lib.sra_useful_flops.restype = ctypes.c_int
 lib.sra_schedule_info.argtypes = [_ctx_p, ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32),
                                   ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64)]
 lib.sra_schedule_info.restype = ctypes.c_int
+lib.sra_split_schedule_copy.argtypes = [_ctx_p, ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32), ctypes.c_int32,
+                                        ctypes.POINTER(ctypes.c_int32)]
+lib.sra_split_schedule_copy.restype = ctypes.c_int
 lib.sra_schedule_copy.argtypes = [_ctx_p, ctypes.POINTER(ctypes.c_int32), ctypes.c_int32,
                                   ctypes.POINTER(ctypes.c_int32)]
 lib.sra_schedule_copy.restype = ctypes.c_int
@@ -201,11 +204,28 @@ def sra_schedule_copy(ctx: int):
     return [dict(zip(keys, buf[8 * i:8 * i + 8])) for i in range(n.value)]
 
 
+def sra_split_schedule_copy(ctx: int):
+    """(n_split, launched work items).  n_split == 1: the plain schedule; otherwise every generation slab appears
+    n_split times with disjoint key ranges (`split` = index + 1), followed by the reference items."""
+    ns, n = ctypes.c_int32(), ctypes.c_int32()
+    _check(lib.sra_split_schedule_copy(ctx, ctypes.byref(ns), None, 0, ctypes.byref(n)), ctx)
+    buf = (ctypes.c_int32 * (8 * max(n.value, 1)))()
+    _check(lib.sra_split_schedule_copy(ctx, ctypes.byref(ns), buf, n.value, ctypes.byref(n)), ctx)
+    keys = ("q_is_ref", "q_row0", "q_rows", "seg0_is_ref", "seg0_start", "seg0_len", "seg1_start", "seg1_len")
+    items = []
+    for i in range(n.value):
+        it = dict(zip(keys, buf[8 * i:8 * i + 8]))
+        it["split"] = it["q_is_ref"] >> 8
+        it["q_is_ref"] &= 1
+        items.append(it)
+    return ns.value, items
+
+
 def sra_cache_bytes(ctx: int) -> int:
     return int(lib.sra_cache_bytes(ctx))
 
 
-KERNEL_CACHE_RELAYOUT, KERNEL_FWD, KERNEL_BWD_PREPROCESS, KERNEL_BWD_MAIN, KERNEL_BWD_DQ_FINALIZE = range(5)
+KERNEL_CACHE_RELAYOUT, KERNEL_FWD, KERNEL_BWD_PREPROCESS, KERNEL_BWD_MAIN, KERNEL_BWD_DQ_FINALIZE, KERNEL_FWD_MERGE = range(6)
 
 
 def sra_set_kernel_timing(ctx: int, enable: bool) -> None:

@@ -17,6 +17,7 @@ using sra::BwdItem;
 using sra::FwdItem;
 using sra::kQRowsPerCta;
 using sra::kTile;
+using sra::kNumSms;
 
 
 namespace {
@@ -121,6 +122,50 @@ static void build_schedule(sra_ctx* ctx) {
     }
   }
   ctx->n_ref_items = int(ctx->fwd_items.size()) - ctx->n_gen_items;
+  // Short-query regime (north_star: "cache-bound short-query cases"; SURVEY.md 8d auxiliary sweep): with fewer G
+  // slabs than ~2 per SM the tensor cores are idle and the step is bound by streaming K/V (mostly the resident
+  // reference cache) out of HBM, so every G slab is cut into n_split key ranges of whole tiles; each range runs
+  // as its own CTA and writes an fp32 partial (O_s, LSE_s), merged by sra_fwd_merge_kernel (flash-decoding).
+  ctx->n_split = 1;
+  ctx->split_items.clear();
+  {
+    const long base = long(ctx->n_gen_items) * ctx->cfg.heads * ctx->cfg.batch;
+    const int t0 = (Ng + kTile - 1) / kTile, t1 = (Nr + kTile - 1) / kTile;
+    const int tiles = t0 + t1;
+    if (base < 2 * kNumSms && tiles >= 16) {
+      // Candidates keep >= 8 key tiles per split.  Take the smallest split count that fills whole waves of
+      // 148 CTAs to >= 92 % (fewer partials to write and merge); if even the largest cannot occupy every SM
+      // once, take the largest.
+      const int n_max = std::min(64, tiles / 8);
+      int best = n_max;
+      if (base * n_max >= kNumSms) {
+        double best_eff = 0.0;
+        for (int n = 2; n <= n_max; ++n) {
+          const long ctas = base * n;
+          if (ctas < kNumSms) continue;
+          const long waves = (ctas + kNumSms - 1) / kNumSms;
+          const double eff = double(ctas) / double(waves * kNumSms);
+          if (eff >= 0.92) { best = n; break; }
+          if (eff > best_eff) { best_eff = eff; best = n; }
+        }
+      }
+      ctx->n_split = best;
+    }
+    if (ctx->n_split > 1) {
+      for (int g = 0; g < ctx->n_gen_items; ++g)
+        for (int sp = 0; sp < ctx->n_split; ++sp) {
+          FwdItem it = ctx->fwd_items[g];
+          const int a = int(long(tiles) * sp / ctx->n_split), b = int(long(tiles) * (sp + 1) / ctx->n_split);  // tiles [a, b)
+          const int g0 = std::min(a, t0), g1 = std::min(b, t0);           // generation key tiles [g0, g1)
+          const int r0 = std::max(a, t0) - t0, r1 = std::max(b, t0) - t0; // reference key tiles [r0, r1)
+          it.q_is_ref = (sp + 1) << 8;
+          it.seg0_start = g0 * kTile; it.seg0_len = g1 > g0 ? std::min(Ng, g1 * kTile) - g0 * kTile : 0;
+          it.seg1_start = r0 * kTile; it.seg1_len = r1 > r0 ? std::min(Nr, r1 * kTile) - r0 * kTile : 0;
+          ctx->split_items.push_back(it);
+        }
+      for (int r = 0; r < ctx->n_ref_items; ++r) ctx->split_items.push_back(ctx->fwd_items[ctx->n_gen_items + r]);
+    }
+  }
   // Backward: key tiles.  G key tiles are seen by all G queries; R key tiles of block j additionally by block j's
   // R queries.  Tiles never straddle a block boundary.
   ctx->bwd_items.clear();
@@ -201,6 +246,13 @@ int sra_create(const sra_config* cfg, sra_ctx** out) {
     cudaSetDevice(dev);
     cudaError_t e = cudaMalloc(&ctx->d_fwd_items, ctx->fwd_items.size() * sizeof(FwdItem));
     if (e == cudaSuccess) e = cudaMemcpy(ctx->d_fwd_items, ctx->fwd_items.data(), ctx->fwd_items.size() * sizeof(FwdItem), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && ctx->n_split > 1) {
+      const size_t prow = size_t(ctx->n_split) * cfg->batch * cfg->heads * cfg->n_gen;
+      e = cudaMalloc(&ctx->d_split_items, ctx->split_items.size() * sizeof(FwdItem));
+      if (e == cudaSuccess) e = cudaMemcpy(ctx->d_split_items, ctx->split_items.data(), ctx->split_items.size() * sizeof(FwdItem), cudaMemcpyHostToDevice);
+      if (e == cudaSuccess) e = cudaMalloc(&ctx->ws_part_o, prow * cfg->head_dim * sizeof(float));
+      if (e == cudaSuccess) e = cudaMalloc(&ctx->ws_part_lse, prow * sizeof(float));
+    }
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_bwd_items, ctx->bwd_items.size() * sizeof(BwdItem));
     if (e == cudaSuccess) e = cudaMemcpy(ctx->d_bwd_items, ctx->bwd_items.data(), ctx->bwd_items.size() * sizeof(BwdItem), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { (void)cudaGetLastError(); sra_destroy(ctx); return e == cudaErrorMemoryAllocation ? SRA_ERR_OOM : SRA_ERR_CUDA; }
@@ -214,6 +266,9 @@ void sra_destroy(sra_ctx* ctx) {
   if (ctx->device >= 0) {
     cudaFree(ctx->d_fwd_items);
     cudaFree(ctx->d_bwd_items);
+    cudaFree(ctx->d_split_items);
+    cudaFree(ctx->ws_part_o);
+    cudaFree(ctx->ws_part_lse);
     cudaFree(ctx->cache_k);
     cudaFree(ctx->cache_v);
     cudaFree(ctx->ws_dq);
@@ -300,8 +355,11 @@ int sra_forward(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) {
     if ((rc = sra::make_tmap_bf16(ctx, &maps[5], vr, B, c.n_ref, H, d, use_cache, kTile))) return rc;
   }
   sra::FwdParams p{};
-  p.items = ctx->d_fwd_items;
-  p.n_items = ctx->n_gen_items + (with_ref_rows ? ctx->n_ref_items : 0);
+  const bool split = ctx->n_split > 1;
+  p.items = split ? ctx->d_split_items : ctx->d_fwd_items;
+  p.n_items = ctx->n_gen_items * ctx->n_split + (with_ref_rows ? ctx->n_ref_items : 0);
+  p.part_o = ctx->ws_part_o;
+  p.part_lse = ctx->ws_part_lse;
   p.heads = H; p.batch = B; p.n_gen = c.n_gen; p.n_ref = c.n_ref;
   p.scale = ctx->scale;
   p.scale_log2 = ctx->scale * 1.4426950408889634f;
@@ -318,6 +376,12 @@ int sra_forward(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) {
   }
   if (e != cudaSuccess) return fail_cuda(ctx, e, "sra_fwd_kernel launch");
   ctx->launches += 1;
+  if (split) {
+    sra::KernelTimer kt(ctx, SRA_KERNEL_FWD_MERGE, cudaStream_t(cuda_stream));
+    e = sra::launch_fwd_merge(p, d, ctx->n_split, cudaStream_t(cuda_stream));
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "sra_fwd_merge_kernel launch");
+    ctx->launches += 1;
+  }
   return SRA_OK;
 }
 
@@ -407,6 +471,18 @@ int sra_schedule_copy(const sra_ctx* ctx, int32_t* items, int32_t capacity, int3
     const int n = std::min<int>(capacity, *n_items);
     static_assert(sizeof(FwdItem) == 8 * sizeof(int32_t), "FwdItem layout is part of the ABI");
     std::memcpy(items, ctx->fwd_items.data(), size_t(n) * sizeof(FwdItem));
+  }
+  return SRA_OK;
+}
+
+int sra_split_schedule_copy(const sra_ctx* ctx, int32_t* n_split, int32_t* items, int32_t capacity, int32_t* n_items) {
+  if (!ctx || !n_split) return SRA_ERR_INVALID_ARG;
+  *n_split = ctx->n_split;
+  const std::vector<FwdItem>& v = ctx->n_split > 1 ? ctx->split_items : ctx->fwd_items;
+  if (n_items) *n_items = int32_t(v.size());
+  if (items) {
+    const int n = std::min<int>(capacity, int(v.size()));
+    std::memcpy(items, v.data(), size_t(n) * sizeof(FwdItem));
   }
   return SRA_OK;
 }

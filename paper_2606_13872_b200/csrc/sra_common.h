@@ -7,13 +7,16 @@
 namespace sra {
 
 constexpr int kTile = 128;         // rows per MMA tile (UMMA M = 128; key tile N = 128)
+constexpr int kNumSms = 148;       // B200
 constexpr int kQRowsPerCta = 256;  // two ping-ponged Q tiles per CTA (forward)
 
 // Forward work item: a 256-row query slab and the (up to two) key
 // segments it may see.  G slab: seg0 = all generation keys, seg1 = all reference keys.
 // R slab of block j: seg0 = reference keys [off[j], off[j+1]), seg1 empty.
 struct FwdItem {
-  int32_t q_is_ref;     // 0: rows of Q_g / O_g, 1: rows of Q_r / O_r
+  int32_t q_is_ref;     // bit 0: 0 = rows of Q_g / O_g, 1 = rows of Q_r / O_r;  bits 8..: 0 = the item sees all of
+                        // its keys and writes O / LSE; s + 1 = key split s of a short-query G slab, writes the
+                        // fp32 partial (O_s, LSE_s) that sra_fwd_merge_kernel combines
   int32_t q_row0;       // first row (token index inside its tensor)
   int32_t q_rows;       // valid rows in this slab, 1..256
   int32_t seg0_is_ref;  // which K/V tensors seg0 reads
@@ -45,6 +48,9 @@ struct FwdParams {
   float* lse_ref;  // may be null
   // coordinate order of the K/V reference tensor maps: 1 = head-major cache [B,H,N,d] => (c, n, h, b)
   int32_t ref_kv_head_major;
+  // key-split partials of short-query G slabs (null when the schedule has no splits)
+  float* part_o;    // fp32 [n_split][B][H][n_gen][d]: O_s = P_s V_s / l_s
+  float* part_lse;  // fp32 [n_split][B][H][n_gen]:    LSE_s (natural log of the scaled scores)
 };
 
 constexpr int kBwdQTile = 64;  // query rows per backward iteration (keys per CTA = kTile)

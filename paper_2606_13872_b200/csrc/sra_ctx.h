@@ -20,6 +20,13 @@ struct sra_ctx {
   int n_gen_items = 0, n_ref_items = 0;
   std::vector<sra::BwdItem> bwd_items;
   sra::FwdItem* d_fwd_items = nullptr;
+  // Short-query regime (few G slabs): every G slab is cut into n_split key ranges so that all SMs stream the
+  // K/V cache; split_items = the n_gen_items * n_split split slabs followed by the R items.
+  int n_split = 1;
+  std::vector<sra::FwdItem> split_items;
+  sra::FwdItem* d_split_items = nullptr;
+  float* ws_part_o = nullptr;
+  float* ws_part_lse = nullptr;
   sra::BwdItem* d_bwd_items = nullptr;
   __nv_bfloat16* cache_k = nullptr;  // [B, H, n_ref, d]
   __nv_bfloat16* cache_v = nullptr;
@@ -63,5 +70,6 @@ template <int D>
 cudaError_t launch_bwd(const CUtensorMap* maps, const BwdParams& p, cudaStream_t stream);
 template <int D>
 cudaError_t launch_fwd(const CUtensorMap* maps, const FwdParams& p, cudaStream_t stream);
+cudaError_t launch_fwd_merge(const FwdParams& p, int head_dim, int n_split, cudaStream_t stream);
 int run_backward(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t stream);
 }  // namespace sra

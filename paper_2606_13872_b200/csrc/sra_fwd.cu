@@ -13,6 +13,8 @@
 // columns) aliases the first 64 columns of S_i once the softmax thread holds S_i in registers.
 // Masked tiles are never visited: the key-tile loop walks only the item's visible segments;
 // only the last tile of a segment pays for a column mask (n_valid < 128).
+#include <algorithm>
+
 #include "ptx.cuh"
 #include "sra_common.h"
 
@@ -78,6 +80,8 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
   const int lane = threadIdx.x & 31;
 
   const FwdItem item = p.items[blockIdx.x];
+  const bool q_is_ref = (item.q_is_ref & 1) != 0;
+  const int split = item.q_is_ref >> 8;  // 0: final output; s + 1: key split s of a short-query G slab
   const int h = blockIdx.y;
   const int b = blockIdx.z;
   const int n0 = (item.seg0_len + kTile - 1) / kTile;
@@ -99,7 +103,7 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
     fence_mbar_init();
   }
   if (warp == 9 && lane == 0) {
-    tma_prefetch_desc(item.q_is_ref ? &tm_q_ref : &tm_q_gen);
+    tma_prefetch_desc(q_is_ref ? &tm_q_ref : &tm_q_gen);
     tma_prefetch_desc(item.seg0_is_ref ? &tm_k_ref : &tm_k_gen);
     tma_prefetch_desc(item.seg0_is_ref ? &tm_v_ref : &tm_v_gen);
   }
@@ -259,30 +263,49 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
         const float l_row = l[i] + exchange(l[i]);
         const int row = i * kTile + row_in_tile;
         const bool valid = row < item.q_rows;
-        const int n_tok = item.q_is_ref ? p.n_ref : p.n_gen;
+        const int n_tok = q_is_ref ? p.n_ref : p.n_gen;
         const int grow = item.q_row0 + row;
-        __nv_bfloat16* obase = item.q_is_ref ? p.o_ref : p.o_gen;
+        __nv_bfloat16* obase = q_is_ref ? p.o_ref : p.o_gen;
         uint4* orow = reinterpret_cast<uint4*>(obase + ((size_t(b) * n_tok + grow) * p.heads + h) * D + hh * (D / 2));
         const float inv_l = 1.0f / l_row;
+        if (split == 0) {
 #pragma unroll
-        for (int c = 0; c < D / 64; ++c) {
-          uint32_t o[32];
-          tmem_ld32(tO + c * 32, o);
-          tmem_wait_ld();
-          if (valid) {
+          for (int c = 0; c < D / 64; ++c) {
+            uint32_t o[32];
+            tmem_ld32(tO + c * 32, o);
+            tmem_wait_ld();
+            if (valid) {
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-              uint4 v;
-              v.x = pack_bf16(__uint_as_float(o[8 * q + 0]) * inv_l, __uint_as_float(o[8 * q + 1]) * inv_l);
-              v.y = pack_bf16(__uint_as_float(o[8 * q + 2]) * inv_l, __uint_as_float(o[8 * q + 3]) * inv_l);
-              v.z = pack_bf16(__uint_as_float(o[8 * q + 4]) * inv_l, __uint_as_float(o[8 * q + 5]) * inv_l);
-              v.w = pack_bf16(__uint_as_float(o[8 * q + 6]) * inv_l, __uint_as_float(o[8 * q + 7]) * inv_l);
-              orow[c * 4 + q] = v;
+              for (int q = 0; q < 4; ++q) {
+                uint4 v;
+                v.x = pack_bf16(__uint_as_float(o[8 * q + 0]) * inv_l, __uint_as_float(o[8 * q + 1]) * inv_l);
+                v.y = pack_bf16(__uint_as_float(o[8 * q + 2]) * inv_l, __uint_as_float(o[8 * q + 3]) * inv_l);
+                v.z = pack_bf16(__uint_as_float(o[8 * q + 4]) * inv_l, __uint_as_float(o[8 * q + 5]) * inv_l);
+                v.w = pack_bf16(__uint_as_float(o[8 * q + 6]) * inv_l, __uint_as_float(o[8 * q + 7]) * inv_l);
+                orow[c * 4 + q] = v;
+              }
             }
           }
+          float* lse = q_is_ref ? p.lse_ref : p.lse_gen;
+          if (lse != nullptr && valid && hh == 0) lse[(size_t(b) * p.heads + h) * n_tok + grow] = m_ref[i] * p.scale + __logf(l_row);
+        } else {
+          // key split: fp32 partial (O_s, LSE_s) of generation rows, head-major so the merge kernel streams it
+          const size_t prow = ((size_t(split - 1) * p.batch + b) * p.heads + h) * p.n_gen + grow;
+          float4* dst = reinterpret_cast<float4*>(p.part_o + prow * D + hh * (D / 2));
+#pragma unroll
+          for (int c = 0; c < D / 64; ++c) {
+            uint32_t o[32];
+            tmem_ld32(tO + c * 32, o);
+            tmem_wait_ld();
+            if (valid) {
+#pragma unroll
+              for (int q = 0; q < 8; ++q)
+                dst[c * 8 + q] = make_float4(__uint_as_float(o[4 * q + 0]) * inv_l, __uint_as_float(o[4 * q + 1]) * inv_l,
+                                             __uint_as_float(o[4 * q + 2]) * inv_l, __uint_as_float(o[4 * q + 3]) * inv_l);
+            }
+          }
+          if (valid && hh == 0) p.part_lse[prow] = m_ref[i] * p.scale + __logf(l_row);
         }
-        float* lse = item.q_is_ref ? p.lse_ref : p.lse_gen;
-        if (lse != nullptr && valid && hh == 0) lse[(size_t(b) * p.heads + h) * n_tok + grow] = m_ref[i] * p.scale + __logf(l_row);
         tc_fence_before();
       }
     }
@@ -290,7 +313,7 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
     reg_dec<56>();
     if (warp == 9 && elect_one()) {
       // ===================================================== TMA loader
-      const CUtensorMap* tq = item.q_is_ref ? &tm_q_ref : &tm_q_gen;
+      const CUtensorMap* tq = q_is_ref ? &tm_q_ref : &tm_q_gen;
       mbar_arrive_expect_tx(bar_q_full, n_qt * C::kTileBytes);
       for (int i = 0; i < n_qt; ++i) load_tile<D>(sQ + i * C::kTileBytes, tq, bar_q_full, item.q_row0 + i * kTile, h, b, false);
       int it = 0;
@@ -389,6 +412,67 @@ cudaError_t launch_fwd(const CUtensorMap* maps, const FwdParams& p, cudaStream_t
   }
   dim3 grid(p.n_items, p.heads, p.batch);
   sra_fwd_kernel<D><<<grid, C::kThreads, C::kSmemBytes, stream>>>(maps[0], maps[1], maps[2], maps[3], maps[4], maps[5], p);
+  return cudaGetLastError();
+}
+
+// a5' (short-query schedules only): O = sum_s exp(LSE_s - LSE) O_s with LSE = log sum_s exp(LSE_s); one warp per
+// (batch, token, head) output row, fp32 partials in, bf16 O (RNE) and fp32 LSE out.  HBM-bound and tiny.
+template <int D>
+__global__ void sra_fwd_merge_kernel(const float* __restrict__ part_o, const float* __restrict__ part_lse,
+                                     __nv_bfloat16* __restrict__ o_gen, float* __restrict__ lse_gen, int n_split, int B,
+                                     int H, int n_gen) {
+  const int lane = threadIdx.x & 31;
+  const size_t warp_id = (blockIdx.x * size_t(blockDim.x) + threadIdx.x) >> 5;
+  const size_t n_warps = (gridDim.x * size_t(blockDim.x)) >> 5;
+  const size_t rows = size_t(B) * n_gen * H;
+  const size_t split_stride = size_t(B) * H * n_gen;
+  constexpr int V = D / 32;  // floats per lane
+  for (size_t r = warp_id; r < rows; r += n_warps) {
+    const int h = int(r % H);
+    const size_t t = r / H;
+    const int n = int(t % n_gen);
+    const int b = int(t / n_gen);
+    const size_t prow = (size_t(b) * H + h) * n_gen + n;
+    float m = -INFINITY;
+    for (int s = 0; s < n_split; ++s) m = fmaxf(m, part_lse[s * split_stride + prow]);
+    float acc[V];
+#pragma unroll
+    for (int k = 0; k < V; ++k) acc[k] = 0.f;
+    float wsum = 0.f;
+    for (int s = 0; s < n_split; ++s) {
+      const float w = __expf(part_lse[s * split_stride + prow] - m);
+      wsum += w;
+      const float* src = part_o + (s * split_stride + prow) * D + lane * V;
+      if (V == 4) {
+        const float4 x = *reinterpret_cast<const float4*>(src);
+        acc[0] = fmaf(w, x.x, acc[0]); acc[1] = fmaf(w, x.y, acc[1]); acc[2] = fmaf(w, x.z, acc[2]); acc[3 % V] = fmaf(w, x.w, acc[3 % V]);
+      } else {
+        const float2 x = *reinterpret_cast<const float2*>(src);
+        acc[0] = fmaf(w, x.x, acc[0]); acc[1] = fmaf(w, x.y, acc[1]);
+      }
+    }
+    const float inv = 1.0f / wsum;
+    __nv_bfloat16* dst = o_gen + ((size_t(b) * n_gen + n) * H + h) * D + lane * V;
+    if (V == 4) {
+      uint2 o;
+      o.x = pack_bf16(acc[0] * inv, acc[1] * inv);
+      o.y = pack_bf16(acc[2 % V] * inv, acc[3 % V] * inv);
+      *reinterpret_cast<uint2*>(dst) = o;
+    } else {
+      *reinterpret_cast<uint32_t*>(dst) = pack_bf16(acc[0] * inv, acc[1] * inv);
+    }
+    if (lse_gen != nullptr && lane == 0) lse_gen[prow] = m + __logf(wsum);
+  }
+}
+
+cudaError_t launch_fwd_merge(const FwdParams& p, int head_dim, int n_split, cudaStream_t stream) {
+  const size_t rows = size_t(p.batch) * p.n_gen * p.heads;
+  const int threads = 256;
+  const int blocks = int(std::min<size_t>((rows * 32 + threads - 1) / threads, size_t(148) * 16));
+  if (head_dim == 128)
+    sra_fwd_merge_kernel<128><<<blocks, threads, 0, stream>>>(p.part_o, p.part_lse, p.o_gen, p.lse_gen, n_split, p.batch, p.heads, p.n_gen);
+  else
+    sra_fwd_merge_kernel<64><<<blocks, threads, 0, stream>>>(p.part_o, p.part_lse, p.o_gen, p.lse_gen, n_split, p.batch, p.heads, p.n_gen);
   return cudaGetLastError();
 }
 

@@ -91,6 +91,14 @@ WORKLOADS: Dict[str, SRAWorkload] = {
     # ragged, non-uniform blocks incl. 1-token block and blocks not dividing 128
     "ragged": SRAWorkload("ragged", 2, 3, 128, 333, (1, 130, 257, 64, 200), "B", 0),
     "ragged64": SRAWorkload("ragged64", 1, 2, 64, 300, (77, 128, 129, 5), "peaked", 0),
+    # cache-bound short-query cases (north_star; SURVEY.md 8d auxiliary sweep): few generation rows against the
+    # 40 s reference cache (174,720 tokens, 3.58 GB of K+V); the library splits the keys across CTAs
+    "short128": SRAWorkload("short128", 1, 40, 128, 128, _uniform(112, 1560), "A", 0),
+    "short512": SRAWorkload("short512", 1, 40, 128, 512, _uniform(112, 1560), "A", 0),
+    "short2048": SRAWorkload("short2048", 1, 40, 128, 2048, _uniform(112, 1560), "A", 0),
+    # scaled-down short-query shapes whose schedules are key-split, every row checkable
+    "short_mini": SRAWorkload("short_mini", 1, 2, 128, 100, (1560, 1560, 300), "B", 0),
+    "short_mini64": SRAWorkload("short_mini64", 2, 2, 64, 300, (1000, 1100), "peaked", 0),
 }
 
 

@@ -97,6 +97,45 @@ def test_schedule_covers_exactly_the_mask(n_gen, blocks):
         B.sra_destroy(ctx)
 
 
+@pytest.mark.parametrize("heads,n_gen,blocks", [(40, 128, (1560,) * 112), (40, 512, (1560,) * 112), (2, 100, (1560, 1560, 300)),
+                                                (2, 300, (1000, 1100)), (3, 3120, (1560,) * 3), (40, 2048, (1560,) * 112)])
+def test_split_schedule_partitions_the_keys(heads, n_gen, blocks):
+    """Short-query schedules: the key ranges of a generation slab's splits are whole 128-key tiles, non-empty,
+    disjoint, and together cover every generation and reference key exactly once; reference items are unchanged."""
+    off = [0]
+    for b in blocks:
+        off.append(off[-1] + b)
+    ctx = B.sra_create(1, heads, 128, n_gen, off)
+    try:
+        plain = B.sra_schedule_copy(ctx)
+        n_split, items = B.sra_split_schedule_copy(ctx)
+        info = B.sra_schedule_info(ctx)
+        if n_split == 1:
+            assert [dict(it, split=0) for it in plain] == items
+            assert info["n_gen_items"] * heads >= 2 * 148 or (n_gen + off[-1]) < 16 * 128
+            return
+        assert len(items) == info["n_gen_items"] * n_split + info["n_ref_items"]
+        assert [dict(it, split=0) for it in plain[info["n_gen_items"]:]] == items[info["n_gen_items"] * n_split:]
+        if n_gen + off[-1] <= 6000:
+            C = _covered_pairs(items, n_gen, off[-1])
+            assert np.array_equal(C, sra_oracle.sra_mask(n_gen, off).astype(np.int32))
+        for g in range(info["n_gen_items"]):
+            cov_g, cov_r = np.zeros(n_gen, dtype=np.int32), np.zeros(off[-1], dtype=np.int32)
+            for sp in range(n_split):
+                it = items[g * n_split + sp]
+                cov_g[it["seg0_start"]:it["seg0_start"] + it["seg0_len"]] += 1
+                cov_r[it["seg1_start"]:it["seg1_start"] + it["seg1_len"]] += 1
+            assert (cov_g == 1).all() and (cov_r == 1).all()
+            for sp in range(n_split):
+                it = items[g * n_split + sp]
+                assert it["split"] == sp + 1 and not it["q_is_ref"]
+                assert (it["q_row0"], it["q_rows"]) == (plain[g]["q_row0"], plain[g]["q_rows"])
+                assert it["seg0_start"] % 128 == 0 and it["seg1_start"] % 128 == 0
+                assert it["seg0_len"] + it["seg1_len"] >= 8 * 128 - 127
+    finally:
+        B.sra_destroy(ctx)
+
+
 @pytest.mark.parametrize("name", ["tiny", "480p", "720p", "sweep40s", "train"])
 def test_useful_flops_closed_form(name):
     """sra_useful_flops = 4 d pairs H B with pairs = N_g (N_g + N_r) + sum b_j^2 (tests/golden/pairs.txt)."""

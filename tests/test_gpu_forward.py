@@ -61,6 +61,18 @@ def test_mini720_full():
     _full_parity("mini720")
 
 
+@pytest.mark.parametrize("name", ["short_mini", "short_mini64"])
+def test_key_split_schedule_full(name):
+    """Short-query schedules (keys split across CTAs, fp32 partials, merge kernel): every row vs the oracle."""
+    from paper_2606_13872_b200 import binding as B
+    w = sra_inputs.WORKLOADS[name]
+    ctx = B.sra_create(w.batch, w.heads, w.head_dim, w.n_gen, w.ref_block_offsets)
+    n_split, _ = B.sra_split_schedule_copy(ctx)
+    B.sra_destroy(ctx)
+    assert n_split > 1, "this workload is meant to exercise the key-split path"
+    _full_parity(name)
+
+
 def test_cached_step_skips_ref_rows():
     """q_ref == NULL (PAPER.md:223 cached denoising step): only G rows are produced, one launch."""
     w = sra_inputs.WORKLOADS["ragged"]

@@ -68,7 +68,9 @@ def _forward_sampled(w, heads, n_random=8, steps=1):
                 B.sra_forward(ctx, gen["q_gen"], gen["k_gen"], gen["v_gen"], o_gen, lse_gen=lse_gen)
                 use_rows = rows[rows < w.n_gen]
             torch.cuda.synchronize()
-            assert B.sra_launch_count(ctx) - launches0 == 1, "one forward = one kernel launch, no cache re-copy"
+            n_split, _ = B.sra_split_schedule_copy(ctx)
+            assert B.sra_launch_count(ctx) - launches0 == (1 if n_split == 1 else 2), \
+                "one forward = one kernel launch (+ the partial merge of a key-split schedule), no cache re-copy"
             assert B.sra_cache_bytes(ctx) == cache_bytes
             assert torch.isfinite(o_gen.float()).all()
             tb = _head_bits({**gen, **ref}, heads)
@@ -100,6 +102,13 @@ def test_720p_dist_b():
 def test_long_reference_sweep_endpoints(name):
     """BASELINE.json configs[3]: the 5 s and 40 s (174,720 reference tokens, 3.58 GB cache) ends of the sweep."""
     _forward_sampled(sra_inputs.WORKLOADS[name], heads=[3], n_random=8, steps=2)
+
+
+@pytest.mark.parametrize("name", ["short128", "short512", "short2048"])
+def test_short_query_against_40s_cache(name):
+    """north_star's cache-bound short-query cases: 128 / 512 / 2048 generation rows against the 40 s resident
+    cache; the 128- and 512-row schedules are key-split (partials + merge), 2048 is not."""
+    _forward_sampled(sra_inputs.WORKLOADS[name], heads=[0, 21], n_random=24, steps=2)
 
 
 def test_sweep_cost_is_linear_in_reference_length():
