@@ -132,7 +132,10 @@ static void build_schedule(sra_ctx* ctx) {
     const long base = long(ctx->n_gen_items) * ctx->cfg.heads * ctx->cfg.batch;
     const int t0 = (Ng + kTile - 1) / kTile, t1 = (Nr + kTile - 1) / kTile;
     const int tiles = t0 + t1;
-    if (base < 2 * kNumSms && tiles >= 16) {
+    const long waves0 = (base + kNumSms - 1) / kNumSms;
+    const bool few = base < 2 * kNumSms;                                                    // cache-bound regime
+    const bool ragged_waves = base < 8 * kNumSms && double(base) / double(waves0 * kNumSms) < 0.85;  // e.g. 2.16 waves
+    if ((few || ragged_waves) && tiles >= 16) {
       // Candidates keep >= 8 key tiles per split.  Take the smallest split count that fills whole waves of
       // 148 CTAs to >= 92 % (fewer partials to write and merge); if even the largest cannot occupy every SM
       // once, take the largest.
