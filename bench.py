@@ -640,15 +640,67 @@ def bench_short(args, w):
     print(json.dumps(out), flush=True)
 
 
+def bench_sweep(args):
+    """--mode sweep (BASELINE.json configs[3]; "linear in reference length"): one full forward
+    layer (cache build + G and R rows) at 5 / 10 / 20 / 40 s of reference; fits t(N_r) = a + c N_r to the
+    forward-kernel times and reports R^2 and t(40 s) / t(5 s) (useful-FLOP ratio 3.88; dense concat: 14.4)."""
+    import numpy as np
+    import torch
+    from paper_2606_13872_b200 import binding as B
+    from paper_2606_13872_b200 import inputs as I
+    if int(os.environ.get("WORLD_SIZE", "1")) != 1:
+        raise SystemExit("bench.py --mode sweep is a single-GPU diagnostic")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the SRA path has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    peaks, peaks_kind = load_peaks()
+    pts = []
+    for name in ("sweep5s", "sweep10s", "sweep20s", "sweep40s"):
+        w = I.WORKLOADS[name]
+        t = {n: I.make_tensor_device(w, n, dev) for n in I.TENSOR_ORDER[:6]}
+        o_gen, o_ref = torch.empty_like(t["q_gen"]), torch.empty_like(t["q_ref"])
+        ctx = B.sra_create(w.batch, w.heads, w.head_dim, w.n_gen, w.ref_block_offsets)
+        B.sra_cache_reference_kv(ctx, t["k_ref"], t["v_ref"])
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        for i in range(max(args.warmup, 3) + args.steps):
+            j = i - max(args.warmup, 3)
+            if j >= 0:
+                ev[j][0].record()
+            B.sra_forward(ctx, t["q_gen"], t["k_gen"], t["v_gen"], o_gen, q_ref=t["q_ref"], o_ref=o_ref)
+            if j >= 0:
+                ev[j][1].record()
+        torch.cuda.synchronize()
+        ms = statistics.median(a.elapsed_time(b) for a, b in ev)
+        fl = useful_flops(w)
+        pts.append({"workload": name, "n_ref": w.n_ref, "ms": ms, "useful_tflop": fl / 1e12, "tflops": fl / (ms * 1e-3) / 1e12})
+        B.sra_destroy(ctx)
+        del t, o_gen, o_ref
+        torch.cuda.empty_cache()
+    x = np.array([p["n_ref"] for p in pts], dtype=np.float64)
+    y = np.array([p["ms"] for p in pts], dtype=np.float64)
+    c, a = np.polyfit(x, y, 1)
+    r2 = 1.0 - float(((a + c * x - y) ** 2).sum() / ((y - y.mean()) ** 2).sum())
+    out = {"metric": "sra_fwd_sweep_linearity", "value": r2, "unit": "R^2 of t(N_r) = a + c N_r", "n_gpus": 1,
+           "steps": args.steps, "warmup": max(args.warmup, 3), "higher_is_better": True, "dtype": "bf16", "data": "synthetic",
+           "config": {"workload": "long-reference sweep: 480p gen (32,760) + 5/10/20/40 s reference in 1560-token blocks"},
+           "fit": {"a_ms": float(a), "c_ms_per_ref_token": float(c), "r2": r2, "t40_over_t5": float(y[-1] / y[0]),
+                   "useful_flop_ratio_40_over_5": pts[-1]["useful_tflop"] / pts[0]["useful_tflop"],
+                   "dense_concat_ratio_40_over_5": float(((32760 + x[-1]) / (32760 + x[0])) ** 2)},
+           "points": pts, "peak_sustained_tflops": peaks["bf16_tflops_sustained"], "peak_kind": peaks_kind}
+    print(json.dumps(out), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default=None, help="default: 720p (--mode fwd), train (--mode train)")
-    ap.add_argument("--mode", default="fwd", choices=["fwd", "train", "short"],
+    ap.add_argument("--mode", default="fwd", choices=["fwd", "train", "short", "sweep"],
                     help="fwd: the BASELINE metric (forward layer); train: configs[4] forward + backward; "
-                         "short: cache-bound short-query cached steps (--workload short128|short512|short2048), HBM roofline")
+                         "short: cache-bound short-query cached steps (--workload short128|short512|short2048), HBM roofline; "
+                         "sweep: configs[3] long-reference sweep, linear fit of time vs reference length")
     ap.add_argument("--train-parity", action="store_true",
                     help="--mode train: also check dQ/dK/dV of one (batch, head) against the oracle (minutes of CPU)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
@@ -670,6 +722,8 @@ def main():
         bench_train(args, w)
     elif args.mode == "short":
         bench_short(args, w)
+    elif args.mode == "sweep":
+        bench_sweep(args)
     else:
         bench_ours(args, w)
 
