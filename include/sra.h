@@ -150,6 +150,17 @@ int sra_schedule_info(const sra_ctx* ctx, int32_t* n_gen_items, int32_t* n_ref_i
  * count in *n_items.  Pure host logic - usable without a GPU. */
 int sra_schedule_copy(const sra_ctx* ctx, int32_t* items, int32_t capacity, int32_t* n_items);
 
+/* Sparse validity masking of reference tokens ("skip invalid reference tokens"; SURVEY.md 8f #1,
+ * reading A8).  `valid`: HOST, n_ref bytes, non-zero = valid; NULL = every token valid again.  One mask per
+ * context, shared by all batch items like the block pattern.  An invalid reference token is never a key (for
+ * generation rows or for the reference rows of its block); as a query its output row is 0 and its LSE is -inf;
+ * its gradient rows are 0.  The library compacts: the schedule, the resident cache, the workspaces and the
+ * kernels only ever see the valid tokens (blocks shrink, empty blocks vanish), so invalid tokens cost nothing;
+ * caller tensors keep their [B, n_ref, H, d] shape and are gathered / scattered by row.  Invalidates the
+ * resident cache (call sra_cache_reference_kv again) and synchronises the device.  Usable without a GPU
+ * (host schedule only). */
+int sra_set_reference_validity(sra_ctx* ctx, const uint8_t* valid);
+
 /* Short-query schedules (north_star "cache-bound short-query cases"): when a context has fewer generation
  * slabs than about two per SM, sra_create cuts every generation slab into *n_split key ranges of whole
  * 128-key tiles; each range runs as its own CTA, writes an fp32 partial (O_s, LSE_s) into a ctx-owned

@@ -18,6 +18,12 @@ reading (A1-A5, listed in DESIGN.md):
     backward (standard softmax-attention calculus, paper silent):
     D = rowsum(dO o O); dV = P^T dO; dP = dO V^T; dS = P o (dP - D); dQ = s dS K; dK = s dS^T Q
 
+Sparse validity masking ("skip invalid reference tokens"; SURVEY.md section 8c reading A8,
+section 8f #1): with an optional per-reference-token flag valid[t],
+    M[i][j] = 0 if j in R and not valid[j]     (an invalid token is nobody's key)
+    M[i][:] = 0 if i in R and not valid[i]     (an invalid token's own row is empty)
+    a row with no visible key has O = 0, P = 0, LSE = -inf (the convention of reading A8).
+
 SRA is exact attention under a fixed mask, so the oracle is that definition written
 out: the mask is materialised as an explicit n x n byte matrix, every quantity is
 fp64, nothing is tiled, fused or reordered.  Inputs are bf16 bit patterns (uint16),
@@ -45,8 +51,9 @@ def block_of(t: int, offsets) -> int:
     raise ValueError(f"token {t} outside reference blocks {offsets}")
 
 
-def sra_mask(n_gen: int, ref_block_offsets) -> np.ndarray:
-    """The explicit SRA mask M, uint8 [n, n] with n = n_gen + n_ref, rows/cols [G ; R]."""
+def sra_mask(n_gen: int, ref_block_offsets, valid=None) -> np.ndarray:
+    """The explicit SRA mask M, uint8 [n, n] with n = n_gen + n_ref, rows/cols [G ; R].
+    `valid` (optional, n_ref flags): invalid reference tokens lose their column and their row."""
     off = [int(x) for x in ref_block_offsets] if len(ref_block_offsets) else [0]
     n_ref = off[-1]
     n = n_gen + n_ref
@@ -59,6 +66,11 @@ def sra_mask(n_gen: int, ref_block_offsets) -> np.ndarray:
             for j in range(n_gen, n):
                 if block_of(j - n_gen, off) == bi:
                     M[i, j] = 1
+    if valid is not None:
+        for t in range(n_ref):
+            if not valid[t]:
+                M[:, n_gen + t] = 0
+                M[n_gen + t, :] = 0
     return M
 
 
@@ -68,11 +80,14 @@ def masked_attention(Q, K, V, M, scale):
     vis = M.astype(bool)
     Sm = np.where(vis, S, -np.inf)
     mx = Sm.max(axis=1, keepdims=True)
-    E = np.where(vis, np.exp(Sm - mx), 0.0)
+    empty = ~vis.any(axis=1, keepdims=True)  # rows with no visible key (invalid reference tokens): O = 0, LSE = -inf
+    mx0 = np.where(empty, 0.0, mx)
+    E = np.where(vis, np.exp(np.where(vis, S, 0.0) - mx0), 0.0)
     Z = E.sum(axis=1, keepdims=True)
-    P = E / Z
+    P = E / np.where(empty, 1.0, Z)
     O = P @ V
-    LSE = (mx + np.log(Z))[:, 0]
+    with np.errstate(divide="ignore"):
+        LSE = np.where(empty, -np.inf, mx0 + np.log(np.where(empty, 1.0, Z)))[:, 0]
     return O, LSE, P
 
 
@@ -83,7 +98,7 @@ def _concat_head(x_gen, x_ref, b, h):
     return np.concatenate(parts, axis=0)
 
 
-def sra_forward(q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, ref_block_offsets, scale):
+def sra_forward(q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, ref_block_offsets, scale, valid=None):
     """SRA forward on bf16-bit inputs [B, N, H, d].
 
     Returns dict(o_gen, o_ref, lse_gen, lse_ref): O fp64 [B,N,H,d], LSE fp64 [B,H,N].
@@ -96,7 +111,7 @@ def sra_forward(q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, ref_block_offsets, sca
     Nr = kr.shape[1]
     have_qr = q_ref is not None
     qr = f(q_ref) if have_qr else np.zeros((B, Nr, H, d))
-    M = sra_mask(Ng, ref_block_offsets)
+    M = sra_mask(Ng, ref_block_offsets, valid)
     o = np.zeros((B, Ng + Nr, H, d))
     lse = np.zeros((B, H, Ng + Nr))
     for b in range(B):
@@ -114,14 +129,14 @@ def sra_forward(q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, ref_block_offsets, sca
     return out
 
 
-def sra_backward(q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, do_gen, do_ref, ref_block_offsets, scale):
+def sra_backward(q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, do_gen, do_ref, ref_block_offsets, scale, valid=None):
     """SRA backward on bf16-bit inputs.  Returns dq/dk/dv for G and R, fp64 [B,N,H,d]."""
     f = bf16_bits_to_f64
     qg, kg, vg, qr, kr, vr = f(q_gen), f(k_gen), f(v_gen), f(q_ref), f(k_ref), f(v_ref)
     dog, dor = f(do_gen), f(do_ref)
     B, Ng, H, d = qg.shape
     Nr = kr.shape[1]
-    M = sra_mask(Ng, ref_block_offsets)
+    M = sra_mask(Ng, ref_block_offsets, valid)
     dq = np.zeros((B, Ng + Nr, H, d))
     dk = np.zeros_like(dq)
     dv = np.zeros_like(dq)
@@ -143,6 +158,6 @@ def sra_backward(q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, do_gen, do_ref, ref_b
             "dq_ref": dq[:, Ng:], "dk_ref": dk[:, Ng:], "dv_ref": dv[:, Ng:]}
 
 
-def count_pairs(n_gen: int, ref_block_offsets) -> int:
+def count_pairs(n_gen: int, ref_block_offsets, valid=None) -> int:
     """Number of unmasked (query,key) pairs per (batch, head), counted from the explicit mask."""
-    return int(sra_mask(n_gen, ref_block_offsets).sum(dtype=np.int64))
+    return int(sra_mask(n_gen, ref_block_offsets, valid).sum(dtype=np.int64))

@@ -24,7 +24,7 @@ SRA_ERR_OOM = -5
 EXPORTS = (
     "sra_create", "sra_cache_reference_kv", "sra_forward", "sra_forward_host", "sra_backward", "sra_destroy", "sra_useful_flops",
     "sra_schedule_info", "sra_schedule_copy", "sra_cache_bytes", "sra_launch_count", "sra_status_string",
-    "sra_last_error", "sra_set_kernel_timing", "sra_kernel_time_ms", "sra_split_schedule_copy",
+    "sra_last_error", "sra_set_kernel_timing", "sra_kernel_time_ms", "sra_split_schedule_copy", "sra_set_reference_validity",
 )
 
 if not os.path.exists(LIB_PATH):
@@ -78,6 +78,8 @@ lib.sra_useful_flops.restype = ctypes.c_int
 lib.sra_schedule_info.argtypes = [_ctx_p, ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32),
                                   ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64)]
 lib.sra_schedule_info.restype = ctypes.c_int
+lib.sra_set_reference_validity.argtypes = [_ctx_p, ctypes.c_char_p]
+lib.sra_set_reference_validity.restype = ctypes.c_int
 lib.sra_split_schedule_copy.argtypes = [_ctx_p, ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32), ctypes.c_int32,
                                         ctypes.POINTER(ctypes.c_int32)]
 lib.sra_split_schedule_copy.restype = ctypes.c_int
@@ -219,6 +221,15 @@ def sra_split_schedule_copy(ctx: int):
         it["q_is_ref"] &= 1
         items.append(it)
     return ns.value, items
+
+
+def sra_set_reference_validity(ctx: int, valid) -> None:
+    """sra_set_reference_validity (include/sra.h): `valid` = sequence / array of n_ref truthy values, or None."""
+    if valid is None:
+        _check(lib.sra_set_reference_validity(ctx, None), ctx)
+        return
+    buf = bytes(bytearray(1 if v else 0 for v in valid))
+    _check(lib.sra_set_reference_validity(ctx, buf), ctx)
 
 
 def sra_cache_bytes(ctx: int) -> int:

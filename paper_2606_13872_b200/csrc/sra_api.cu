@@ -4,6 +4,7 @@
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -81,7 +82,8 @@ int make_tmap_bf16(sra_ctx* ctx, CUtensorMap* out, const void* ptr, int B, int N
 // [B, N, H, d] -> [B, H, N, d], 16 bytes per thread (a1: pure HBM copy, 2 * bytes of traffic).
 __global__ void relayout_head_major_kernel(const uint4* __restrict__ src0, const uint4* __restrict__ src1,
                                            uint4* __restrict__ dst0, uint4* __restrict__ dst1, int N, int H, int vec,
-                                           size_t total) {
+                                           size_t total, const int32_t* __restrict__ gidx, int n_src) {
+  // gidx != null: only the valid reference tokens are cached (row n of the cache = source token gidx[n])
   for (size_t i = blockIdx.x * size_t(blockDim.x) + threadIdx.x; i < total; i += size_t(gridDim.x) * blockDim.x) {
     const int c = int(i % vec);
     size_t t = i / vec;
@@ -90,16 +92,116 @@ __global__ void relayout_head_major_kernel(const uint4* __restrict__ src0, const
     const int n = int(t % N);
     const size_t bb = t / N;
     const size_t o = ((bb * H + hh) * size_t(N) + n) * vec + c;
-    dst0[o] = src0[i];
-    dst1[o] = src1[i];
+    const size_t in = gidx ? ((bb * n_src + gidx[n]) * H + hh) * size_t(vec) + c : i;
+    dst0[o] = src0[in];
+    dst1[o] = src1[in];
   }
+}
+
+// Validity path.  dst[b, i, :, :] = src[b, gidx[i], :, :]  (rows of H*d bf16, 16 B per thread)
+__global__ void gather_rows_kernel(const uint4* __restrict__ src, uint4* __restrict__ dst, const int32_t* __restrict__ gidx,
+                                   int n_src, int n_dst, int row_vec, size_t total) {
+  for (size_t i = blockIdx.x * size_t(blockDim.x) + threadIdx.x; i < total; i += size_t(gridDim.x) * blockDim.x) {
+    const int c = int(i % row_vec);
+    const size_t t = i / row_vec;
+    const int n = int(t % n_dst);
+    const size_t b = t / n_dst;
+    dst[i] = src[(b * n_src + gidx[n]) * row_vec + c];
+  }
+}
+// dst[b, n, :, :] = cidx[n] >= 0 ? src[b, cidx[n], :, :] : 0   (every row of dst is written)
+__global__ void expand_rows_kernel(const uint4* __restrict__ src, uint4* __restrict__ dst, const int32_t* __restrict__ cidx,
+                                   int n_src, int n_dst, int row_vec, size_t total) {
+  for (size_t i = blockIdx.x * size_t(blockDim.x) + threadIdx.x; i < total; i += size_t(gridDim.x) * blockDim.x) {
+    const int c = int(i % row_vec);
+    const size_t t = i / row_vec;
+    const int n = int(t % n_dst);
+    const size_t b = t / n_dst;
+    const int k = cidx[n];
+    dst[i] = k >= 0 ? src[(b * n_src + k) * row_vec + c] : make_uint4(0u, 0u, 0u, 0u);
+  }
+}
+// LSE [B*H, n]: gather (compact = 1) or expand with -inf for invalid rows (the empty-row convention)
+__global__ void lse_map_kernel(const float* __restrict__ src, float* __restrict__ dst, const int32_t* __restrict__ idx,
+                               int n_src, int n_dst, size_t total) {
+  for (size_t i = blockIdx.x * size_t(blockDim.x) + threadIdx.x; i < total; i += size_t(gridDim.x) * blockDim.x) {
+    const int n = int(i % n_dst);
+    const size_t bh = i / n_dst;
+    const int k = idx[n];
+    dst[i] = k >= 0 ? src[bh * n_src + k] : -INFINITY;
+  }
+}
+
+static int cbuf_get(sra_ctx* ctx, int slot, void** out) {
+  const sra_config& c = ctx->cfg;
+  if (!ctx->cbuf[slot]) {
+    const size_t bytes = slot == 8 ? size_t(c.batch) * c.heads * std::max(ctx->nr, 1) * 4
+                                   : size_t(c.batch) * std::max(ctx->nr, 1) * c.heads * c.head_dim * 2;
+    if (cudaMalloc(&ctx->cbuf[slot], bytes) != cudaSuccess) {
+      (void)cudaGetLastError();
+      ctx->cbuf[slot] = nullptr;
+      return ctx_fail(ctx, SRA_ERR_OOM, "validity compaction buffer allocation failed");
+    }
+  }
+  *out = ctx->cbuf[slot];
+  return SRA_OK;
+}
+static int grid_for(size_t total) { return int(std::min<size_t>((total + 255) / 256, size_t(148) * 16)); }
+
+int compact_rows(sra_ctx* ctx, int slot, const void* src, const void** out, cudaStream_t stream) {
+  *out = nullptr;
+  if (!src) return SRA_OK;
+  void* dst;
+  if (int rc = cbuf_get(ctx, slot, &dst)) return rc;
+  *out = dst;
+  const sra_config& c = ctx->cfg;
+  const int row_vec = c.heads * c.head_dim / 8;
+  const size_t total = size_t(c.batch) * ctx->nr * row_vec;
+  if (total == 0) return SRA_OK;
+  gather_rows_kernel<<<grid_for(total), 256, 0, stream>>>(static_cast<const uint4*>(src), static_cast<uint4*>(dst), ctx->d_gidx,
+                                                         c.n_ref, ctx->nr, row_vec, total);
+  ctx->launches += 1;
+  return cudaGetLastError() == cudaSuccess ? SRA_OK : ctx_fail(ctx, SRA_ERR_CUDA, "gather_rows launch failed");
+}
+int compact_lse(sra_ctx* ctx, const float* src, const float** out, cudaStream_t stream) {
+  *out = nullptr;
+  if (!src) return SRA_OK;
+  void* dst;
+  if (int rc = cbuf_get(ctx, 8, &dst)) return rc;
+  *out = static_cast<const float*>(dst);
+  const sra_config& c = ctx->cfg;
+  const size_t total = size_t(c.batch) * c.heads * ctx->nr;
+  if (total == 0) return SRA_OK;
+  lse_map_kernel<<<grid_for(total), 256, 0, stream>>>(src, static_cast<float*>(dst), ctx->d_gidx, c.n_ref, ctx->nr, total);
+  ctx->launches += 1;
+  return cudaGetLastError() == cudaSuccess ? SRA_OK : ctx_fail(ctx, SRA_ERR_CUDA, "lse gather launch failed");
+}
+int compact_out(sra_ctx* ctx, int slot, void** out) { return cbuf_get(ctx, slot, out); }
+int expand_rows(sra_ctx* ctx, int slot, void* dst, cudaStream_t stream) {
+  if (!dst) return SRA_OK;
+  const sra_config& c = ctx->cfg;
+  const int row_vec = c.heads * c.head_dim / 8;
+  const size_t total = size_t(c.batch) * c.n_ref * row_vec;
+  expand_rows_kernel<<<grid_for(total), 256, 0, stream>>>(static_cast<const uint4*>(ctx->cbuf[slot]), static_cast<uint4*>(dst),
+                                                         ctx->d_cidx, ctx->nr, c.n_ref, row_vec, total);
+  ctx->launches += 1;
+  return cudaGetLastError() == cudaSuccess ? SRA_OK : ctx_fail(ctx, SRA_ERR_CUDA, "expand_rows launch failed");
+}
+int expand_lse(sra_ctx* ctx, float* dst, cudaStream_t stream) {
+  if (!dst) return SRA_OK;
+  const sra_config& c = ctx->cfg;
+  const size_t total = size_t(c.batch) * c.heads * c.n_ref;
+  lse_map_kernel<<<grid_for(total), 256, 0, stream>>>(static_cast<const float*>(ctx->cbuf[8]), dst, ctx->d_cidx, ctx->nr, c.n_ref, total);
+  ctx->launches += 1;
+  return cudaGetLastError() == cudaSuccess ? SRA_OK : ctx_fail(ctx, SRA_ERR_CUDA, "lse expand launch failed");
 }
 
 }  // namespace sra
 
 // ------------------------------------------------------------------------------------------------ schedule
 static void build_schedule(sra_ctx* ctx) {
-  const int Ng = ctx->cfg.n_gen, Nr = ctx->cfg.n_ref;
+  const int Ng = ctx->cfg.n_gen, Nr = ctx->nr;
+  const std::vector<int32_t>& off = ctx->offe;
   ctx->fwd_items.clear();
   // G slabs: every generation key tile, then every reference key tile.
   for (int r0 = 0; r0 < Ng; r0 += kQRowsPerCta) {
@@ -111,8 +213,8 @@ static void build_schedule(sra_ctx* ctx) {
   }
   ctx->n_gen_items = int(ctx->fwd_items.size());
   // R slabs: only the keys of the slab's own block ("reference tokens only self-attend").
-  for (int j = 0; j + 1 < int(ctx->off.size()); ++j) {
-    const int s = ctx->off[j], e = ctx->off[j + 1];
+  for (int j = 0; j + 1 < int(off.size()); ++j) {
+    const int s = off[j], e = off[j + 1];
     for (int r0 = s; r0 < e; r0 += kQRowsPerCta) {
       FwdItem it{};
       it.q_is_ref = 1; it.q_row0 = r0; it.q_rows = std::min(kQRowsPerCta, e - r0);
@@ -177,8 +279,8 @@ static void build_schedule(sra_ctx* ctx) {
     it.k_is_ref = 0; it.k_row0 = k0; it.k_rows = std::min(kTile, Ng - k0);
     ctx->bwd_items.push_back(it);
   }
-  for (int j = 0; j + 1 < int(ctx->off.size()); ++j) {
-    const int s = ctx->off[j], e = ctx->off[j + 1];
+  for (int j = 0; j + 1 < int(off.size()); ++j) {
+    const int s = off[j], e = off[j + 1];
     for (int k0 = s; k0 < e; k0 += kTile) {
       BwdItem it{};
       it.k_is_ref = 1; it.k_row0 = k0; it.k_rows = std::min(kTile, e - k0);
@@ -186,6 +288,28 @@ static void build_schedule(sra_ctx* ctx) {
       ctx->bwd_items.push_back(it);
     }
   }
+}
+
+// (Re)allocates the device copies of the schedule and the key-split workspace.
+static int upload_schedule(sra_ctx* ctx) {
+  const sra_config& c = ctx->cfg;
+  cudaFree(ctx->d_fwd_items); cudaFree(ctx->d_bwd_items); cudaFree(ctx->d_split_items);
+  cudaFree(ctx->ws_part_o); cudaFree(ctx->ws_part_lse);
+  ctx->d_fwd_items = nullptr; ctx->d_bwd_items = nullptr; ctx->d_split_items = nullptr;
+  ctx->ws_part_o = nullptr; ctx->ws_part_lse = nullptr;
+  cudaError_t e = cudaMalloc(&ctx->d_fwd_items, ctx->fwd_items.size() * sizeof(FwdItem));
+  if (e == cudaSuccess) e = cudaMemcpy(ctx->d_fwd_items, ctx->fwd_items.data(), ctx->fwd_items.size() * sizeof(FwdItem), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess && ctx->n_split > 1) {
+    const size_t prow = size_t(ctx->n_split) * c.batch * c.heads * c.n_gen;
+    e = cudaMalloc(&ctx->d_split_items, ctx->split_items.size() * sizeof(FwdItem));
+    if (e == cudaSuccess) e = cudaMemcpy(ctx->d_split_items, ctx->split_items.data(), ctx->split_items.size() * sizeof(FwdItem), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->ws_part_o, prow * c.head_dim * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->ws_part_lse, prow * sizeof(float));
+  }
+  if (e == cudaSuccess) e = cudaMalloc(&ctx->d_bwd_items, ctx->bwd_items.size() * sizeof(BwdItem));
+  if (e == cudaSuccess) e = cudaMemcpy(ctx->d_bwd_items, ctx->bwd_items.data(), ctx->bwd_items.size() * sizeof(BwdItem), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) { (void)cudaGetLastError(); return e == cudaErrorMemoryAllocation ? SRA_ERR_OOM : SRA_ERR_CUDA; }
+  return SRA_OK;
 }
 
 // ------------------------------------------------------------------------------------------------ C ABI
@@ -227,6 +351,8 @@ int sra_create(const sra_config* cfg, sra_ctx** out) {
   for (int j = 0; j < cfg->n_ref_blocks; ++j) ctx->off.push_back(cfg->ref_block_offsets[j + 1]);
   ctx->cfg.ref_block_offsets = nullptr;
   ctx->scale = cfg->softmax_scale > 0.f ? cfg->softmax_scale : 1.0f / std::sqrt(float(cfg->head_dim));
+  ctx->nr = cfg->n_ref;
+  ctx->offe = ctx->off;
   build_schedule(ctx);
 
   // Device discovery.  Without a usable CUDA device the ctx is host-only: the schedule can be inspected, every
@@ -247,18 +373,7 @@ int sra_create(const sra_config* cfg, sra_ctx** out) {
   ctx->sm100 = (prop.major == 10);
   if (ctx->sm100) {
     cudaSetDevice(dev);
-    cudaError_t e = cudaMalloc(&ctx->d_fwd_items, ctx->fwd_items.size() * sizeof(FwdItem));
-    if (e == cudaSuccess) e = cudaMemcpy(ctx->d_fwd_items, ctx->fwd_items.data(), ctx->fwd_items.size() * sizeof(FwdItem), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess && ctx->n_split > 1) {
-      const size_t prow = size_t(ctx->n_split) * cfg->batch * cfg->heads * cfg->n_gen;
-      e = cudaMalloc(&ctx->d_split_items, ctx->split_items.size() * sizeof(FwdItem));
-      if (e == cudaSuccess) e = cudaMemcpy(ctx->d_split_items, ctx->split_items.data(), ctx->split_items.size() * sizeof(FwdItem), cudaMemcpyHostToDevice);
-      if (e == cudaSuccess) e = cudaMalloc(&ctx->ws_part_o, prow * cfg->head_dim * sizeof(float));
-      if (e == cudaSuccess) e = cudaMalloc(&ctx->ws_part_lse, prow * sizeof(float));
-    }
-    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_bwd_items, ctx->bwd_items.size() * sizeof(BwdItem));
-    if (e == cudaSuccess) e = cudaMemcpy(ctx->d_bwd_items, ctx->bwd_items.data(), ctx->bwd_items.size() * sizeof(BwdItem), cudaMemcpyHostToDevice);
-    if (e != cudaSuccess) { (void)cudaGetLastError(); sra_destroy(ctx); return e == cudaErrorMemoryAllocation ? SRA_ERR_OOM : SRA_ERR_CUDA; }
+    if (int rc = upload_schedule(ctx)) { sra_destroy(ctx); return rc; }
   }
   *out = ctx;
   return SRA_OK;
@@ -272,6 +387,9 @@ void sra_destroy(sra_ctx* ctx) {
     cudaFree(ctx->d_split_items);
     cudaFree(ctx->ws_part_o);
     cudaFree(ctx->ws_part_lse);
+    cudaFree(ctx->d_gidx);
+    cudaFree(ctx->d_cidx);
+    for (void* q : ctx->cbuf) cudaFree(q);
     cudaFree(ctx->cache_k);
     cudaFree(ctx->cache_v);
     cudaFree(ctx->ws_dq);
@@ -299,7 +417,8 @@ int sra_cache_reference_kv(sra_ctx* ctx, const void* k_ref, const void* v_ref, v
   if (ctx->cfg.n_ref == 0) return SRA_OK;
   if (!k_ref || !v_ref) return fail(ctx, SRA_ERR_INVALID_ARG, "k_ref / v_ref must be non-NULL");
   const sra_config& c = ctx->cfg;
-  const size_t elems = size_t(c.batch) * c.n_ref * c.heads * c.head_dim;
+  if (ctx->nr == 0) { ctx->cache_valid = true; return SRA_OK; }  // every reference token is invalid: nothing to cache
+  const size_t elems = size_t(c.batch) * ctx->nr * c.heads * c.head_dim;
   if (!ctx->cache_k) {
     cudaError_t e = cudaMalloc(&ctx->cache_k, elems * 2);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->cache_v, elems * 2);
@@ -318,7 +437,7 @@ int sra_cache_reference_kv(sra_ctx* ctx, const void* k_ref, const void* v_ref, v
     sra::KernelTimer kt(ctx, SRA_KERNEL_CACHE_RELAYOUT, cudaStream_t(cuda_stream));
     sra::relayout_head_major_kernel<<<blocks, threads, 0, cudaStream_t(cuda_stream)>>>(
         static_cast<const uint4*>(k_ref), static_cast<const uint4*>(v_ref), reinterpret_cast<uint4*>(ctx->cache_k),
-        reinterpret_cast<uint4*>(ctx->cache_v), c.n_ref, c.heads, vec, total);
+        reinterpret_cast<uint4*>(ctx->cache_v), ctx->nr, c.heads, vec, total, ctx->has_valid ? ctx->d_gidx : nullptr, c.n_ref);
     e = cudaGetLastError();
   }
   if (e != cudaSuccess) return fail_cuda(ctx, e, "cache relayout launch");
@@ -326,6 +445,8 @@ int sra_cache_reference_kv(sra_ctx* ctx, const void* k_ref, const void* v_ref, v
   ctx->cache_valid = true;
   return SRA_OK;
 }
+
+static int forward_core(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream);
 
 int sra_forward(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) {
   if (!ctx) return SRA_ERR_INVALID_ARG;
@@ -343,6 +464,37 @@ int sra_forward(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) {
   for (const void* q : ptrs)
     if (q && (reinterpret_cast<uintptr_t>(q) & 15)) return fail(ctx, SRA_ERR_INVALID_ARG, "tensor pointers must be 16-byte aligned");
 
+  if (!ctx->has_valid || c.n_ref == 0) return forward_core(ctx, a, cuda_stream);
+  // Validity path: the kernels run on the compacted reference; invalid reference rows get
+  // O = 0, LSE = -inf.
+  cudaStream_t st = cudaStream_t(cuda_stream);
+  sra_fwd_args e = *a;
+  int rc;
+  if ((rc = sra::compact_rows(ctx, 0, a->q_ref, &e.q_ref, st))) return rc;
+  if ((rc = sra::compact_rows(ctx, 1, a->k_ref, &e.k_ref, st))) return rc;
+  if ((rc = sra::compact_rows(ctx, 2, a->v_ref, &e.v_ref, st))) return rc;
+  e.o_ref = nullptr; e.lse_ref = nullptr;
+  if (with_ref_rows) {
+    void* q;
+    if ((rc = sra::compact_out(ctx, 3, &q))) return rc;
+    e.o_ref = q;
+    if (a->lse_ref) { if ((rc = sra::compact_out(ctx, 8, &q))) return rc; e.lse_ref = static_cast<float*>(q); }
+  }
+  if ((rc = forward_core(ctx, &e, cuda_stream))) return rc;
+  if (with_ref_rows) {
+    if ((rc = sra::expand_rows(ctx, 3, a->o_ref, st))) return rc;
+    if (a->lse_ref && (rc = sra::expand_lse(ctx, a->lse_ref, st))) return rc;
+  }
+  return SRA_OK;
+}
+
+// The launch itself, on the effective (validity-compacted) reference: `a` holds device pointers whose reference
+// tensors have nr rows.
+static int forward_core(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) {
+  const sra_config& c = ctx->cfg;
+  const int nr = ctx->nr;
+  const bool with_ref_rows = a->q_ref != nullptr && nr > 0;
+  const bool use_cache = nr > 0 && a->k_ref == nullptr;
   CUtensorMap maps[6];
   const int B = c.batch, H = c.heads, d = c.head_dim;
   int rc;
@@ -350,12 +502,12 @@ int sra_forward(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) {
   if ((rc = sra::make_tmap_bf16(ctx, &maps[1], a->k_gen, B, c.n_gen, H, d, false, kTile))) return rc;
   if ((rc = sra::make_tmap_bf16(ctx, &maps[2], a->v_gen, B, c.n_gen, H, d, false, kTile))) return rc;
   maps[3] = maps[0]; maps[4] = maps[1]; maps[5] = maps[2];  // placeholders when n_ref == 0 (never dereferenced)
-  if (c.n_ref > 0) {
-    if (with_ref_rows && (rc = sra::make_tmap_bf16(ctx, &maps[3], a->q_ref, B, c.n_ref, H, d, false, kTile))) return rc;
+  if (nr > 0) {
+    if (with_ref_rows && (rc = sra::make_tmap_bf16(ctx, &maps[3], a->q_ref, B, nr, H, d, false, kTile))) return rc;
     const void* kr = use_cache ? ctx->cache_k : a->k_ref;
     const void* vr = use_cache ? ctx->cache_v : a->v_ref;
-    if ((rc = sra::make_tmap_bf16(ctx, &maps[4], kr, B, c.n_ref, H, d, use_cache, kTile))) return rc;
-    if ((rc = sra::make_tmap_bf16(ctx, &maps[5], vr, B, c.n_ref, H, d, use_cache, kTile))) return rc;
+    if ((rc = sra::make_tmap_bf16(ctx, &maps[4], kr, B, nr, H, d, use_cache, kTile))) return rc;
+    if ((rc = sra::make_tmap_bf16(ctx, &maps[5], vr, B, nr, H, d, use_cache, kTile))) return rc;
   }
   sra::FwdParams p{};
   const bool split = ctx->n_split > 1;
@@ -363,7 +515,7 @@ int sra_forward(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) {
   p.n_items = ctx->n_gen_items * ctx->n_split + (with_ref_rows ? ctx->n_ref_items : 0);
   p.part_o = ctx->ws_part_o;
   p.part_lse = ctx->ws_part_lse;
-  p.heads = H; p.batch = B; p.n_gen = c.n_gen; p.n_ref = c.n_ref;
+  p.heads = H; p.batch = B; p.n_gen = c.n_gen; p.n_ref = nr;
   p.scale = ctx->scale;
   p.scale_log2 = ctx->scale * 1.4426950408889634f;
   p.o_gen = static_cast<__nv_bfloat16*>(a->o_gen);
@@ -440,10 +592,10 @@ int sra_backward(sra_ctx* ctx, const sra_bwd_args* a, void* cuda_stream) {
 int sra_useful_flops(const sra_ctx* ctx, int include_ref_rows, int backward, double* out) {
   if (!ctx || !out) return SRA_ERR_INVALID_ARG;
   const sra_config& c = ctx->cfg;
-  double pairs = double(c.n_gen) * (double(c.n_gen) + double(c.n_ref));
+  double pairs = double(c.n_gen) * (double(c.n_gen) + double(ctx->nr));  // invalid reference tokens are not useful work
   if (include_ref_rows)
-    for (size_t j = 0; j + 1 < ctx->off.size(); ++j) {
-      const double bsz = double(ctx->off[j + 1] - ctx->off[j]);
+    for (size_t j = 0; j + 1 < ctx->offe.size(); ++j) {
+      const double bsz = double(ctx->offe[j + 1] - ctx->offe[j]);
       pairs += bsz * bsz;
     }
   *out = 4.0 * c.head_dim * pairs * c.heads * c.batch * (backward ? 2.5 : 1.0);
@@ -490,10 +642,48 @@ int sra_split_schedule_copy(const sra_ctx* ctx, int32_t* n_split, int32_t* items
   return SRA_OK;
 }
 
+int sra_set_reference_validity(sra_ctx* ctx, const uint8_t* valid) {
+  if (!ctx) return SRA_ERR_INVALID_ARG;
+  ctx->err.clear();
+  const sra_config& c = ctx->cfg;
+  std::vector<int32_t> gidx, cidx(size_t(std::max(c.n_ref, 0)), -1), offe(1, 0);
+  bool all = true;
+  for (size_t j = 0; j + 1 < ctx->off.size(); ++j) {
+    int cnt = 0;
+    for (int t = ctx->off[j]; t < ctx->off[j + 1]; ++t) {
+      if (!valid || valid[t]) { cidx[t] = int32_t(gidx.size()); gidx.push_back(t); ++cnt; } else all = false;
+    }
+    if (cnt > 0) offe.push_back(offe.back() + cnt);  // a block with no valid token disappears
+  }
+  ctx->has_valid = !all;
+  ctx->nr = int(gidx.size());
+  ctx->offe = all ? ctx->off : offe;
+  ctx->h_gidx = gidx;
+  build_schedule(ctx);
+  ctx->cache_valid = false;  // the resident cache holds the previous compaction
+  if (ctx->device >= 0 && ctx->sm100) {
+    cudaSetDevice(ctx->device);
+    cudaDeviceSynchronize();
+    cudaFree(ctx->cache_k); cudaFree(ctx->cache_v); ctx->cache_k = ctx->cache_v = nullptr;
+    cudaFree(ctx->ws_dq); cudaFree(ctx->ws_delta); cudaFree(ctx->ws_lse2); ctx->ws_dq = ctx->ws_delta = ctx->ws_lse2 = nullptr;
+    for (void*& q : ctx->cbuf) { cudaFree(q); q = nullptr; }
+    cudaFree(ctx->d_gidx); cudaFree(ctx->d_cidx); ctx->d_gidx = ctx->d_cidx = nullptr;
+    if (int rc = upload_schedule(ctx)) return fail(ctx, rc, "schedule upload failed");
+    if (ctx->has_valid) {
+      cudaError_t e = cudaMalloc(&ctx->d_gidx, std::max<size_t>(gidx.size(), 1) * 4);
+      if (e == cudaSuccess) e = cudaMalloc(&ctx->d_cidx, std::max<size_t>(cidx.size(), 1) * 4);
+      if (e == cudaSuccess && !gidx.empty()) e = cudaMemcpy(ctx->d_gidx, gidx.data(), gidx.size() * 4, cudaMemcpyHostToDevice);
+      if (e == cudaSuccess && !cidx.empty()) e = cudaMemcpy(ctx->d_cidx, cidx.data(), cidx.size() * 4, cudaMemcpyHostToDevice);
+      if (e != cudaSuccess) return fail_cuda(ctx, e, "validity index upload");
+    }
+  }
+  return SRA_OK;
+}
+
 int64_t sra_cache_bytes(const sra_ctx* ctx) {
   if (!ctx || !ctx->cache_k) return 0;
   const sra_config& c = ctx->cfg;
-  return int64_t(2) * c.batch * c.n_ref * c.heads * c.head_dim * 2;
+  return int64_t(2) * c.batch * ctx->nr * c.heads * c.head_dim * 2;
 }
 
 int sra_set_kernel_timing(sra_ctx* ctx, int enable) {

@@ -523,6 +523,8 @@ cudaError_t launch_bwd(const CUtensorMap* m, const BwdParams& p, cudaStream_t st
 template cudaError_t launch_bwd<128>(const CUtensorMap*, const BwdParams&, cudaStream_t);
 
 // ------------------------------------------------------------------------------------------------ host driver
+static int run_backward_core(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t stream);
+
 int run_backward(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t stream) {
   const sra_config& c = ctx->cfg;
   const int B = c.batch, H = c.heads, d = c.head_dim;
@@ -541,7 +543,36 @@ int run_backward(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t stream) {
   for (const void* q : ptrs)
     if (q && (reinterpret_cast<uintptr_t>(q) & 15)) return ctx_fail(ctx, SRA_ERR_INVALID_ARG, "tensor pointers must be 16-byte aligned");
 
-  const int n_cat = c.n_gen + c.n_ref;
+  if (!ctx->has_valid || c.n_ref == 0) return run_backward_core(ctx, a, stream);
+  // Validity path: gather the valid reference rows, run on the compacted reference, scatter the
+  // reference gradients back (rows of invalid tokens are zero).
+  sra_bwd_args v = *a;
+  int rc;
+  if ((rc = compact_rows(ctx, 0, a->q_ref, &v.q_ref, stream))) return rc;
+  if ((rc = compact_rows(ctx, 1, a->k_ref, &v.k_ref, stream))) return rc;
+  if ((rc = compact_rows(ctx, 2, a->v_ref, &v.v_ref, stream))) return rc;
+  if ((rc = compact_rows(ctx, 3, a->o_ref, &v.o_ref, stream))) return rc;
+  if ((rc = compact_rows(ctx, 4, a->do_ref, &v.do_ref, stream))) return rc;
+  if ((rc = compact_lse(ctx, a->lse_ref, &v.lse_ref, stream))) return rc;
+  if ((rc = compact_out(ctx, 5, &v.dq_ref))) return rc;
+  if ((rc = compact_out(ctx, 6, &v.dk_ref))) return rc;
+  if ((rc = compact_out(ctx, 7, &v.dv_ref))) return rc;
+  if ((rc = run_backward_core(ctx, &v, stream))) return rc;
+  if ((rc = expand_rows(ctx, 5, a->dq_ref, stream))) return rc;
+  if ((rc = expand_rows(ctx, 6, a->dk_ref, stream))) return rc;
+  if ((rc = expand_rows(ctx, 7, a->dv_ref, stream))) return rc;
+  return SRA_OK;
+}
+
+// The launches themselves, on the effective (validity-compacted) reference.
+static int run_backward_core(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t stream) {
+  const sra_config& c = ctx->cfg;
+  const int B = c.batch, H = c.heads, d = c.head_dim;
+  const int nr = ctx->nr;
+  const bool has_ref = nr > 0;
+  const bool use_cache = has_ref && a->k_ref == nullptr;
+  cudaError_t e;
+  const int n_cat = c.n_gen + nr;
   const int n_pad = (n_cat + 63) / 64 * 64;
   const size_t vec_bytes = size_t(B) * H * n_pad * 4;
   const size_t dq_bytes = vec_bytes * d;
@@ -557,7 +588,7 @@ int run_backward(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t stream) {
     }
     ctx->ws_dq_bytes = dq_bytes;
   }
-  cudaError_t e = cudaMemsetAsync(ctx->ws_dq, 0, dq_bytes, stream);
+  e = cudaMemsetAsync(ctx->ws_dq, 0, dq_bytes, stream);
   if (e != cudaSuccess) return ctx_fail_cuda(ctx, e, "dQ workspace memset");
 
   {  // a6
@@ -568,7 +599,7 @@ int run_backward(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t stream) {
     sra_bwd_preprocess_kernel<128><<<blocks, threads, 0, stream>>>(
         static_cast<const __nv_bfloat16*>(a->o_gen), static_cast<const __nv_bfloat16*>(a->do_gen), a->lse_gen,
         static_cast<const __nv_bfloat16*>(a->o_ref), static_cast<const __nv_bfloat16*>(a->do_ref), a->lse_ref,
-        ctx->ws_delta, ctx->ws_lse2, B, H, c.n_gen, c.n_ref, n_pad);
+        ctx->ws_delta, ctx->ws_lse2, B, H, c.n_gen, nr, n_pad);
     if ((e = cudaGetLastError()) != cudaSuccess) return ctx_fail_cuda(ctx, e, "bwd preprocess launch");
     ctx->launches += 1;
   }
@@ -581,18 +612,18 @@ int run_backward(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t stream) {
   if ((rc = make_tmap_bf16(ctx, &m[5], a->v_gen, B, c.n_gen, H, d, false, kTile))) return rc;
   m[2] = m[0]; m[3] = m[1]; m[6] = m[4]; m[7] = m[5];
   if (has_ref) {
-    if ((rc = make_tmap_bf16(ctx, &m[2], a->q_ref, B, c.n_ref, H, d, false, kBwdQTile))) return rc;
-    if ((rc = make_tmap_bf16(ctx, &m[3], a->do_ref, B, c.n_ref, H, d, false, kBwdQTile))) return rc;
+    if ((rc = make_tmap_bf16(ctx, &m[2], a->q_ref, B, nr, H, d, false, kBwdQTile))) return rc;
+    if ((rc = make_tmap_bf16(ctx, &m[3], a->do_ref, B, nr, H, d, false, kBwdQTile))) return rc;
     const void* kr = use_cache ? ctx->cache_k : a->k_ref;
     const void* vr = use_cache ? ctx->cache_v : a->v_ref;
-    if ((rc = make_tmap_bf16(ctx, &m[6], kr, B, c.n_ref, H, d, use_cache, kTile))) return rc;
-    if ((rc = make_tmap_bf16(ctx, &m[7], vr, B, c.n_ref, H, d, use_cache, kTile))) return rc;
+    if ((rc = make_tmap_bf16(ctx, &m[6], kr, B, nr, H, d, use_cache, kTile))) return rc;
+    if ((rc = make_tmap_bf16(ctx, &m[7], vr, B, nr, H, d, use_cache, kTile))) return rc;
   }
 
   BwdParams p{};
   p.items = ctx->d_bwd_items;
   p.n_items = int(ctx->bwd_items.size());
-  p.heads = H; p.batch = B; p.n_gen = c.n_gen; p.n_ref = c.n_ref; p.n_pad = n_pad;
+  p.heads = H; p.batch = B; p.n_gen = c.n_gen; p.n_ref = nr; p.n_pad = n_pad;
   p.scale = ctx->scale;
   p.scale_log2 = ctx->scale * 1.4426950408889634f;
   p.lse2 = ctx->ws_lse2; p.delta = ctx->ws_delta; p.dq_ws = ctx->ws_dq;
@@ -613,7 +644,7 @@ int run_backward(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t stream) {
     KernelTimer kt(ctx, SRA_KERNEL_BWD_DQ_FINALIZE, stream);
     sra_bwd_dq_finalize_kernel<128><<<blocks, threads, 0, stream>>>(ctx->ws_dq, static_cast<__nv_bfloat16*>(a->dq_gen),
                                                                    static_cast<__nv_bfloat16*>(a->dq_ref), B, H, c.n_gen,
-                                                                   c.n_ref, n_pad, ctx->scale);
+                                                                   nr, n_pad, ctx->scale);
     if ((e = cudaGetLastError()) != cudaSuccess) return ctx_fail_cuda(ctx, e, "dQ finalize launch");
     ctx->launches += 1;
   }

@@ -13,6 +13,16 @@
 struct sra_ctx {
   sra_config cfg{};
   std::vector<int32_t> off;  // n_ref_blocks + 1
+  // Reference validity (sra_set_reference_validity): kernels, schedule, cache and workspaces see the
+  // COMPACTED reference (valid tokens only, blocks shrunk, empty blocks dropped); nr / offe equal n_ref / off
+  // when every token is valid.
+  int nr = 0;                  // effective reference tokens
+  std::vector<int32_t> offe;   // effective block offsets
+  bool has_valid = false;
+  std::vector<int32_t> h_gidx; // compact index -> reference token
+  int32_t* d_gidx = nullptr;   // [nr]
+  int32_t* d_cidx = nullptr;   // [n_ref]: reference token -> compact index, -1 = invalid
+  void* cbuf[9] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // compact q,k,v,o,do,dq,dk,dv (bf16) + lse (fp32)
   float scale = 0.f;
   int device = -1;       // -1: host-only context (no usable CUDA device)
   bool sm100 = false;
@@ -72,4 +82,10 @@ template <int D>
 cudaError_t launch_fwd(const CUtensorMap* maps, const FwdParams& p, cudaStream_t stream);
 cudaError_t launch_fwd_merge(const FwdParams& p, int head_dim, int n_split, cudaStream_t stream);
 int run_backward(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t stream);
+// compaction helpers of the validity path (sra_api.cu)
+int compact_rows(sra_ctx* ctx, int slot, const void* src, const void** out, cudaStream_t stream);
+int compact_lse(sra_ctx* ctx, const float* src, const float** out, cudaStream_t stream);
+int compact_out(sra_ctx* ctx, int slot, void** out);
+int expand_rows(sra_ctx* ctx, int slot, void* dst, cudaStream_t stream);
+int expand_lse(sra_ctx* ctx, float* dst, cudaStream_t stream);
 }  // namespace sra

@@ -136,6 +136,38 @@ def test_split_schedule_partitions_the_keys(heads, n_gen, blocks):
         B.sra_destroy(ctx)
 
 
+@pytest.mark.parametrize("n_gen,blocks,seed", [(256, (128,) * 4, 0), (333, (1, 130, 257, 64, 200), 1), (50, (300, 5), 2)])
+def test_validity_schedule_covers_exactly_the_valid_mask(n_gen, blocks, seed):
+    """sra_set_reference_validity: the schedule is rebuilt on the compacted reference; mapped back
+    through the compaction it covers every unmasked (query, key) pair of the validity-aware mask exactly once and
+    nothing else, and the useful-FLOP count follows the valid tokens only.  NULL restores the plain schedule."""
+    off = [0]
+    for b in blocks:
+        off.append(off[-1] + b)
+    rng = np.random.default_rng(seed)
+    valid = rng.random(off[-1]) < 0.7
+    valid[off[1]:off[2]] = False  # one block entirely invalid
+    keep = np.flatnonzero(valid)
+    ctx = B.sra_create(1, 1, 64, n_gen, off)
+    try:
+        plain = B.sra_schedule_copy(ctx)
+        B.sra_set_reference_validity(ctx, valid)
+        items = B.sra_schedule_copy(ctx)
+        n_c = len(keep)
+        Cc = _covered_pairs(items, n_gen, n_c)  # in compact coordinates
+        M = sra_oracle.sra_mask(n_gen, off, valid).astype(np.int32)
+        idx = np.concatenate([np.arange(n_gen), n_gen + keep])
+        assert np.array_equal(Cc, M[np.ix_(idx, idx)])
+        assert M.sum() == Cc.sum(), "pairs outside the compacted rows/columns must all be masked"
+        assert B.sra_useful_flops(ctx, True) == 4.0 * 64 * float(M.sum())
+        B.sra_set_reference_validity(ctx, None)
+        assert B.sra_schedule_copy(ctx) == plain
+        B.sra_set_reference_validity(ctx, np.zeros(off[-1], dtype=bool))  # nothing valid: plain self-attention over G
+        assert all(not it["q_is_ref"] and it["seg1_len"] == 0 for it in B.sra_schedule_copy(ctx))
+    finally:
+        B.sra_destroy(ctx)
+
+
 @pytest.mark.parametrize("name", ["tiny", "480p", "720p", "sweep40s", "train"])
 def test_useful_flops_closed_form(name):
     """sra_useful_flops = 4 d pairs H B with pairs = N_g (N_g + N_r) + sum b_j^2 (tests/golden/pairs.txt)."""

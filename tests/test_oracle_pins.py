@@ -426,3 +426,63 @@ def test_backward_invariants():
         sl = slice(off[j], off[j + 1])
         assert np.array_equal(g3["dk_ref"][:, sl], g["dk_ref"][:, sl]) and np.array_equal(g3["dv_ref"][:, sl], g["dv_ref"][:, sl])
     assert not np.allclose(g3["dk_ref"][:, off[1]:off[2]], g["dk_ref"][:, off[1]:off[2]])
+
+
+# ------------------------------------------------------------------ sparse validity masking
+def _delete_invalid(t, off, valid):
+    """The same problem with the invalid reference tokens physically removed (blocks shrink, empty blocks vanish):
+    an independent formulation of validity masking - no predicate, just a smaller unmasked SRA problem."""
+    keep = np.flatnonzero(valid)
+    out = dict(t)
+    for k in ("q_ref", "k_ref", "v_ref", "do_ref"):
+        if k in out:
+            out[k] = np.ascontiguousarray(out[k][:, keep])
+    off2 = [0]
+    for j in range(len(off) - 1):
+        c = int(np.count_nonzero(valid[off[j]:off[j + 1]]))
+        if c:
+            off2.append(off2[-1] + c)
+    return out, off2, keep
+
+
+@pytest.mark.parametrize("seed,Ng,blocks", [(0, 7, (5, 9, 3)), (1, 1, (4,)), (2, 12, (2, 2, 6, 1))])
+def test_validity_mask_equals_deleting_invalid_tokens(seed, Ng, blocks):
+    """Validity pins: (1) forward and backward with valid[] equal the unmasked oracle on the problem with the invalid
+    tokens deleted (G rows, valid R rows, all gradients); (2) invalid R rows give O = 0, LSE = -inf and zero
+    gradients; (3) the pair count has the closed form N_g (N_g + sum_j v_j) + sum_j v_j^2; (4) a block that is
+    entirely invalid disappears; (5) valid = all ones changes nothing."""
+    rng = np.random.default_rng(seed)
+    off = [0]
+    for b in blocks:
+        off.append(off[-1] + b)
+    Nr, B, H, d = off[-1], 2, 2, 8
+    t = {k: rand_bits(rng, (B, Ng if k.endswith("gen") else Nr, H, d)) for k in
+         ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref", "do_gen", "do_ref")}
+    valid = rng.random(Nr) < 0.6
+    valid[off[1]:off[2] if len(off) > 2 else off[1]] = False  # (4): kill the whole second block when there is one
+    if not valid.any():
+        valid[0] = True
+    scale = 0.3
+    a6 = [t[k] for k in ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref")]
+    fm = sra_oracle.sra_forward(*a6, off, scale, valid=valid)
+    bm = sra_oracle.sra_backward(*a6, t["do_gen"], t["do_ref"], off, scale, valid=valid)
+    t2, off2, keep = _delete_invalid(t, off, valid)
+    b6 = [t2[k] for k in ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref")]
+    fd = sra_oracle.sra_forward(*b6, off2, scale)
+    bd = sra_oracle.sra_backward(*b6, t2["do_gen"], t2["do_ref"], off2, scale)
+    np.testing.assert_allclose(fm["o_gen"], fd["o_gen"], rtol=0, atol=1e-13)
+    np.testing.assert_allclose(fm["lse_gen"], fd["lse_gen"], rtol=0, atol=1e-13)
+    np.testing.assert_allclose(fm["o_ref"][:, keep], fd["o_ref"], rtol=0, atol=1e-13)
+    np.testing.assert_allclose(fm["lse_ref"][:, :, keep], fd["lse_ref"], rtol=0, atol=1e-13)
+    inv = np.flatnonzero(~valid)
+    assert np.all(fm["o_ref"][:, inv] == 0.0) and np.all(np.isneginf(fm["lse_ref"][:, :, inv]))
+    for g in ("dq", "dk", "dv"):
+        np.testing.assert_allclose(bm[g + "_gen"], bd[g + "_gen"], rtol=0, atol=1e-12)
+        np.testing.assert_allclose(bm[g + "_ref"][:, keep], bd[g + "_ref"], rtol=0, atol=1e-12)
+        assert np.all(bm[g + "_ref"][:, inv] == 0.0)
+    v = [int(np.count_nonzero(valid[off[j]:off[j + 1]])) for j in range(len(off) - 1)]
+    assert sra_oracle.count_pairs(Ng, off, valid) == Ng * (Ng + sum(v)) + sum(x * x for x in v)
+    ones = np.ones(Nr, dtype=bool)
+    f1 = sra_oracle.sra_forward(*a6, off, scale, valid=ones)
+    f0 = sra_oracle.sra_forward(*a6, off, scale)
+    assert all(np.array_equal(f1[k], f0[k]) for k in f0)
