@@ -17,7 +17,8 @@
 //       is what bounds this kernel: 32 KB of fp32 partial dQ per (key tile, query tile) pair of 10.5 MFLOP.
 //   a8  sra_bwd_dq_finalize_kernel  workspace * scale -> bf16 dQ [B, N, H, d]
 //
-// TMEM columns (D = 128): S0 @0 (64), S1 @64 (64), dP @128 (64), dQ^T @192 (64), dV @256 (128), dK @384 (128).
+// TMEM columns (D = 128): S0 @0 (64), S1 @64 (64), dP0 @128 (64), dP1 @192 (64), dV @256 (128), dK @384 (128);
+// dQ^T(it) overwrites dP^T(it) in dP[it & 1].
 #include "ptx.cuh"
 #include "sra_common.h"
 #include "sra_ctx.h"
@@ -36,11 +37,12 @@ struct BwdCfg {
   static constexpr int kStageBytes = 2 * kQBytes;       // Q_i + dO_i
   static constexpr int kDsBytes = kTile * kQT * 2;      // dS^T tile [128 keys][64 queries] bf16, x2 buffers
   static constexpr int kVecBytes = kStages * 2 * kQT * 4;  // lse2[64] + delta[64] per stage
-  static constexpr int kNumBars = 1 + 2 * kStages + 2 + 1 + 2 + 2 + 2 + 2 + 1;
+  static constexpr int kNumBars = 1 + 2 * kStages + 2 + 2 + 2 + 2 + 2 + 2 + 2 + 1;
   static constexpr int kSmemBytes = 2 * kKBytes + kStages * kStageBytes + 2 * kDsBytes + kVecBytes + kNumBars * 8 + 16;
   static constexpr int kThreads = 512;  // P, dS and dQ warpgroups, MMA + TMA warps (+2 idle)
-  // TMEM columns
-  static constexpr int kColS = 0, kColDP = 128, kColDQ = 192, kColDV = 256, kColDK = 256 + D;
+  // TMEM columns: S0 | S1 | dP0 | dP1 (64 each) | dV | dK.  dQ^T(it) is written over dP^T(it) in dP[it & 1] once the dS
+  // warpgroup has read it, so dP^T(it+1) has a buffer of its own and does not wait for tile it's dS / dQ chain.
+  static constexpr int kColS = 0, kColDP = 128, kColDV = 256, kColDK = 256 + D;
 };
 
 template <int D>
@@ -98,12 +100,12 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
   const uint32_t bar_q_full = sBar + 8;                         // [ST]
   const uint32_t bar_q_empty = bar_q_full + 8 * ST;             // [ST]
   const uint32_t bar_s_full = bar_q_empty + 8 * ST;             // [2]
-  const uint32_t bar_dp_full = bar_s_full + 16;                 // [1]
-  const uint32_t bar_p_full = bar_dp_full + 8;                  // [2]
+  const uint32_t bar_dp_full = bar_s_full + 16;                 // [2]
+  const uint32_t bar_p_full = bar_dp_full + 16;                 // [2]
   const uint32_t bar_ds_full = bar_p_full + 16;                 // [2]
   const uint32_t bar_ds_empty = bar_ds_full + 16;               // [2]
-  const uint32_t bar_dq_full = bar_ds_empty + 16;               // [1]
-  const uint32_t bar_dq_empty = bar_dq_full + 8;                // [1]
+  const uint32_t bar_dq_full = bar_ds_empty + 16;               // [2]
+  const uint32_t bar_dq_empty = bar_dq_full + 16;               // [1]
   const uint32_t bar_acc_full = bar_dq_empty + 8;               // [1]
   const uint32_t s_tmem_ptr = bar_acc_full + 8;
   uint32_t* tmem_ptr_generic = reinterpret_cast<uint32_t*>(smem_raw + (s_tmem_ptr - smem_u32(smem_raw)));
@@ -129,9 +131,9 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
       mbar_init(bar_p_full + 8 * i, 128);
       mbar_init(bar_ds_full + 8 * i, 128);
       mbar_init(bar_ds_empty + 8 * i, 1);
+      mbar_init(bar_dp_full + 8 * i, 1);
+      mbar_init(bar_dq_full + 8 * i, 1);
     }
-    mbar_init(bar_dp_full, 1);
-    mbar_init(bar_dq_full, 1);
     mbar_init(bar_dq_empty, 128);
     mbar_init(bar_acc_full, 1);
     fence_mbar_init();
@@ -225,11 +227,11 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
     for (int it = 0; it < n_it; ++it) {
       const int bf = it & 1, s = it % ST;
       const uint32_t tP = tmem + lane_off + C::kColS + bf * QT;
-      const uint32_t tDP = tmem + lane_off + C::kColDP;
+      const uint32_t tDP = tmem + lane_off + C::kColDP + bf * QT;
       const uint32_t vec = sVec + s * (2 * QT * 4) + QT * 4;  // delta[64]
       mbar_wait(bar_q_full + 8 * s, (it / ST) & 1);  // acquire the loader's delta writes
       mbar_wait(bar_p_full + 8 * bf, (it >> 1) & 1);
-      mbar_wait(bar_dp_full, it & 1);
+      mbar_wait(bar_dp_full + 8 * bf, (it >> 1) & 1);
       tc_fence_after();
       uint32_t pb[32], dp[2][32];
       tmem_ld32(tP, pb);
@@ -266,11 +268,11 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
     const uint32_t lane_off = uint32_t(wq * 32) << 16;
     for (int it = 0; it < n_it; ++it) {
       const QTile qt = q_tile_of(it, n0, item, p.n_gen);
-      mbar_wait(bar_dq_full, it & 1);
+      mbar_wait(bar_dq_full + 8 * (it & 1), (it >> 1) & 1);
       tc_fence_after();
       uint32_t r[2][32];
-      tmem_ld32(tmem + lane_off + C::kColDQ, r[0]);
-      tmem_ld32(tmem + lane_off + C::kColDQ + 32, r[1]);
+      tmem_ld32(tmem + lane_off + C::kColDP + (it & 1) * QT, r[0]);
+      tmem_ld32(tmem + lane_off + C::kColDP + (it & 1) * QT + 32, r[1]);
       tmem_wait_ld();
       tc_fence_before();
       mbar_arrive(bar_dq_empty);
@@ -350,7 +352,7 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
       constexpr uint32_t idesc_st = make_idesc_bf16(kTile, QT, 0, 0);   // S^T, dP^T : [128 x 64], K = d
       constexpr uint32_t idesc_acc = make_idesc_bf16(kTile, D, 0, 1);   // dV, dK    : [128 x D],  K = 64 queries
       constexpr uint32_t idesc_dq = make_idesc_bf16(D, QT, 1, 1);       // dQ^T      : [D x 64],    K = 128 keys
-      const uint32_t tS0 = tmem + C::kColS, tDP = tmem + C::kColDP, tDQ = tmem + C::kColDQ;
+      const uint32_t tS0 = tmem + C::kColS, tDP0 = tmem + C::kColDP;
       const uint32_t tDV = tmem + C::kColDV, tDK = tmem + C::kColDK;
       // Descriptor low words (start address, LBO); stepping along K or to another stage is one 32-bit add.
       constexpr uint32_t kHi = desc_hi_sw128(1024);
@@ -371,7 +373,7 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
       tc_fence_after();
       issue_kq(tS0, k_km, 0);
       umma_commit(bar_s_full);
-      issue_kq(tDP, v_km, C::kQBytes);
+      issue_kq(tDP0, v_km, C::kQBytes);
       umma_commit(bar_dp_full);
       for (int it = 0; it < n_it; ++it) {
         const int bf = it & 1, s = it % ST;
@@ -385,6 +387,11 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
           tc_fence_after();
           issue_kq(tS0 + (bf ^ 1) * QT, k_km, oQ1);  // S^T(it+1); its buffer held P^T(it-1), consumed by dV(it-1)
           umma_commit(bar_s_full + 8 * (bf ^ 1));
+          // dP^T(it+1) -> dP[bf ^ 1], which last held dQ^T(it-1): only the dQ warpgroup's drain of that tile gates it
+          mbar_wait(bar_dq_empty, (it & 1) ^ 1);
+          tc_fence_after();
+          issue_kq(tDP0 + (bf ^ 1) * QT, v_km, oQ1 + C::kQBytes);
+          umma_commit(bar_dp_full + 8 * (bf ^ 1));
         }
         // dV += P^T(it) dO_it : A = P^T from TMEM (16 queries = 8 columns per step), B = dO_it [queries][d] MN-major
         mbar_wait(bar_p_full + 8 * bf, (it >> 1) & 1);
@@ -395,22 +402,17 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
                   (it > 0 || kk > 0) ? 1u : 0u);
         mbar_wait(bar_ds_full + 8 * bf, (it >> 1) & 1);  // dS^T(it) in smem; dP^T(it) has been read out of TMEM
         tc_fence_after();
-        if (more) {
-          issue_kq(tDP, v_km, oQ1 + C::kQBytes);  // dP^T(it+1)
-          umma_commit(bar_dp_full);
-        }
         // dK += dS^T(it) Q_it : A = dS^T [keys][queries] K-major (one 128-byte box), B = Q_it [queries][d] MN-major
 #pragma unroll
         for (int kk = 0; kk < QT / 16; ++kk)
           umma_ss(tDK, desc64(ds_km + ((ods + kk * 32) >> 4), kHi), desc64(st_mn + ((oQ + kk * 2048) >> 4), kHi),
                   idesc_acc, (it > 0 || kk > 0) ? 1u : 0u);
-        // dQ_it^T = K^T dS^T(it) : A = K [keys][d] MN-major, B = dS^T [keys][queries] MN-major, K = 128 keys
-        mbar_wait(bar_dq_empty, (it & 1) ^ 1);
-        tc_fence_after();
+        // dQ_it^T = K^T dS^T(it) : A = K [keys][d] MN-major, B = dS^T [keys][queries] MN-major, K = 128 keys; written
+        // over dP^T(it), which the dS warpgroup has read (ds_full)
 #pragma unroll
         for (int kk = 0; kk < kTile / 16; ++kk)
-          umma_ss(tDQ, desc64(k_mn + ((kk * 2048) >> 4), kHi), desc64(ds_mn + ((ods + kk * 2048) >> 4), kHi), idesc_dq, kk > 0);
-        umma_commit(bar_dq_full);
+          umma_ss(tDP0 + bf * QT, desc64(k_mn + ((kk * 2048) >> 4), kHi), desc64(ds_mn + ((ods + kk * 2048) >> 4), kHi), idesc_dq, kk > 0);
+        umma_commit(bar_dq_full + 8 * bf);
         umma_commit(bar_q_empty + 8 * s);
         umma_commit(bar_ds_empty + 8 * bf);
       }
