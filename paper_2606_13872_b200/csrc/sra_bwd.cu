@@ -13,8 +13,8 @@
 //       second one (thread = key = TMEM lane; the two are pipeline stages of consecutive tiles).  dQ_i^T is
 //       drained by a third warpgroup (thread = d = TMEM lane) straight from registers into the fp32 workspace
 //       [B*H][n_pad][d] with coalesced red.global.add.f32 (many key tiles add into the same query rows; the
-//       summation order is not deterministic - SURVEY.md 8c A13).  The L2 reduction rate (~2.8 TB/s measured)
-//       is what bounds this kernel: 32 KB of fp32 partial dQ per (key tile, query tile) pair of 10.5 MFLOP.
+//       summation order is not deterministic - SURVEY.md 8c A13).  What bounds the kernel is the tensor pipe
+//       itself: the N = 64 SS MMAs (S^T, dP^T, dQ^T) run at 2/3 rate (operand reads), see DESIGN.md 6.2.
 //   a8  sra_bwd_dq_finalize_kernel  workspace * scale -> bf16 dQ [B, N, H, d]
 //
 // TMEM columns (D = 128): S0 @0 (64), S1 @64 (64), dP0 @128 (64), dP1 @192 (64), dV @256 (128), dK @384 (128);
