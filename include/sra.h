@@ -108,7 +108,12 @@ typedef struct {
  * `cuda_stream` the host->device copies of q/k/v into ctx-owned staging buffers (allocated on first
  * use, freed by sra_destroy), the same forward kernel as sra_forward, and the device->host copies of
  * the outputs.  The results are valid after the caller synchronises the stream.  Requires the
- * resident cache when n_ref > 0 (SRA_ERR_NO_REF_CACHE otherwise). */
+ * resident cache when n_ref > 0 (SRA_ERR_NO_REF_CACHE otherwise).
+ * With batch == 1 and at least 16 query slabs the step is pipelined: K/V first, then the generation rows in 8
+ * slabs whose host->device and device->host copies run on two ctx-owned copy streams underneath the forward
+ * launches of the neighbouring slabs (query slabs are independent work items), reference rows before the last two
+ * slabs.  The copy streams are ordered after prior work on `cuda_stream`, and `cuda_stream` waits for the last
+ * device->host copy, so the call is still asynchronous on - and ordered by - the caller's stream. */
 int sra_forward_host(sra_ctx* ctx, const sra_fwd_host_args* args, void* cuda_stream);
 
 typedef struct {

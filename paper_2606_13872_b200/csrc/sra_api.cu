@@ -396,6 +396,10 @@ void sra_destroy(sra_ctx* ctx) {
     cudaFree(ctx->ws_delta);
     cudaFree(ctx->ws_lse2);
     for (void* s : ctx->stage) cudaFree(s);
+    if (ctx->s_h2d) cudaStreamDestroy(ctx->s_h2d);
+    if (ctx->s_d2h) cudaStreamDestroy(ctx->s_d2h);
+    for (cudaEvent_t ev : ctx->pipe_ev)
+      if (ev) cudaEventDestroy(ev);
     for (auto& e : ctx->ev)
       for (cudaEvent_t x : e)
         if (x) cudaEventDestroy(x);
@@ -513,6 +517,11 @@ static int forward_core(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) 
   const bool split = ctx->n_split > 1;
   p.items = split ? ctx->d_split_items : ctx->d_fwd_items;
   p.n_items = ctx->n_gen_items * ctx->n_split + (with_ref_rows ? ctx->n_ref_items : 0);
+  if (ctx->sub_count >= 0) {  // sra_forward_host pipelines a step as several launches over item sub-ranges
+    p.items += ctx->sub_first;
+    p.n_items = ctx->sub_count;
+    if (p.n_items == 0) return SRA_OK;
+  }
   p.part_o = ctx->ws_part_o;
   p.part_lse = ctx->ws_part_lse;
   p.heads = H; p.batch = B; p.n_gen = c.n_gen; p.n_ref = nr;
@@ -540,6 +549,102 @@ static int forward_core(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) 
   return SRA_OK;
 }
 
+// Pipelined host path (batch 1): K/V first, then the generation rows in kChunks slabs - the H2D copy of slab c+1 and
+// the D2H copy of slab c-1 run on their own streams under the forward launch of slab c (query slabs are independent
+// work items, PCIe is full duplex); the reference rows go last.  Everything is ordered after prior work on `st`
+// and `st` is made to wait for the last D2H copy, so the call stays asynchronous on the caller's stream.
+static int forward_host_pipelined(sra_ctx* ctx, const sra_fwd_host_args* a, cudaStream_t st, bool with_ref_rows) {
+  constexpr int kChunks = 8;
+  const sra_config& c = ctx->cfg;
+  const size_t row = size_t(c.heads) * c.head_dim * 2;
+  const size_t gen_bytes = size_t(c.n_gen) * row, ref_bytes = size_t(c.n_ref) * row;
+  if (!ctx->s_h2d) {
+    cudaError_t e = cudaStreamCreateWithFlags(&ctx->s_h2d, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->s_d2h, cudaStreamNonBlocking);
+    ctx->pipe_ev.resize(2 * kChunks + 5);
+    for (cudaEvent_t& ev : ctx->pipe_ev)
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "pipeline stream / event creation");
+  }
+  cudaEvent_t* ev_q = ctx->pipe_ev.data();            // [kChunks] slab c of Q is on the device
+  cudaEvent_t* ev_c = ev_q + kChunks;                 // [kChunks] slab c of O is computed
+  cudaEvent_t ev_start = ev_c[kChunks], ev_kv = ev_c[kChunks + 1], ev_qr = ev_c[kChunks + 2], ev_cr = ev_c[kChunks + 3],
+              ev_done = ev_c[kChunks + 4];
+  char* dq = static_cast<char*>(ctx->stage[0]);
+  char* dout = static_cast<char*>(ctx->stage[3]);
+  const char* hq = static_cast<const char*>(a->q_gen);
+  char* hout = static_cast<char*>(a->o_gen);
+  sra_fwd_args d{};
+  d.q_gen = ctx->stage[0]; d.k_gen = ctx->stage[1]; d.v_gen = ctx->stage[2]; d.o_gen = ctx->stage[3];
+  d.lse_gen = a->lse_gen ? static_cast<float*>(ctx->stage[6]) : nullptr;
+  cudaError_t e = cudaEventRecord(ev_start, st);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->s_h2d, ev_start, 0);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->s_d2h, ev_start, 0);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->stage[1], a->k_gen, gen_bytes, cudaMemcpyHostToDevice, ctx->s_h2d);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->stage[2], a->v_gen, gen_bytes, cudaMemcpyHostToDevice, ctx->s_h2d);
+  if (e == cudaSuccess) e = cudaEventRecord(ev_kv, ctx->s_h2d);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev_kv, 0);
+  const int per = (ctx->n_gen_items + kChunks - 1) / kChunks;
+  auto rows_of = [&](int ch, int& i0, int& i1, size_t& r0, size_t& r1) {
+    i0 = std::min(ch * per, ctx->n_gen_items);
+    i1 = std::min(i0 + per, ctx->n_gen_items);
+    r0 = size_t(i0) * kQRowsPerCta;
+    r1 = std::min<size_t>(size_t(i1) * kQRowsPerCta, size_t(c.n_gen));
+  };
+  // every H2D copy is enqueued (and its event recorded) before the first launch waits on one
+  for (int ch = 0; ch < kChunks && e == cudaSuccess; ++ch) {
+    int i0, i1; size_t r0, r1;
+    rows_of(ch, i0, i1, r0, r1);
+    if (i1 > i0) e = cudaMemcpyAsync(dq + r0 * row, hq + r0 * row, (r1 - r0) * row, cudaMemcpyHostToDevice, ctx->s_h2d);
+    if (e == cudaSuccess) e = cudaEventRecord(ev_q[ch], ctx->s_h2d);
+  }
+  if (e == cudaSuccess && with_ref_rows) {
+    e = cudaMemcpyAsync(ctx->stage[4], a->q_ref, ref_bytes, cudaMemcpyHostToDevice, ctx->s_h2d);
+    if (e == cudaSuccess) e = cudaEventRecord(ev_qr, ctx->s_h2d);
+  }
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "host->device copy");
+  auto run_ref_rows = [&]() -> int {
+    // reference rows: their q_ref copy has had the first slabs' compute time to land; their output copy is
+    // hidden under the remaining slabs
+    cudaError_t er = cudaStreamWaitEvent(st, ev_qr, 0);
+    if (er != cudaSuccess) return fail_cuda(ctx, er, "pipelined host copy");
+    sra_fwd_args dr = d;
+    dr.q_ref = ctx->stage[4]; dr.o_ref = ctx->stage[5];
+    dr.lse_ref = a->lse_ref ? static_cast<float*>(ctx->stage[7]) : nullptr;
+    ctx->sub_first = ctx->n_gen_items; ctx->sub_count = ctx->n_ref_items;
+    const int rc = forward_core(ctx, &dr, st);
+    ctx->sub_count = -1;
+    if (rc) return rc;
+    er = cudaEventRecord(ev_cr, st);
+    if (er == cudaSuccess) er = cudaStreamWaitEvent(ctx->s_d2h, ev_cr, 0);
+    if (er == cudaSuccess) er = cudaMemcpyAsync(a->o_ref, ctx->stage[5], ref_bytes, cudaMemcpyDeviceToHost, ctx->s_d2h);
+    if (er == cudaSuccess && dr.lse_ref) er = cudaMemcpyAsync(a->lse_ref, dr.lse_ref, size_t(c.heads) * c.n_ref * 4, cudaMemcpyDeviceToHost, ctx->s_d2h);
+    return er == cudaSuccess ? SRA_OK : fail_cuda(ctx, er, "pipelined host copy");
+  };
+  for (int ch = 0; ch < kChunks; ++ch) {
+    int i0, i1; size_t r0, r1;
+    rows_of(ch, i0, i1, r0, r1);
+    if (with_ref_rows && ch == kChunks - 2)
+      if (int rc = run_ref_rows()) return rc;
+    e = cudaStreamWaitEvent(st, ev_q[ch], 0);
+    if (e != cudaSuccess) break;
+    ctx->sub_first = i0; ctx->sub_count = i1 - i0;
+    const int rc = forward_core(ctx, &d, st);
+    ctx->sub_count = -1;
+    if (rc) return rc;
+    e = cudaEventRecord(ev_c[ch], st);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->s_d2h, ev_c[ch], 0);
+    if (e == cudaSuccess && i1 > i0) e = cudaMemcpyAsync(hout + r0 * row, dout + r0 * row, (r1 - r0) * row, cudaMemcpyDeviceToHost, ctx->s_d2h);
+    if (e != cudaSuccess) break;
+  }
+  if (e == cudaSuccess && d.lse_gen)
+    e = cudaMemcpyAsync(a->lse_gen, d.lse_gen, size_t(c.heads) * c.n_gen * 4, cudaMemcpyDeviceToHost, ctx->s_d2h);
+  if (e == cudaSuccess) e = cudaEventRecord(ev_done, ctx->s_d2h);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev_done, 0);
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "pipelined host copy");
+  return SRA_OK;
+}
+
 int sra_forward_host(sra_ctx* ctx, const sra_fwd_host_args* a, void* cuda_stream) {
   if (!ctx) return SRA_ERR_INVALID_ARG;
   ctx->err.clear();
@@ -562,6 +667,8 @@ int sra_forward_host(sra_ctx* ctx, const sra_fwd_host_args* a, void* cuda_stream
       if (e != cudaSuccess) { (void)cudaGetLastError(); ctx->stage[i] = nullptr; return fail(ctx, SRA_ERR_OOM, "staging buffer allocation failed"); }
     }
   cudaStream_t st = cudaStream_t(cuda_stream);
+  if (c.batch == 1 && ctx->n_split == 1 && !ctx->has_valid && ctx->n_gen_items >= 16)
+    return forward_host_pipelined(ctx, a, st, with_ref_rows);
   cudaError_t e = cudaMemcpyAsync(ctx->stage[0], a->q_gen, gen_bytes, cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->stage[1], a->k_gen, gen_bytes, cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->stage[2], a->v_gen, gen_bytes, cudaMemcpyHostToDevice, st);

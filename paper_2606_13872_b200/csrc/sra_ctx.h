@@ -48,6 +48,10 @@ struct sra_ctx {
   size_t ws_dq_bytes = 0;
   // host-buffer staging of sra_forward_host (lazy): q,k,v,o gen; q,o ref; lse gen/ref
   void* stage[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  // sra_forward_host pipeline (lazy): copy streams and events; sub-range override of the forward launch
+  cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
+  std::vector<cudaEvent_t> pipe_ev;
+  int sub_first = 0, sub_count = -1;  // forward_core launches items [sub_first, sub_first + sub_count) when sub_count >= 0
   int64_t launches = 0;
   // optional per-kernel timing (sra_set_kernel_timing)
   bool timing = false;

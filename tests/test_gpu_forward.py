@@ -148,3 +148,38 @@ def test_480p_sampled_rows():
     assert np.abs(lse_gpu - lse_ref).max() <= LSE_TOL
     # property at any size: every output finite
     assert np.isfinite(out["o_gen"]).all() and np.isfinite(out["o_ref"]).all()
+
+
+@pytest.mark.parametrize("name", ["host_pipe", "ragged"])
+def test_forward_host_matches_device_path(name):
+    """sra_forward_host (HOST pointers; the e2e leg of bench.py): the pipelined path (batch 1, >= 16 query slabs: K/V
+    first, then query slabs with copies overlapped on their own streams) and the plain path (everything else) must
+    return exactly the bytes sra_forward returns for the same inputs."""
+    from paper_2606_13872_b200 import binding as B
+    w = (sra_inputs.SRAWorkload("host_pipe", 1, 2, 128, 4200, (700, 300), "B", 0) if name == "host_pipe"
+         else sra_inputs.WORKLOADS[name])
+    t = sra_inputs.make_inputs(w)
+    dev_out = run_gpu_forward(w, t, use_cache=True)
+    dev = torch.device("cuda:0")
+    ctx = B.sra_create(w.batch, w.heads, w.head_dim, w.n_gen, w.ref_block_offsets)
+    try:
+        B.sra_cache_reference_kv(ctx, t["k_ref"].to(dev), t["v_ref"].to(dev))
+        h = {k: t[k].pin_memory() for k in ("q_gen", "k_gen", "v_gen", "q_ref")}
+        o_gen = torch.full(t["q_gen"].shape, float("nan"), dtype=torch.bfloat16).pin_memory()
+        o_ref = torch.full(t["q_ref"].shape, float("nan"), dtype=torch.bfloat16).pin_memory()
+        lse_gen = torch.full((w.batch, w.heads, w.n_gen), float("nan")).pin_memory()
+        lse_ref = torch.full((w.batch, w.heads, w.n_ref), float("nan")).pin_memory()
+        for _ in range(2):  # twice: the second call reuses the staging buffers, streams and events
+            B.sra_forward_host(ctx, h["q_gen"], h["k_gen"], h["v_gen"], o_gen, q_ref=h["q_ref"], o_ref=o_ref,
+                               lse_gen=lse_gen, lse_ref=lse_ref)
+            torch.cuda.synchronize()
+            assert np.array_equal(o_gen.float().numpy(), dev_out["o_gen"])
+            assert np.array_equal(o_ref.float().numpy(), dev_out["o_ref"])
+            assert np.array_equal(lse_gen.numpy(), dev_out["lse_gen"]) and np.array_equal(lse_ref.numpy(), dev_out["lse_ref"])
+            o_gen.fill_(float("nan")); o_ref.fill_(float("nan"))
+        # cached denoising step through the host entry point (no reference rows)
+        B.sra_forward_host(ctx, h["q_gen"], h["k_gen"], h["v_gen"], o_gen, lse_gen=lse_gen)
+        torch.cuda.synchronize()
+        assert np.array_equal(o_gen.float().numpy(), dev_out["o_gen"])
+    finally:
+        B.sra_destroy(ctx)
