@@ -253,6 +253,13 @@ def bench_ours(args, w):
     ctx = B.sra_create(w.batch, w.heads, w.head_dim, w.n_gen, w.ref_block_offsets)
     fl = useful_flops(w)
     assert abs(B.sra_useful_flops(ctx, True) - fl) <= 1e-6 * fl
+    if args.window >= 0:
+        # refiner-style sparse temporal attention: 21 latent frames, generation keys of frames within
+        # the window only.  Parity for this path is in tests/test_gpu_temporal.py (numpy oracle).
+        n_frames = 21 if w.n_gen % 21 == 0 else 1
+        B.sra_set_temporal_window(ctx, [i * (w.n_gen // n_frames) for i in range(n_frames + 1)], args.window)
+        fl = B.sra_useful_flops(ctx, True)
+        args.no_oracle = True
     if args.invalid_frac > 0 and w.n_ref:
         # sparse validity masking: a seeded per-token mask; useful FLOPs follow the valid tokens only.
         # Parity for this path is in tests/test_gpu_validity.py (numpy oracle); the C-oracle legs are skipped here.
@@ -395,7 +402,8 @@ def bench_ours(args, w):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
-        "config": config_of(w, args, {"invalid_ref_frac": args.invalid_frac} if args.invalid_frac > 0 else None),
+        "config": config_of(w, args, {**({"invalid_ref_frac": args.invalid_frac} if args.invalid_frac > 0 else {}),
+                                      **({"temporal_window_frames": args.window} if args.window >= 0 else {})} or None),
         "pct_of_peak": {"measured_sustained": 100 * value / world / peaks["bf16_tflops_sustained"],
                         "measured_burst": 100 * value / world / peaks["bf16_tflops"],
                         "nominal_2250": 100 * value / world / NOMINAL_BF16_TFLOPS},
@@ -714,6 +722,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-oracle", action="store_true", help="skip the cpu_baseline / parity legs")
     ap.add_argument("--oracle-rows", type=int, default=192, help="generation rows in the oracle sample")
+    ap.add_argument("--window", type=int, default=-1,
+                    help="--mode fwd: sparse temporal attention window in latent frames (PAPER.md:143); -1 = off")
     ap.add_argument("--invalid-frac", type=float, default=0.0,
                     help="--mode fwd: fraction of reference tokens marked invalid (sparse validity masking, PAPER.md:225)")
     args = ap.parse_args()

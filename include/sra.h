@@ -155,6 +155,17 @@ int sra_schedule_info(const sra_ctx* ctx, int32_t* n_gen_items, int32_t* n_ref_i
  * count in *n_items.  Pure host logic - usable without a GPU. */
 int sra_schedule_copy(const sra_ctx* ctx, int32_t* items, int32_t capacity, int32_t* n_items);
 
+/* Sparse temporal attention of the super-resolution refiner ("sparse temporal attention that restricts
+ * each frame's receptive field to a local neighborhood").  The paper gives no window size and no
+ * mask; the reading taken (A17): generation tokens are grouped in frames by `gen_frame_offsets` (HOST,
+ * n_frames + 1 ints from 0 to n_gen, strictly increasing); a generation query of frame f sees the generation keys
+ * of frames [f - window, f + window] (clipped) and - the refiner keeps the video reference conditioning - every
+ * reference key; reference rows are unchanged.  window < 0 turns it off (gen_frame_offsets may then be NULL);
+ * window >= n_frames - 1 is plain SRA.  The schedule is rebuilt: forward slabs and backward key tiles never straddle
+ * a frame and masked tiles are never enumerated, so cost is linear in the window.  Forward and backward are
+ * supported; the key-split short-query schedule is not combined with a window.  Synchronises the device. */
+int sra_set_temporal_window(sra_ctx* ctx, int32_t n_frames, const int32_t* gen_frame_offsets, int32_t window);
+
 /* Sparse validity masking of reference tokens ("skip invalid reference tokens"; SURVEY.md 8f #1,
  * reading A8).  `valid`: HOST, n_ref bytes, non-zero = valid; NULL = every token valid again.  One mask per
  * context, shared by all batch items like the block pattern.  An invalid reference token is never a key (for

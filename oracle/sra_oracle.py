@@ -24,6 +24,11 @@ section 8f #1): with an optional per-reference-token flag valid[t],
     M[i][:] = 0 if i in R and not valid[i]     (an invalid token's own row is empty)
     a row with no visible key has O = 0, P = 0, LSE = -inf (the convention of reading A8).
 
+Sparse temporal attention of the SR refiner ("restricts each frame's receptive field to a local
+neighborhood"; no window size or mask is given - reading A17 of DESIGN.md): with generation frame offsets fr[] and a
+window w (frames on each side),
+    M[i][j] = 0 if i, j in G and |frame(i) - frame(j)| > w        (G -> R and the R rows are unchanged).
+
 SRA is exact attention under a fixed mask, so the oracle is that definition written
 out: the mask is materialised as an explicit n x n byte matrix, every quantity is
 fp64, nothing is tiled, fused or reordered.  Inputs are bf16 bit patterns (uint16),
@@ -51,9 +56,10 @@ def block_of(t: int, offsets) -> int:
     raise ValueError(f"token {t} outside reference blocks {offsets}")
 
 
-def sra_mask(n_gen: int, ref_block_offsets, valid=None) -> np.ndarray:
+def sra_mask(n_gen: int, ref_block_offsets, valid=None, gen_frame_offsets=None, window=-1) -> np.ndarray:
     """The explicit SRA mask M, uint8 [n, n] with n = n_gen + n_ref, rows/cols [G ; R].
-    `valid` (optional, n_ref flags): invalid reference tokens lose their column and their row."""
+    `valid` (optional, n_ref flags): invalid reference tokens lose their column and their row.
+    `gen_frame_offsets`, `window` >= 0 (optional): G -> G restricted to frames within the window."""
     off = [int(x) for x in ref_block_offsets] if len(ref_block_offsets) else [0]
     n_ref = off[-1]
     n = n_gen + n_ref
@@ -66,6 +72,13 @@ def sra_mask(n_gen: int, ref_block_offsets, valid=None) -> np.ndarray:
             for j in range(n_gen, n):
                 if block_of(j - n_gen, off) == bi:
                     M[i, j] = 1
+    if gen_frame_offsets is not None and window >= 0:
+        fr = [int(x) for x in gen_frame_offsets]
+        for i in range(n_gen):
+            fi = block_of(i, fr)
+            for j in range(n_gen):
+                if abs(block_of(j, fr) - fi) > window:
+                    M[i, j] = 0
     if valid is not None:
         for t in range(n_ref):
             if not valid[t]:
@@ -98,7 +111,8 @@ def _concat_head(x_gen, x_ref, b, h):
     return np.concatenate(parts, axis=0)
 
 
-def sra_forward(q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, ref_block_offsets, scale, valid=None):
+def sra_forward(q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, ref_block_offsets, scale, valid=None,
+                gen_frame_offsets=None, window=-1):
     """SRA forward on bf16-bit inputs [B, N, H, d].
 
     Returns dict(o_gen, o_ref, lse_gen, lse_ref): O fp64 [B,N,H,d], LSE fp64 [B,H,N].
@@ -111,7 +125,7 @@ def sra_forward(q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, ref_block_offsets, sca
     Nr = kr.shape[1]
     have_qr = q_ref is not None
     qr = f(q_ref) if have_qr else np.zeros((B, Nr, H, d))
-    M = sra_mask(Ng, ref_block_offsets, valid)
+    M = sra_mask(Ng, ref_block_offsets, valid, gen_frame_offsets, window)
     o = np.zeros((B, Ng + Nr, H, d))
     lse = np.zeros((B, H, Ng + Nr))
     for b in range(B):
@@ -129,14 +143,15 @@ def sra_forward(q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, ref_block_offsets, sca
     return out
 
 
-def sra_backward(q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, do_gen, do_ref, ref_block_offsets, scale, valid=None):
+def sra_backward(q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, do_gen, do_ref, ref_block_offsets, scale, valid=None,
+                 gen_frame_offsets=None, window=-1):
     """SRA backward on bf16-bit inputs.  Returns dq/dk/dv for G and R, fp64 [B,N,H,d]."""
     f = bf16_bits_to_f64
     qg, kg, vg, qr, kr, vr = f(q_gen), f(k_gen), f(v_gen), f(q_ref), f(k_ref), f(v_ref)
     dog, dor = f(do_gen), f(do_ref)
     B, Ng, H, d = qg.shape
     Nr = kr.shape[1]
-    M = sra_mask(Ng, ref_block_offsets, valid)
+    M = sra_mask(Ng, ref_block_offsets, valid, gen_frame_offsets, window)
     dq = np.zeros((B, Ng + Nr, H, d))
     dk = np.zeros_like(dq)
     dv = np.zeros_like(dq)

@@ -24,7 +24,7 @@ SRA_ERR_OOM = -5
 EXPORTS = (
     "sra_create", "sra_cache_reference_kv", "sra_forward", "sra_forward_host", "sra_backward", "sra_destroy", "sra_useful_flops",
     "sra_schedule_info", "sra_schedule_copy", "sra_cache_bytes", "sra_launch_count", "sra_status_string",
-    "sra_last_error", "sra_set_kernel_timing", "sra_kernel_time_ms", "sra_split_schedule_copy", "sra_set_reference_validity",
+    "sra_last_error", "sra_set_kernel_timing", "sra_kernel_time_ms", "sra_split_schedule_copy", "sra_set_reference_validity", "sra_set_temporal_window",
 )
 
 if not os.path.exists(LIB_PATH):
@@ -80,6 +80,8 @@ lib.sra_schedule_info.argtypes = [_ctx_p, ctypes.POINTER(ctypes.c_int32), ctypes
 lib.sra_schedule_info.restype = ctypes.c_int
 lib.sra_set_reference_validity.argtypes = [_ctx_p, ctypes.c_char_p]
 lib.sra_set_reference_validity.restype = ctypes.c_int
+lib.sra_set_temporal_window.argtypes = [_ctx_p, ctypes.c_int32, ctypes.POINTER(ctypes.c_int32), ctypes.c_int32]
+lib.sra_set_temporal_window.restype = ctypes.c_int
 lib.sra_split_schedule_copy.argtypes = [_ctx_p, ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32), ctypes.c_int32,
                                         ctypes.POINTER(ctypes.c_int32)]
 lib.sra_split_schedule_copy.restype = ctypes.c_int
@@ -221,6 +223,16 @@ def sra_split_schedule_copy(ctx: int):
         it["q_is_ref"] &= 1
         items.append(it)
     return ns.value, items
+
+
+def sra_set_temporal_window(ctx: int, gen_frame_offsets, window: int) -> None:
+    """sra_set_temporal_window (include/sra.h).  window < 0 (or gen_frame_offsets None) turns the window off."""
+    if gen_frame_offsets is None or window < 0:
+        _check(lib.sra_set_temporal_window(ctx, 0, None, -1), ctx)
+        return
+    off = [int(x) for x in gen_frame_offsets]
+    arr = (ctypes.c_int32 * len(off))(*off)
+    _check(lib.sra_set_temporal_window(ctx, len(off) - 1, arr, int(window)), ctx)
 
 
 def sra_set_reference_validity(ctx: int, valid) -> None:

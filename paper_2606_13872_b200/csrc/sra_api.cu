@@ -203,13 +203,23 @@ static void build_schedule(sra_ctx* ctx) {
   const int Ng = ctx->cfg.n_gen, Nr = ctx->nr;
   const std::vector<int32_t>& off = ctx->offe;
   ctx->fwd_items.clear();
-  // G slabs: every generation key tile, then every reference key tile.
-  for (int r0 = 0; r0 < Ng; r0 += kQRowsPerCta) {
-    FwdItem it{};
-    it.q_is_ref = 0; it.q_row0 = r0; it.q_rows = std::min(kQRowsPerCta, Ng - r0);
-    it.seg0_is_ref = 0; it.seg0_start = 0; it.seg0_len = Ng;
-    it.seg1_start = 0; it.seg1_len = Nr;
-    ctx->fwd_items.push_back(it);
+  // G slabs: every generation key tile, then every reference key tile.  With a temporal window
+  // ("restricts each frame's receptive field to a local neighborhood") a slab never straddles a frame
+  // and walks only the generation keys of frames [f - w, f + w]; the reference stays fully visible.
+  std::vector<int32_t> fr = {0, Ng};
+  const bool windowed = ctx->window >= 0 && ctx->gen_frames.size() >= 2;
+  if (windowed) fr = ctx->gen_frames;
+  const int F = int(fr.size()) - 1;
+  for (int f = 0; f < F; ++f) {
+    const int lo = windowed ? fr[std::max(0, f - ctx->window)] : 0;
+    const int hi = windowed ? fr[std::min(F, f + ctx->window + 1)] : Ng;
+    for (int r0 = fr[f]; r0 < fr[f + 1]; r0 += kQRowsPerCta) {
+      FwdItem it{};
+      it.q_is_ref = 0; it.q_row0 = r0; it.q_rows = std::min(kQRowsPerCta, fr[f + 1] - r0);
+      it.seg0_is_ref = 0; it.seg0_start = lo; it.seg0_len = hi - lo;
+      it.seg1_start = 0; it.seg1_len = Nr;
+      ctx->fwd_items.push_back(it);
+    }
   }
   ctx->n_gen_items = int(ctx->fwd_items.size());
   // R slabs: only the keys of the slab's own block ("reference tokens only self-attend").
@@ -237,7 +247,7 @@ static void build_schedule(sra_ctx* ctx) {
     const long waves0 = (base + kNumSms - 1) / kNumSms;
     const bool few = base < 2 * kNumSms;                                                    // cache-bound regime
     const bool ragged_waves = base < 8 * kNumSms && double(base) / double(waves0 * kNumSms) < 0.85;  // e.g. 2.16 waves
-    if ((few || ragged_waves) && tiles >= 16) {
+    if ((few || ragged_waves) && tiles >= 16 && !windowed) {
       // Candidates keep >= 8 key tiles per split.  Take the smallest split count that fills whole waves of
       // 148 CTAs to >= 92 % (fewer partials to write and merge); if even the largest cannot occupy every SM
       // once, take the largest.
@@ -274,16 +284,24 @@ static void build_schedule(sra_ctx* ctx) {
   // Backward: key tiles.  G key tiles are seen by all G queries; R key tiles of block j additionally by block j's
   // R queries.  Tiles never straddle a block boundary.
   ctx->bwd_items.clear();
-  for (int k0 = 0; k0 < Ng; k0 += kTile) {
-    BwdItem it{};
-    it.k_is_ref = 0; it.k_row0 = k0; it.k_rows = std::min(kTile, Ng - k0);
-    ctx->bwd_items.push_back(it);
+  // (With a temporal window, G key tiles do not straddle frames either and are seen by the queries of frames
+  // [f - w, f + w] only.)
+  for (int f = 0; f < F; ++f) {
+    const int lo = windowed ? fr[std::max(0, f - ctx->window)] : 0;
+    const int hi = windowed ? fr[std::min(F, f + ctx->window + 1)] : Ng;
+    for (int k0 = fr[f]; k0 < fr[f + 1]; k0 += kTile) {
+      BwdItem it{};
+      it.k_is_ref = 0; it.k_row0 = k0; it.k_rows = std::min(kTile, fr[f + 1] - k0);
+      it.g_start = lo; it.g_len = hi - lo;
+      ctx->bwd_items.push_back(it);
+    }
   }
   for (int j = 0; j + 1 < int(off.size()); ++j) {
     const int s = off[j], e = off[j + 1];
     for (int k0 = s; k0 < e; k0 += kTile) {
       BwdItem it{};
       it.k_is_ref = 1; it.k_row0 = k0; it.k_rows = std::min(kTile, e - k0);
+      it.g_start = 0; it.g_len = Ng;
       it.seg1_start = s; it.seg1_len = e - s;
       ctx->bwd_items.push_back(it);
     }
@@ -700,6 +718,14 @@ int sra_useful_flops(const sra_ctx* ctx, int include_ref_rows, int backward, dou
   if (!ctx || !out) return SRA_ERR_INVALID_ARG;
   const sra_config& c = ctx->cfg;
   double pairs = double(c.n_gen) * (double(c.n_gen) + double(ctx->nr));  // invalid reference tokens are not useful work
+  if (ctx->window >= 0 && ctx->gen_frames.size() >= 2) {  // temporal window: generation keys of frames [f - w, f + w] only
+    const std::vector<int32_t>& fr = ctx->gen_frames;
+    const int F = int(fr.size()) - 1;
+    pairs = 0.0;
+    for (int f = 0; f < F; ++f)
+      pairs += double(fr[f + 1] - fr[f]) *
+               (double(fr[std::min(F, f + ctx->window + 1)] - fr[std::max(0, f - ctx->window)]) + double(ctx->nr));
+  }
   if (include_ref_rows)
     for (size_t j = 0; j + 1 < ctx->offe.size(); ++j) {
       const double bsz = double(ctx->offe[j + 1] - ctx->offe[j]);
@@ -745,6 +771,29 @@ int sra_split_schedule_copy(const sra_ctx* ctx, int32_t* n_split, int32_t* items
   if (items) {
     const int n = std::min<int>(capacity, int(v.size()));
     std::memcpy(items, v.data(), size_t(n) * sizeof(FwdItem));
+  }
+  return SRA_OK;
+}
+
+int sra_set_temporal_window(sra_ctx* ctx, int32_t n_frames, const int32_t* gen_frame_offsets, int32_t window) {
+  if (!ctx) return SRA_ERR_INVALID_ARG;
+  ctx->err.clear();
+  if (window >= 0) {
+    if (n_frames < 1 || !gen_frame_offsets || gen_frame_offsets[0] != 0 || gen_frame_offsets[n_frames] != ctx->cfg.n_gen)
+      return fail(ctx, SRA_ERR_INVALID_ARG, "gen_frame_offsets must run from 0 to n_gen");
+    for (int f = 0; f < n_frames; ++f)
+      if (gen_frame_offsets[f + 1] <= gen_frame_offsets[f]) return fail(ctx, SRA_ERR_INVALID_ARG, "gen_frame_offsets must be strictly increasing");
+    ctx->gen_frames.assign(gen_frame_offsets, gen_frame_offsets + n_frames + 1);
+    ctx->window = window;
+  } else {
+    ctx->gen_frames.clear();
+    ctx->window = -1;
+  }
+  build_schedule(ctx);
+  if (ctx->device >= 0 && ctx->sm100) {
+    cudaSetDevice(ctx->device);
+    cudaDeviceSynchronize();
+    if (int rc = upload_schedule(ctx)) return fail(ctx, rc, "schedule upload failed");
   }
   return SRA_OK;
 }

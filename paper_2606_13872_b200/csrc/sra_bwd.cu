@@ -65,8 +65,8 @@ __device__ __forceinline__ QTile q_tile_of(int it, int n0, const BwdItem& item, 
   QTile t;
   if (it < n0) {
     t.is_ref = 0;
-    t.row0 = it * kBwdQTile;
-    t.valid = min(kBwdQTile, n_gen - t.row0);
+    t.row0 = item.g_start + it * kBwdQTile;
+    t.valid = min(kBwdQTile, item.g_start + item.g_len - t.row0);
     t.cat0 = t.row0;
   } else {
     t.is_ref = 1;
@@ -116,7 +116,7 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
   const int h = blockIdx.y;
   const int b = blockIdx.z;
   const int bh = b * p.heads + h;
-  const int n0 = (p.n_gen + QT - 1) / QT;
+  const int n0 = (item.g_len + QT - 1) / QT;  // generation query tiles that see this key tile
   const int n1 = (item.seg1_len + QT - 1) / QT;
   const int n_it = n0 + n1;
 

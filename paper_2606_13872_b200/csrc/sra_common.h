@@ -25,14 +25,16 @@ struct FwdItem {
 };
 
 // Backward work item: a 128-key tile and the (up to two) query segments that see it.
-// G key tile: seg0 = all generation queries.  R key tile of block j: seg0 = all generation
-// queries, seg1 = reference queries [off[j], off[j+1]).
+// G key tile: generation queries [g_start, g_start + g_len) (all of them, or - with a temporal window - the frames
+// whose window holds the tile's frame).  R key tile of block j: all generation queries, plus seg1 = reference
+// queries [off[j], off[j+1]).
 struct BwdItem {
   int32_t k_is_ref;
   int32_t k_row0;
   int32_t k_rows;  // valid keys 1..128
   int32_t seg1_start, seg1_len;  // reference-query segment (len 0 = absent)
-  int32_t pad[3];
+  int32_t g_start, g_len;        // generation-query segment that sees this tile (all of G unless a temporal window is set)
+  int32_t pad[1];
 };
 
 struct FwdParams {

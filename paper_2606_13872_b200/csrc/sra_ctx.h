@@ -16,6 +16,10 @@ struct sra_ctx {
   // Reference validity (sra_set_reference_validity): kernels, schedule, cache and workspaces see the
   // COMPACTED reference (valid tokens only, blocks shrunk, empty blocks dropped); nr / offe equal n_ref / off
   // when every token is valid.
+  // Sparse temporal attention (sra_set_temporal_window): generation frame offsets and window (frames on
+  // each side); window < 0 = off (every generation row sees every generation key)
+  std::vector<int32_t> gen_frames;
+  int window = -1;
   int nr = 0;                  // effective reference tokens
   std::vector<int32_t> offe;   // effective block offsets
   bool has_valid = false;

@@ -168,6 +168,36 @@ def test_validity_schedule_covers_exactly_the_valid_mask(n_gen, blocks, seed):
         B.sra_destroy(ctx)
 
 
+@pytest.mark.parametrize("frames,blocks,w", [((300, 300, 300, 300), (128, 257), 1), ((100, 513, 77, 260, 5), (), 0),
+                                             ((256,) * 6, (300,), 2), ((90, 90, 90), (64,), 5)])
+def test_temporal_window_schedule_covers_exactly_the_mask(frames, blocks, w):
+    """sra_set_temporal_window: forward slabs never straddle a frame, cover exactly the windowed mask,
+    and the useful-FLOP count follows it; window < 0 restores the plain schedule."""
+    fr = [0]
+    for n in frames:
+        fr.append(fr[-1] + n)
+    off = [0]
+    for b in blocks:
+        off.append(off[-1] + b)
+    ctx = B.sra_create(1, 1, 64, fr[-1], off)
+    try:
+        plain = B.sra_schedule_copy(ctx)
+        B.sra_set_temporal_window(ctx, fr, w)
+        items = B.sra_schedule_copy(ctx)
+        M = sra_oracle.sra_mask(fr[-1], off, None, fr, w).astype(np.int32)
+        assert np.array_equal(_covered_pairs(items, fr[-1], off[-1]), M)
+        assert B.sra_useful_flops(ctx, True) == 4.0 * 64 * float(M.sum())
+        for it in items:
+            if not it["q_is_ref"]:
+                f = max(i for i in range(len(frames)) if fr[i] <= it["q_row0"])
+                assert it["q_row0"] + it["q_rows"] <= fr[f + 1], "a generation slab straddles a frame"
+        assert B.sra_split_schedule_copy(ctx)[0] == 1
+        B.sra_set_temporal_window(ctx, None, -1)
+        assert B.sra_schedule_copy(ctx) == plain
+    finally:
+        B.sra_destroy(ctx)
+
+
 @pytest.mark.parametrize("name", ["tiny", "480p", "720p", "sweep40s", "train"])
 def test_useful_flops_closed_form(name):
     """sra_useful_flops = 4 d pairs H B with pairs = N_g (N_g + N_r) + sum b_j^2 (tests/golden/pairs.txt)."""

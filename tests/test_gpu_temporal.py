@@ -1,0 +1,92 @@
+"""-m gpu parity of the refiner's sparse temporal attention (reading A17): generation
+queries see the generation keys of frames within a window plus every reference key.  CUDA path through the C ABI
+(sra_set_temporal_window + forward / backward) vs the fp64 oracle that materialises the windowed mask, every row.
+
+Contract tolerance (BASELINE.json north_star): bf16 I/O, fp32 accumulation, max-abs <= 2e-2, mean-abs <= 2e-3, plus
+rel_l2 <= 1e-2.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import sra_oracle
+from paper_2606_13872_b200 import inputs as sra_inputs
+from tests.gpu_util import bits
+from tests.util import assert_parity
+
+pytestmark = pytest.mark.gpu
+GRADS = ("dq_gen", "dk_gen", "dv_gen", "dq_ref", "dk_ref", "dv_ref")
+
+
+def _run(w, t, fr, window, valid, backward):
+    from paper_2606_13872_b200 import binding as B
+    dev = torch.device("cuda:0")
+    g = {k: v.to(dev) for k, v in t.items()}
+    ctx = B.sra_create(w.batch, w.heads, w.head_dim, w.n_gen, w.ref_block_offsets)
+    try:
+        B.sra_set_temporal_window(ctx, fr, window)
+        if valid is not None:
+            B.sra_set_reference_validity(ctx, valid)
+        nan = float("nan")
+        o_gen, o_ref = torch.full_like(g["q_gen"], nan), torch.full_like(g["q_ref"], nan)
+        lse_gen = torch.full((w.batch, w.heads, w.n_gen), nan, device=dev)
+        lse_ref = torch.full((w.batch, w.heads, w.n_ref), nan, device=dev)
+        B.sra_cache_reference_kv(ctx, g["k_ref"], g["v_ref"])
+        B.sra_forward(ctx, g["q_gen"], g["k_gen"], g["v_gen"], o_gen, q_ref=g["q_ref"], o_ref=o_ref, lse_gen=lse_gen,
+                      lse_ref=lse_ref)
+        out = {"o_gen": o_gen, "o_ref": o_ref, "lse_gen": lse_gen, "lse_ref": lse_ref}
+        if backward:
+            grads = {n: torch.full_like(g["q_gen" if n.endswith("_gen") else "q_ref"], nan) for n in GRADS}
+            B.sra_backward(ctx, q_gen=g["q_gen"], k_gen=g["k_gen"], v_gen=g["v_gen"], q_ref=g["q_ref"], k_ref=None, v_ref=None,
+                           o_gen=o_gen, o_ref=o_ref, lse_gen=lse_gen, lse_ref=lse_ref, do_gen=g["do_gen"],
+                           do_ref=g["do_ref"], **grads)
+            out.update(grads)
+        torch.cuda.synchronize()
+        return {k: v.float().cpu().numpy() for k, v in out.items()}
+    finally:
+        B.sra_destroy(ctx)
+
+
+def _check(w, fr, window, valid=None, backward=True):
+    t = sra_inputs.make_inputs(w, with_grad=True)
+    got = _run(w, t, fr, window, valid, backward)
+    tb = bits(t)
+    scale = 1.0 / math.sqrt(w.head_dim)
+    a6 = [tb[k] for k in ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref")]
+    kw = dict(valid=valid, gen_frame_offsets=fr, window=window)
+    ref = sra_oracle.sra_forward(*a6, w.ref_block_offsets, scale, **kw)
+    keep = np.arange(w.n_ref) if valid is None else np.flatnonzero(valid)
+    assert_parity(got["o_gen"], ref["o_gen"], f"{w.name} O_g")
+    assert np.abs(got["lse_gen"] - ref["lse_gen"]).max() <= 2e-3
+    assert_parity(got["o_ref"][:, keep], ref["o_ref"][:, keep], f"{w.name} O_r")
+    if backward:
+        bref = sra_oracle.sra_backward(*a6, tb["do_gen"], tb["do_ref"], w.ref_block_offsets, scale, **kw)
+        for n in GRADS:
+            a, b = (got[n], bref[n]) if n.endswith("_gen") else (got[n][:, keep], bref[n][:, keep])
+            assert_parity(a, b, f"{w.name} {n}")
+
+
+@pytest.mark.parametrize("window", [0, 1, 3])
+def test_temporal_window_ragged_frames(window):
+    """Frames that do not divide 128 / 256, ragged reference blocks, B2 H3 d128; forward and backward."""
+    w = sra_inputs.SRAWorkload("temporal_ragged", 2, 3, 128, 1000, (130, 257, 64), "B", 0)
+    _check(w, [0, 100, 357, 400, 777, 1000], window)
+
+
+def test_temporal_window_real_frames_with_validity():
+    """Four real 1560-token latent frames, window 1, with a third of the reference marked invalid."""
+    w = sra_inputs.SRAWorkload("temporal_480", 1, 2, 128, 4 * 1560, (1560, 300), "B", 0)
+    valid = np.random.default_rng(3).random(w.n_ref) < 0.67
+    _check(w, [0, 1560, 3120, 4680, 6240], 1, valid=valid)
+
+
+def test_temporal_window_covering_everything_is_plain_sra():
+    from tests.gpu_util import run_gpu_forward
+    w = sra_inputs.WORKLOADS["ragged"]
+    t = sra_inputs.make_inputs(w, with_grad=True)
+    base = run_gpu_forward(w, t, use_cache=True)
+    got = _run(w, t, [0, 100, 200, 333], 2, None, backward=False)
+    assert_parity(got["o_gen"], base["o_gen"], "window >= n_frames - 1", rel_l2_tol=1e-3)
+    assert np.array_equal(got["o_ref"], base["o_ref"])

@@ -486,3 +486,49 @@ def test_validity_mask_equals_deleting_invalid_tokens(seed, Ng, blocks):
     f1 = sra_oracle.sra_forward(*a6, off, scale, valid=ones)
     f0 = sra_oracle.sra_forward(*a6, off, scale)
     assert all(np.array_equal(f1[k], f0[k]) for k in f0)
+
+
+# ------------------------------------------------------------------ sparse temporal attention
+@pytest.mark.parametrize("seed,frames,blocks,w", [(0, (3, 5, 2, 4), (3, 4), 1), (1, (4, 4, 4), (), 0), (2, (2, 3, 1, 5, 2), (6,), 2)])
+def test_temporal_window_mask_and_gradients(seed, frames, blocks, w):
+    """Temporal-window pins: (1) the mask equals an independently written |frame(i) - frame(j)| <= w rule
+    (searchsorted, not the oracle's block lookup) on G x G and is untouched elsewhere; (2) forward and backward equal
+    torch fp64 SDPA + autograd under that boolean mask (library routine); (3) w >= n_frames - 1 is plain SRA; (4) w = 0
+    without a reference is per-frame dense attention; (5) pair count = sum_f n_f (window keys_f + N_r) + sum_j b_j^2."""
+    rng = np.random.default_rng(seed)
+    fr = np.concatenate([[0], np.cumsum(frames)]).astype(np.int64)
+    off = [0]
+    for b in blocks:
+        off.append(off[-1] + b)
+    Ng, Nr, B, H, d = int(fr[-1]), off[-1], 1, 2, 8
+    fid = np.searchsorted(fr, np.arange(Ng), side="right") - 1
+    M = sra_oracle.sra_mask(Ng, off, None, fr, w).astype(bool)
+    M0 = sra_oracle.sra_mask(Ng, off).astype(bool)
+    want = M0.copy()
+    want[:Ng, :Ng] = np.abs(fid[:, None] - fid[None, :]) <= w
+    assert np.array_equal(M, want)
+    assert np.array_equal(sra_oracle.sra_mask(Ng, off, None, fr, len(frames) - 1), M0.astype(np.uint8))
+    keys = [int(fr[min(len(frames), f + w + 1)] - fr[max(0, f - w)]) for f in range(len(frames))]
+    assert int(M.sum()) == sum(n * (k + Nr) for n, k in zip(frames, keys)) + sum(b * b for b in blocks)
+    t = {k: rand_bits(rng, (B, Ng if k.endswith("gen") else Nr, H, d)) for k in
+         ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref", "do_gen", "do_ref")}
+    scale = 0.35
+    a6 = [t[k] for k in ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref")]
+    fwd = sra_oracle.sra_forward(*a6, off, scale, gen_frame_offsets=fr, window=w)
+    bwd = sra_oracle.sra_backward(*a6, t["do_gen"], t["do_ref"], off, scale, gen_frame_offsets=fr, window=w)
+    cat = lambda g, r: torch.tensor(np.concatenate([bits_to_f64(t[g]), bits_to_f64(t[r])], axis=1)[0].transpose(1, 0, 2))
+    q, k, v = (cat(a, b).requires_grad_(True) for a, b in (("q_gen", "q_ref"), ("k_gen", "k_ref"), ("v_gen", "v_ref")))
+    do = cat("do_gen", "do_ref")
+    o = torch.nn.functional.scaled_dot_product_attention(q, k, v, attn_mask=torch.tensor(want), scale=scale)
+    o.backward(do)
+    o_or = np.concatenate([fwd["o_gen"], fwd["o_ref"]], axis=1)[0].transpose(1, 0, 2) if Nr else fwd["o_gen"][0].transpose(1, 0, 2)
+    np.testing.assert_allclose(o_or, o.detach().numpy(), rtol=0, atol=1e-12)
+    for name, g in (("dq", q.grad), ("dk", k.grad), ("dv", v.grad)):
+        got = np.concatenate([bwd[name + "_gen"], bwd[name + "_ref"]], axis=1)[0].transpose(1, 0, 2)
+        np.testing.assert_allclose(got, g.numpy(), rtol=0, atol=1e-11)
+    if w == 0 and Nr == 0:
+        for f in range(len(frames)):
+            sl = slice(int(fr[f]), int(fr[f + 1]))
+            qf, kf, vf = (torch.tensor(bits_to_f64(t[n])[0, sl].transpose(1, 0, 2)) for n in ("q_gen", "k_gen", "v_gen"))
+            of = torch.nn.functional.scaled_dot_product_attention(qf, kf, vf, scale=scale)
+            np.testing.assert_allclose(fwd["o_gen"][0, sl].transpose(1, 0, 2), of.numpy(), rtol=0, atol=1e-12)
