@@ -82,6 +82,9 @@ WORKLOADS: Dict[str, SRAWorkload] = {
     "sweep10s": SRAWorkload("sweep10s", 1, 40, 128, 21 * 1560, _uniform(28, 1560), "A", 0),
     "sweep20s": SRAWorkload("sweep20s", 1, 40, 128, 21 * 1560, _uniform(56, 1560), "A", 0),
     "sweep40s": SRAWorkload("sweep40s", 1, 40, 128, 21 * 1560, _uniform(112, 1560), "A", 0),
+    # derived shape (SURVEY.md 8d "optional 1080p point": 68 x 120 = 8160 tokens per frame by the same 16x-per-side rule;
+    # no config pins it and the paper gives no token counts) - an extra scaling point only
+    "1080p": SRAWorkload("1080p", 1, 40, 128, 21 * 8160, _uniform(14, 8160), "A", 0),
     # [4] training fwd+bwd: B2, Q/K/V/dO ~ N(0,1)
     "train": SRAWorkload("train", 2, 40, 128, 21 * 1560, _uniform(14, 1560), "B", 0),
     # scaled-down, fully checkable shapes with the real boundary structure (SURVEY.md section 8d tier 3)
