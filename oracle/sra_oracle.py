@@ -29,6 +29,13 @@ neighborhood"; no window size or mask is given - reading A17 of DESIGN.md): with
 window w (frames on each side),
     M[i][j] = 0 if i, j in G and |frame(i) - frame(j)| > w        (G -> R and the R rows are unchanged).
 
+Producer side of the reference-KV cache ("eliminating redundant linear projections and RoPE
+computations across all steps").  The paper names RoPE and gives no formula, table or pairing;
+reading A18 of DESIGN.md: the RoFormer definition on interleaved pairs, angles supplied by the caller per token,
+    (y[2i] + j y[2i+1]) = (x[2i] + j x[2i+1]) * (cos[t, i] + j sin[t, i]),        t = token, i < d/2,
+shared by every head and batch entry; the rotated tensor is stored in bf16 (round to nearest even), the precision the
+attention consumes.  `rope` below is that definition as one complex multiplication.
+
 SRA is exact attention under a fixed mask, so the oracle is that definition written
 out: the mask is materialised as an explicit n x n byte matrix, every quantity is
 fp64, nothing is tiled, fused or reordered.  Inputs are bf16 bit patterns (uint16),
@@ -46,6 +53,33 @@ def bf16_bits_to_f64(bits: np.ndarray) -> np.ndarray:
     """Exact upcast of bf16 bit patterns (uint16) to float64."""
     bits = np.ascontiguousarray(bits, dtype=np.uint16)
     return (bits.astype(np.uint32) << np.uint32(16)).view(np.float32).astype(np.float64)
+
+
+def f64_to_bf16_bits(x: np.ndarray) -> np.ndarray:
+    """Round fp64 to bf16 (nearest, ties to even) and return the bit patterns (uint16).  Finite inputs whose magnitude
+    is inside the normal bf16 range; bf16 = the top 16 bits of the fp32 encoding, so the rounding is done on the value:
+    x = m * 2^e with 1 <= |m| < 2, keep 8 significant bits."""
+    x = np.asarray(x, dtype=np.float64)
+    m, e = np.frexp(x)                      # x = m * 2^e, 0.5 <= |m| < 1
+    q = np.rint(m * 256.0)                  # 8 significant bits; np.rint rounds ties to even
+    y = np.ldexp(q, e - 8)                  # exactly representable in bf16 (and so in fp32)
+    return (y.astype(np.float32).view(np.uint32) >> np.uint32(16)).astype(np.uint16)
+
+
+def rope(x_bits: np.ndarray, cos: np.ndarray, sin: np.ndarray) -> np.ndarray:
+    """Rotary position embedding of a bf16 tensor [B, N, H, d] by per-token angles, fp64 (reading A18).
+
+    cos, sin: [N, d/2] (the caller's table; any position scheme, e.g. the 3-D grid of a video DiT).  Element pair
+    (2i, 2i+1) of every head of token t is multiplied, as a complex number, by cos[t,i] + j sin[t,i].
+    Returns fp64 [B, N, H, d], unrounded; `f64_to_bf16_bits` gives what the cache stores."""
+    x = bf16_bits_to_f64(x_bits)
+    z = x[..., 0::2] + 1j * x[..., 1::2]
+    w = np.asarray(cos, dtype=np.float64) + 1j * np.asarray(sin, dtype=np.float64)
+    y = z * w[None, :, None, :]
+    out = np.empty_like(x)
+    out[..., 0::2] = y.real
+    out[..., 1::2] = y.imag
+    return out
 
 
 def block_of(t: int, offsets) -> int:

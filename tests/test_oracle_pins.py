@@ -532,3 +532,113 @@ def test_temporal_window_mask_and_gradients(seed, frames, blocks, w):
             qf, kf, vf = (torch.tensor(bits_to_f64(t[n])[0, sl].transpose(1, 0, 2)) for n in ("q_gen", "k_gen", "v_gen"))
             of = torch.nn.functional.scaled_dot_product_attention(qf, kf, vf, scale=scale)
             np.testing.assert_allclose(fwd["o_gen"][0, sl].transpose(1, 0, 2), of.numpy(), rtol=0, atol=1e-12)
+
+
+# ----------------------------------------------------------------------------- RoPE producer (reading A18)
+def _angles(N, half, rng=None, base=10000.0):
+    """theta[t, i] = t * base^(-i / half): the 1-D RoFormer table, the structure the relative-position pin needs."""
+    w = base ** (-np.arange(half) / half)
+    return np.arange(N)[:, None] * w[None, :]
+
+
+def test_rope_literal_cases():
+    """Values the definition fixes: angle 0 = identity; pi/2 maps the pair (a, b) -> (-b, a); pi negates; a unit vector
+    in element 0 becomes (cos, sin) in elements (0, 1) - this pins the interleaved pairing (not (0, d/2)) and the sign
+    of the sine term."""
+    x = np.zeros((1, 4, 1, 8))
+    x[0, :, 0, :] = [[1, 2, 3, 4, 5, 6, 7, 8]] * 4
+    bits = to_bf16_bits(x)
+    th = np.array([0.0, np.pi / 2, np.pi, 0.0])[:, None] * np.ones((1, 4))
+    y = sra_oracle.rope(bits, np.cos(th), np.sin(th))
+    np.testing.assert_allclose(y[0, 0, 0], [1, 2, 3, 4, 5, 6, 7, 8], atol=1e-14)
+    np.testing.assert_allclose(y[0, 1, 0], [-2, 1, -4, 3, -6, 5, -8, 7], atol=1e-14)
+    np.testing.assert_allclose(y[0, 2, 0], [-1, -2, -3, -4, -5, -6, -7, -8], atol=1e-14)
+    e0 = np.zeros((1, 1, 1, 8)); e0[..., 0] = 1.0
+    a = np.array([[0.3, 1.1, -0.7, 2.0]])
+    y = sra_oracle.rope(to_bf16_bits(e0), np.cos(a), np.sin(a))[0, 0, 0]
+    np.testing.assert_allclose(y, [math.cos(0.3), math.sin(0.3), 0, 0, 0, 0, 0, 0], atol=1e-15)
+    # per-pair angles are used pair by pair: unit vector in element 5 (pair 2, imaginary part)
+    e5 = np.zeros((1, 1, 1, 8)); e5[..., 5] = 1.0
+    y = sra_oracle.rope(to_bf16_bits(e5), np.cos(a), np.sin(a))[0, 0, 0]
+    np.testing.assert_allclose(y, [0, 0, 0, 0, -math.sin(-0.7), math.cos(-0.7), 0, 0], atol=1e-15)
+
+
+def test_rope_brute_force_rotation_matrices():
+    """Element by element with explicit 2x2 rotation matrices [[c, -s], [s, c]] in python loops."""
+    rng = np.random.default_rng(5)
+    B, N, H, d = 2, 5, 3, 6
+    bits = rand_bits(rng, (B, N, H, d))
+    th = rng.uniform(-4, 4, size=(N, d // 2))
+    y = sra_oracle.rope(bits, np.cos(th), np.sin(th))
+    x = bits_to_f64(bits)
+    for b in range(B):
+        for t in range(N):
+            for h in range(H):
+                for i in range(d // 2):
+                    c, s = math.cos(th[t, i]), math.sin(th[t, i])
+                    a, bb = x[b, t, h, 2 * i], x[b, t, h, 2 * i + 1]
+                    assert abs(y[b, t, h, 2 * i] - (c * a - s * bb)) < 1e-14
+                    assert abs(y[b, t, h, 2 * i + 1] - (s * a + c * bb)) < 1e-14
+
+
+def test_rope_invariants():
+    """(i) norms of every (token, head) vector are preserved; (ii) with theta = t * omega the score <rope(q)_m, rope(k)_n>
+    depends on m - n only (the property RoPE exists for): shifting every position by the same amount leaves Q K^T
+    unchanged, and the score equals Re sum_i q_i conj(k_i) e^{j (m - n) omega_i} computed directly; (iii) rotations
+    compose: angles a then b = angle a + b."""
+    rng = np.random.default_rng(6)
+    B, N, H, d = 1, 7, 2, 16
+    qb, kb = rand_bits(rng, (B, N, H, d)), rand_bits(rng, (B, N, H, d))
+    th = _angles(N + 11, d // 2)
+    q0, k0 = sra_oracle.rope(qb, np.cos(th[:N]), np.sin(th[:N])), sra_oracle.rope(kb, np.cos(th[:N]), np.sin(th[:N]))
+    q1, k1 = sra_oracle.rope(qb, np.cos(th[11:]), np.sin(th[11:])), sra_oracle.rope(kb, np.cos(th[11:]), np.sin(th[11:]))
+    x = bits_to_f64(qb)
+    np.testing.assert_allclose(np.linalg.norm(q0, axis=-1), np.linalg.norm(x, axis=-1), rtol=1e-13)
+    S0 = np.einsum("bmhd,bnhd->bhmn", q0, k0)
+    S1 = np.einsum("bmhd,bnhd->bhmn", q1, k1)
+    np.testing.assert_allclose(S0, S1, atol=1e-11)
+    q, k = bits_to_f64(qb), bits_to_f64(kb)
+    qc, kc = q[..., 0::2] + 1j * q[..., 1::2], k[..., 0::2] + 1j * k[..., 1::2]
+    omega = th[1]
+    for m in range(N):
+        for n in range(N):
+            want = (qc[0, m] * np.conj(kc[0, n]) * np.exp(1j * (m - n) * omega)[None, :]).sum(axis=-1).real
+            np.testing.assert_allclose(S0[0, :, m, n], want, atol=1e-11)
+    # composition (on values that survive the bf16 round trip exactly: small integers rotated by multiples of pi/2)
+    xi = to_bf16_bits(rng.integers(-8, 9, size=(1, 4, 1, 8)).astype(np.float64))
+    a = (np.pi / 2) * rng.integers(0, 4, size=(4, 4))
+    bnd = (np.pi / 2) * rng.integers(0, 4, size=(4, 4))
+    y1 = np.rint(sra_oracle.rope(xi, np.cos(a), np.sin(a)))
+    y2 = sra_oracle.rope(to_bf16_bits(y1), np.cos(bnd), np.sin(bnd))
+    np.testing.assert_allclose(y2, sra_oracle.rope(xi, np.cos(a + bnd), np.sin(a + bnd)), atol=1e-12)
+
+
+def test_bf16_rounding_matches_library_and_ties():
+    """f64_to_bf16_bits against torch's fp32 -> bf16 conversion (a different implementation) on values that are exact
+    in fp32, plus hand-made ties: 1 + 2^-8 is halfway between 1 and 1 + 2^-7 -> even (1.0); 1 + 3 * 2^-8 -> 1 + 2^-6."""
+    rng = np.random.default_rng(7)
+    x = (rng.standard_normal(20000) * np.exp(rng.uniform(-20, 20, 20000))).astype(np.float32).astype(np.float64)
+    np.testing.assert_array_equal(sra_oracle.f64_to_bf16_bits(x), to_bf16_bits(x))
+    ties = np.array([1.0 + 2.0 ** -8, 1.0 + 3 * 2.0 ** -8, -(1.0 + 2.0 ** -8), 2.0 - 2.0 ** -8, 0.0])
+    got = bits_to_f64(sra_oracle.f64_to_bf16_bits(ties))
+    np.testing.assert_array_equal(got, [1.0, 1.0 + 2.0 ** -6, -1.0, 2.0, 0.0])
+    # round trip: every bf16 value is a fixed point
+    allb = np.arange(0x0080, 0x7F80, 7, dtype=np.uint16)
+    np.testing.assert_array_equal(sra_oracle.f64_to_bf16_bits(sra_oracle.bf16_bits_to_f64(allb)), allb)
+
+
+def test_rope_then_attention_is_relative():
+    """End to end through the attention oracle: rotating Q and K by a table and by the same table shifted in position
+    gives the same O (G rows, no reference) - the composition the cached-producer path relies on."""
+    rng = np.random.default_rng(8)
+    B, N, H, d = 1, 6, 1, 8
+    qb, kb, vb = (rand_bits(rng, (B, N, H, d)) for _ in range(3))
+    th = _angles(N + 5, d // 2)
+    outs = []
+    for sh in (0, 5):
+        c, s = np.cos(th[sh:sh + N]), np.sin(th[sh:sh + N])
+        # fp64 rotated values are not bf16: run the attention definition on them directly
+        Q, K = sra_oracle.rope(qb, c, s)[0, :, 0], sra_oracle.rope(kb, c, s)[0, :, 0]
+        O, _, _ = sra_oracle.masked_attention(Q, K, bits_to_f64(vb)[0, :, 0], np.ones((N, N), np.uint8), 1 / math.sqrt(d))
+        outs.append(O)
+    np.testing.assert_allclose(outs[0], outs[1], atol=1e-12)
