@@ -72,6 +72,24 @@ int sra_create(const sra_config* cfg, sra_ctx** out);
  * is read by every later sra_forward whose k_ref/v_ref are NULL.  n_ref == 0 => no-op. */
 int sra_cache_reference_kv(sra_ctx* ctx, const void* k_ref, const void* v_ref, void* cuda_stream);
 
+/* Fused producer of the cache (PAPER.md:223 - caching "eliminat[es] redundant linear projections and RoPE computations
+ * across all steps").  Same as sra_cache_reference_kv, but k_ref is the PRE-RoPE key projection and
+ * the rotation is applied inside the kernel that writes the resident head-major layout, so the rotated keys never
+ * make a round trip through HBM.  Reading A18 (the paper gives no formula): RoFormer rotation on
+ * interleaved pairs, (y[2i] + j y[2i+1]) = (x[2i] + j x[2i+1]) (cos[t,i] + j sin[t,i]), fp32 arithmetic, result
+ * rounded to bf16 (nearest even); the same table for every head and batch entry.
+ * cos_ref / sin_ref: DEVICE fp32 [n_ref, d/2], row t = ORIGINAL reference token t (also when a validity mask compacts
+ * the cache).  v_ref is copied unrotated.  Both tables must be non-NULL (SRA_ERR_INVALID_ARG). */
+int sra_cache_reference_kv_rope(sra_ctx* ctx, const void* k_ref, const void* v_ref, const float* cos_ref,
+                                const float* sin_ref, void* cuda_stream);
+
+/* The per-step side of the same operation: rotates, IN PLACE, one or two DEVICE bf16 tensors [B, n_tokens, H, d]
+ * (typically the fresh Q_g and K_g of a denoising step, or Q_r / K_r in training) by the table cos / sin
+ * (DEVICE fp32 [n_tokens, d/2]) with the arithmetic stated above.  x1 may be NULL.  One launch, 16 bytes per thread,
+ * HBM-bound: 2 * bytes(x0, x1) + the table.  n_tokens <= 0 => no-op. */
+int sra_apply_rope(sra_ctx* ctx, void* x0, void* x1, const float* cos, const float* sin, int32_t n_tokens,
+                   void* cuda_stream);
+
 typedef struct {
   const void* q_gen; /* DEVICE bf16 [B, n_gen, H, d]                                              */
   const void* k_gen; /* DEVICE bf16 [B, n_gen, H, d]                                              */
@@ -199,7 +217,8 @@ int64_t sra_cache_bytes(const sra_ctx* ctx);
 #define SRA_KERNEL_BWD_MAIN 3       /* a7 */
 #define SRA_KERNEL_BWD_DQ_FINALIZE 4 /* a8 */
 #define SRA_KERNEL_FWD_MERGE 5       /* a5': merge of key-split partials (short-query schedules only) */
-#define SRA_NUM_KERNELS 6
+#define SRA_KERNEL_ROPE 6            /* sra_apply_rope (8f #3); the fused cache producer reports as CACHE_RELAYOUT */
+#define SRA_NUM_KERNELS 7
 int sra_set_kernel_timing(sra_ctx* ctx, int enable);
 int sra_kernel_time_ms(sra_ctx* ctx, int which, float* ms);
 

@@ -22,7 +22,7 @@ SRA_ERR_NO_REF_CACHE = -4
 SRA_ERR_OOM = -5
 
 EXPORTS = (
-    "sra_create", "sra_cache_reference_kv", "sra_forward", "sra_forward_host", "sra_backward", "sra_destroy", "sra_useful_flops",
+    "sra_create", "sra_cache_reference_kv", "sra_cache_reference_kv_rope", "sra_apply_rope", "sra_forward", "sra_forward_host", "sra_backward", "sra_destroy", "sra_useful_flops",
     "sra_schedule_info", "sra_schedule_copy", "sra_cache_bytes", "sra_launch_count", "sra_status_string",
     "sra_last_error", "sra_set_kernel_timing", "sra_kernel_time_ms", "sra_split_schedule_copy", "sra_set_reference_validity", "sra_set_temporal_window",
 )
@@ -65,6 +65,12 @@ lib.sra_create.argtypes = [ctypes.POINTER(sra_config), ctypes.POINTER(_ctx_p)]
 lib.sra_create.restype = ctypes.c_int
 lib.sra_cache_reference_kv.argtypes = [_ctx_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
 lib.sra_cache_reference_kv.restype = ctypes.c_int
+lib.sra_cache_reference_kv_rope.argtypes = [_ctx_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
+                                            ctypes.c_void_p]
+lib.sra_cache_reference_kv_rope.restype = ctypes.c_int
+lib.sra_apply_rope.argtypes = [_ctx_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32,
+                               ctypes.c_void_p]
+lib.sra_apply_rope.restype = ctypes.c_int
 lib.sra_forward.argtypes = [_ctx_p, ctypes.POINTER(sra_fwd_args), ctypes.c_void_p]
 lib.sra_forward.restype = ctypes.c_int
 lib.sra_forward_host.argtypes = [_ctx_p, ctypes.POINTER(sra_fwd_host_args), ctypes.c_void_p]
@@ -153,6 +159,16 @@ def sra_destroy(ctx: Optional[int]) -> None:
 
 def sra_cache_reference_kv(ctx: int, k_ref, v_ref, stream=None) -> None:
     _check(lib.sra_cache_reference_kv(ctx, _ptr(k_ref), _ptr(v_ref), _stream(stream)), ctx)
+
+
+def sra_cache_reference_kv_rope(ctx: int, k_ref, v_ref, cos_ref, sin_ref, stream=None) -> None:
+    """k_ref pre-RoPE; cos_ref / sin_ref fp32 device tensors [n_ref, d/2] (include/sra.h)."""
+    _check(lib.sra_cache_reference_kv_rope(ctx, _ptr(k_ref), _ptr(v_ref), _ptr(cos_ref), _ptr(sin_ref), _stream(stream)), ctx)
+
+
+def sra_apply_rope(ctx: int, x0, x1, cos, sin, n_tokens: int, stream=None) -> None:
+    """In-place rotation of x0 (and x1 unless None), bf16 device tensors [B, n_tokens, H, d]."""
+    _check(lib.sra_apply_rope(ctx, _ptr(x0), _ptr(x1), _ptr(cos), _ptr(sin), int(n_tokens), _stream(stream)), ctx)
 
 
 def sra_forward(ctx: int, q_gen, k_gen, v_gen, o_gen, q_ref=None, k_ref=None, v_ref=None, o_ref=None,
@@ -248,7 +264,7 @@ def sra_cache_bytes(ctx: int) -> int:
     return int(lib.sra_cache_bytes(ctx))
 
 
-KERNEL_CACHE_RELAYOUT, KERNEL_FWD, KERNEL_BWD_PREPROCESS, KERNEL_BWD_MAIN, KERNEL_BWD_DQ_FINALIZE, KERNEL_FWD_MERGE = range(6)
+KERNEL_CACHE_RELAYOUT, KERNEL_FWD, KERNEL_BWD_PREPROCESS, KERNEL_BWD_MAIN, KERNEL_BWD_DQ_FINALIZE, KERNEL_FWD_MERGE, KERNEL_ROPE = range(7)
 
 
 def sra_set_kernel_timing(ctx: int, enable: bool) -> None:

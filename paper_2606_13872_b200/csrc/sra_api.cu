@@ -98,6 +98,53 @@ __global__ void relayout_head_major_kernel(const uint4* __restrict__ src0, const
   }
 }
 
+// RoPE (reading A18): 8 bf16 = 4 interleaved pairs, each multiplied as a complex number by
+// (cos, sin)[4 pairs] in fp32 and rounded back to bf16.
+__device__ __forceinline__ uint32_t rope_pair(uint32_t w, float c, float s) {
+  const float a = __uint_as_float(w << 16), b = __uint_as_float(w & 0xffff0000u);
+  const __nv_bfloat162 r = __floats2bfloat162_rn(fmaf(a, c, -b * s), fmaf(a, s, b * c));
+  return *reinterpret_cast<const uint32_t*>(&r);
+}
+__device__ __forceinline__ uint4 rope_vec(uint4 x, float4 c, float4 s) {
+  return make_uint4(rope_pair(x.x, c.x, s.x), rope_pair(x.y, c.y, s.y), rope_pair(x.z, c.z, s.z), rope_pair(x.w, c.w, s.w));
+}
+
+// The fused cache producer: relayout_head_major_kernel with the rotation of K folded into the copy
+// (K: read pre-RoPE [B, N, H, d], write rotated [B, H, N, d]; V: plain relayout).  cos/sin rows are indexed by the
+// ORIGINAL token (gidx[n] under a validity mask).  Traffic = 2 * bytes(K, V) + the table once per head from L2.
+__global__ void relayout_rope_head_major_kernel(const uint4* __restrict__ src0, const uint4* __restrict__ src1,
+                                                uint4* __restrict__ dst0, uint4* __restrict__ dst1, int N, int H, int vec,
+                                                size_t total, const int32_t* __restrict__ gidx, int n_src,
+                                                const float4* __restrict__ cs, const float4* __restrict__ sn) {
+  for (size_t i = blockIdx.x * size_t(blockDim.x) + threadIdx.x; i < total; i += size_t(gridDim.x) * blockDim.x) {
+    const int c = int(i % vec);
+    size_t t = i / vec;
+    const int hh = int(t % H);
+    t /= H;
+    const int n = int(t % N);
+    const size_t bb = t / N;
+    const int tok = gidx ? gidx[n] : n;
+    const size_t o = ((bb * H + hh) * size_t(N) + n) * vec + c;
+    const size_t in = gidx ? ((bb * n_src + tok) * H + hh) * size_t(vec) + c : i;
+    const size_t tb = size_t(tok) * vec + c;  // float4 index: row tok of [n_src, d/2], pairs [4c, 4c + 4)
+    dst0[o] = rope_vec(src0[in], __ldg(cs + tb), __ldg(sn + tb));
+    dst1[o] = src1[in];
+  }
+}
+
+// In-place rotation of one or two [B, N, H, d] tensors (the per-step Q_g / K_g side).
+__global__ void rope_inplace_kernel(uint4* __restrict__ x0, uint4* __restrict__ x1, int N, int H, int vec, size_t total,
+                                    const float4* __restrict__ cs, const float4* __restrict__ sn) {
+  for (size_t i = blockIdx.x * size_t(blockDim.x) + threadIdx.x; i < total; i += size_t(gridDim.x) * blockDim.x) {
+    const int c = int(i % vec);
+    const int tok = int((i / (size_t(vec) * H)) % N);
+    const size_t tb = size_t(tok) * vec + c;
+    const float4 cc = __ldg(cs + tb), ss = __ldg(sn + tb);
+    x0[i] = rope_vec(x0[i], cc, ss);
+    if (x1) x1[i] = rope_vec(x1[i], cc, ss);
+  }
+}
+
 // Validity path.  dst[b, i, :, :] = src[b, gidx[i], :, :]  (rows of H*d bf16, 16 B per thread)
 __global__ void gather_rows_kernel(const uint4* __restrict__ src, uint4* __restrict__ dst, const int32_t* __restrict__ gidx,
                                    int n_src, int n_dst, int row_vec, size_t total) {
@@ -432,12 +479,14 @@ static int check_device(sra_ctx* ctx) {
   return SRA_OK;
 }
 
-int sra_cache_reference_kv(sra_ctx* ctx, const void* k_ref, const void* v_ref, void* cuda_stream) {
+static int cache_reference_kv(sra_ctx* ctx, const void* k_ref, const void* v_ref, const float* cos_ref, const float* sin_ref,
+                              bool rope, void* cuda_stream) {
   if (!ctx) return SRA_ERR_INVALID_ARG;
   ctx->err.clear();
   if (int rc = check_device(ctx)) return rc;
   if (ctx->cfg.n_ref == 0) return SRA_OK;
   if (!k_ref || !v_ref) return fail(ctx, SRA_ERR_INVALID_ARG, "k_ref / v_ref must be non-NULL");
+  if (rope && (!cos_ref || !sin_ref)) return fail(ctx, SRA_ERR_INVALID_ARG, "cos_ref / sin_ref must be non-NULL");
   const sra_config& c = ctx->cfg;
   if (ctx->nr == 0) { ctx->cache_valid = true; return SRA_OK; }  // every reference token is invalid: nothing to cache
   const size_t elems = size_t(c.batch) * ctx->nr * c.heads * c.head_dim;
@@ -457,14 +506,53 @@ int sra_cache_reference_kv(sra_ctx* ctx, const void* k_ref, const void* v_ref, v
   cudaError_t e;
   {
     sra::KernelTimer kt(ctx, SRA_KERNEL_CACHE_RELAYOUT, cudaStream_t(cuda_stream));
-    sra::relayout_head_major_kernel<<<blocks, threads, 0, cudaStream_t(cuda_stream)>>>(
-        static_cast<const uint4*>(k_ref), static_cast<const uint4*>(v_ref), reinterpret_cast<uint4*>(ctx->cache_k),
-        reinterpret_cast<uint4*>(ctx->cache_v), ctx->nr, c.heads, vec, total, ctx->has_valid ? ctx->d_gidx : nullptr, c.n_ref);
+    const int32_t* gidx = ctx->has_valid ? ctx->d_gidx : nullptr;
+    if (rope)
+      sra::relayout_rope_head_major_kernel<<<blocks, threads, 0, cudaStream_t(cuda_stream)>>>(
+          static_cast<const uint4*>(k_ref), static_cast<const uint4*>(v_ref), reinterpret_cast<uint4*>(ctx->cache_k),
+          reinterpret_cast<uint4*>(ctx->cache_v), ctx->nr, c.heads, vec, total, gidx, c.n_ref,
+          reinterpret_cast<const float4*>(cos_ref), reinterpret_cast<const float4*>(sin_ref));
+    else
+      sra::relayout_head_major_kernel<<<blocks, threads, 0, cudaStream_t(cuda_stream)>>>(
+          static_cast<const uint4*>(k_ref), static_cast<const uint4*>(v_ref), reinterpret_cast<uint4*>(ctx->cache_k),
+          reinterpret_cast<uint4*>(ctx->cache_v), ctx->nr, c.heads, vec, total, gidx, c.n_ref);
     e = cudaGetLastError();
   }
   if (e != cudaSuccess) return fail_cuda(ctx, e, "cache relayout launch");
   ctx->launches += 1;
   ctx->cache_valid = true;
+  return SRA_OK;
+}
+
+int sra_cache_reference_kv(sra_ctx* ctx, const void* k_ref, const void* v_ref, void* cuda_stream) {
+  return cache_reference_kv(ctx, k_ref, v_ref, nullptr, nullptr, false, cuda_stream);
+}
+
+int sra_cache_reference_kv_rope(sra_ctx* ctx, const void* k_ref, const void* v_ref, const float* cos_ref,
+                                const float* sin_ref, void* cuda_stream) {
+  return cache_reference_kv(ctx, k_ref, v_ref, cos_ref, sin_ref, true, cuda_stream);
+}
+
+int sra_apply_rope(sra_ctx* ctx, void* x0, void* x1, const float* cos, const float* sin, int32_t n_tokens,
+                   void* cuda_stream) {
+  if (!ctx) return SRA_ERR_INVALID_ARG;
+  ctx->err.clear();
+  if (int rc = check_device(ctx)) return rc;
+  if (n_tokens <= 0) return SRA_OK;
+  if (!x0 || !cos || !sin) return fail(ctx, SRA_ERR_INVALID_ARG, "x0 / cos / sin must be non-NULL");
+  const sra_config& c = ctx->cfg;
+  const int vec = c.head_dim / 8;
+  const size_t total = size_t(c.batch) * n_tokens * c.heads * vec;
+  cudaError_t e;
+  {
+    sra::KernelTimer kt(ctx, SRA_KERNEL_ROPE, cudaStream_t(cuda_stream));
+    sra::rope_inplace_kernel<<<sra::grid_for(total), 256, 0, cudaStream_t(cuda_stream)>>>(
+        static_cast<uint4*>(x0), static_cast<uint4*>(x1), n_tokens, c.heads, vec, total,
+        reinterpret_cast<const float4*>(cos), reinterpret_cast<const float4*>(sin));
+    e = cudaGetLastError();
+  }
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "rope launch");
+  ctx->launches += 1;
   return SRA_OK;
 }
 

@@ -148,3 +148,48 @@ def make_tensor_device(w: SRAWorkload, tensor: str, device, step: int = 0, seed_
     if scale != 1.0:
         x.mul_(scale)
     return x.to(torch.bfloat16)
+
+
+# ----------------------------------------------------------------------------- RoPE angle tables (inputs of 8f #3)
+_GRID_WIDTH = {1560: 52, 3600: 80, 8160: 120}  # tokens per latent frame -> tokens per row (30x52, 45x80, 68x120)
+
+
+def rope_tables(w: SRAWorkload, which: str, base: float = 10000.0):
+    """(cos, sin) fp32 CPU tensors [n, d/2] for the `which` in {"gen", "ref"} tokens of workload `w`.
+
+    An INPUT of the path (include/sra.h takes the table from the caller), drawn up here so that both sides rotate by
+    the same numbers.  Recipe (synthetic; the paper names RoPE and gives no scheme - stands in for the 3-D table of a
+    video DiT): token t sits at (frame, row, column) of a latent grid; the d/2 pairs are split into three groups
+    (d/2 - 2*(d/2 // 3) temporal, d/2 // 3 rows, d/2 // 3 columns); pair j of a group of size m turns by
+    position * base^(-j/m).  Generation tokens: frame = t // P, P = n_gen / 21 when that is one of the paper's grids
+    (width from _GRID_WIDTH), else P = 64 with width 8.  Reference tokens: frame = -(block index + 1) (reference frames
+    sit before the clip), row / column from the index inside the block with the same width rule.
+    Angles are formed in fp64 and the cosines / sines rounded once to fp32."""
+    half = w.head_dim // 2
+    m_hw = half // 3
+    m_t = half - 2 * m_hw
+    if which == "gen":
+        n = w.n_gen
+        per = n // 21 if n % 21 == 0 and (n // 21) in _GRID_WIDTH else 64
+        width = _GRID_WIDTH.get(per, 8)
+        t = torch.arange(n, dtype=torch.int64)
+        frame, inner = t // per, t % per
+    elif which == "ref":
+        n = w.n_ref
+        frame = torch.empty(n, dtype=torch.int64)
+        inner = torch.empty(n, dtype=torch.int64)
+        off = w.ref_block_offsets
+        width = 8
+        for k, size in enumerate(w.ref_block_sizes):
+            frame[off[k]:off[k + 1]] = -(k + 1)
+            inner[off[k]:off[k + 1]] = torch.arange(size, dtype=torch.int64)
+            width = _GRID_WIDTH.get(int(size), width)
+    else:
+        raise ValueError(which)
+    pos = (frame.double(), (inner // width).double(), (inner % width).double())
+    cols = []
+    for p, m in zip(pos, (m_t, m_hw, m_hw)):
+        freq = base ** (-torch.arange(m, dtype=torch.float64) / max(m, 1))
+        cols.append(p[:, None] * freq[None, :])
+    ang = torch.cat(cols, dim=1) if n else torch.zeros(0, half, dtype=torch.float64)
+    return torch.cos(ang).float().contiguous(), torch.sin(ang).float().contiguous()

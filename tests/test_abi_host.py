@@ -58,6 +58,8 @@ def test_null_handling():
     assert B.lib.sra_backward(None, None, None) == B.SRA_ERR_INVALID_ARG
     assert B.lib.sra_forward_host(None, None, None) == B.SRA_ERR_INVALID_ARG
     assert B.lib.sra_cache_bytes(None) == 0
+    assert B.lib.sra_cache_reference_kv_rope(None, None, None, None, None, None) == B.SRA_ERR_INVALID_ARG
+    assert B.lib.sra_apply_rope(None, None, None, None, None, 4, None) == B.SRA_ERR_INVALID_ARG
 
 
 def _covered_pairs(items, n_gen, n_ref):
@@ -230,6 +232,8 @@ def test_no_device_means_unsupported_not_fallback():
         dummy = ctypes.c_void_p(16)
         assert B.lib.sra_cache_reference_kv(ctx, dummy, dummy, None) == B.SRA_ERR_UNSUPPORTED
         assert b"no CUDA device" in B.lib.sra_last_error(ctx)
+        assert B.lib.sra_cache_reference_kv_rope(ctx, dummy, dummy, dummy, dummy, None) == B.SRA_ERR_UNSUPPORTED
+        assert B.lib.sra_apply_rope(ctx, dummy, None, dummy, dummy, 8, None) == B.SRA_ERR_UNSUPPORTED
         bw = B.sra_bwd_args()
         assert B.lib.sra_backward(ctx, ctypes.byref(bw), None) == B.SRA_ERR_UNSUPPORTED
     finally:
