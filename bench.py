@@ -656,6 +656,80 @@ def bench_short(args, w):
     print(json.dumps(out), flush=True)
 
 
+def bench_rope(args, w):
+    """--mode rope: the producer side of the reference-KV cache.  Pure data movement
+    with 6 FLOP per pair, so it is judged on HBM GB/s.  Times, per launch with the library's own CUDA events,
+      fused   : sra_cache_reference_kv_rope - rotate K_r inside the head-major cache write
+                (algorithmic bytes = read K_r, V_r + write both caches + the fp32 table once),
+      unfused : sra_apply_rope on K_r in place, then sra_cache_reference_kv (one more read + write of K_r),
+      step    : sra_apply_rope on the fresh Q_g, K_g of a denoising step (read + write of both + the table).
+    The headline value is the fused producer; the tensors (>= 0.8 GB) exceed L2, so nothing is flushed."""
+    import torch
+    from paper_2606_13872_b200 import binding as B
+    from paper_2606_13872_b200 import inputs as I
+    if int(os.environ.get("WORLD_SIZE", "1")) != 1:
+        raise SystemExit("bench.py --mode rope is a single-GPU diagnostic")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the SRA path has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    peaks, peaks_kind = load_peaks()
+    t = {n: I.make_tensor_device(w, n, dev) for n in ("k_ref", "v_ref", "q_gen", "k_gen")}
+    cr, sr = (x.to(dev) for x in I.rope_tables(w, "ref"))
+    cg, sg = (x.to(dev) for x in I.rope_tables(w, "gen"))
+    ctx = B.sra_create(w.batch, w.heads, w.head_dim, w.n_gen, w.ref_block_offsets)
+    B.sra_set_kernel_timing(ctx, True)
+    row = w.heads * w.head_dim * 2
+    kv_bytes = w.batch * w.n_ref * row
+    g_bytes = w.batch * w.n_gen * row
+    tab_ref, tab_gen = w.n_ref * w.head_dim * 4, w.n_gen * w.head_dim * 4   # cos + sin, [n, d/2] fp32 each
+    alg = {"fused": 4 * kv_bytes + tab_ref, "unfused": 6 * kv_bytes + tab_ref, "step": 4 * g_bytes + tab_gen}
+    ms = {"fused": [], "unfused": [], "step": []}
+    n_warm = max(args.warmup, 3)
+    launches0 = 0
+    sampler = ClockSampler(0)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for i in range(n_warm + args.steps):
+        if i == n_warm:
+            torch.cuda.synchronize()
+            launches0 = B.sra_launch_count(ctx)
+            sampler.start()
+            e0.record()
+        B.sra_cache_reference_kv_rope(ctx, t["k_ref"], t["v_ref"], cr, sr)
+        a = B.sra_kernel_time_ms(ctx, B.KERNEL_CACHE_RELAYOUT)
+        B.sra_apply_rope(ctx, t["k_ref"], None, cr, sr, w.n_ref)     # (values keep rotating; the timing does not care)
+        b = B.sra_kernel_time_ms(ctx, B.KERNEL_ROPE)
+        B.sra_cache_reference_kv(ctx, t["k_ref"], t["v_ref"])
+        b += B.sra_kernel_time_ms(ctx, B.KERNEL_CACHE_RELAYOUT)
+        B.sra_apply_rope(ctx, t["q_gen"], t["k_gen"], cg, sg, w.n_gen)
+        c = B.sra_kernel_time_ms(ctx, B.KERNEL_ROPE)
+        if i >= n_warm:
+            ms["fused"].append(a); ms["unfused"].append(b); ms["step"].append(c)
+    e1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    launches = B.sra_launch_count(ctx) - launches0
+    B.sra_destroy(ctx)
+    med = {k: statistics.median(v) for k, v in ms.items()}
+    gbs = {k: alg[k] / (med[k] * 1e-3) / 1e9 for k in med}
+    cfg = config_of(w, args)
+    cfg["step"] = "sra_cache_reference_kv_rope (fused RoPE + head-major cache write); also the unfused route and the per-step Q_g/K_g rotation"
+    cfg["l2"] = "tensors larger than L2, no flush"
+    out = {
+        "metric": "sra_rope_cache_producer_gbs", "value": gbs["fused"], "unit": "GB/s", "n_gpus": 1, "steps": args.steps,
+        "warmup": n_warm, "ms_per_step": med["fused"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16", "data": "synthetic", "config": cfg, "e2e": None, "gpu_launches": int(launches), "clocks": clocks,
+        "roofline": {"bound": "hbm", "kernel": "relayout_rope_head_major_kernel", "achieved": gbs["fused"],
+                     "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": gbs["fused"] / peaks["hbm_gbs"],
+                     "peak_kind": f"{peaks_kind} copy bandwidth", "kernel_ms": med["fused"],
+                     "algorithmic_bytes_per_launch": alg["fused"], "traffic": None},
+        "rope": {k: {"ms": med[k], "algorithmic_bytes": alg[k], "gbs": gbs[k]} for k in med},
+        "fused_over_unfused_time": med["fused"] / med["unfused"],
+        "cpu_baseline": None, "parity": None,
+    }
+    print(json.dumps(out), flush=True)
+
+
 def bench_sweep(args):
     """--mode sweep (BASELINE.json configs[3]; "linear in reference length"): one full forward
     layer (cache build + G and R rows) at 5 / 10 / 20 / 40 s of reference; fits t(N_r) = a + c N_r to the
@@ -713,7 +787,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default=None, help="default: 720p (--mode fwd), train (--mode train)")
-    ap.add_argument("--mode", default="fwd", choices=["fwd", "train", "short", "sweep"],
+    ap.add_argument("--mode", default="fwd", choices=["fwd", "train", "short", "sweep", "rope"],
                     help="fwd: the BASELINE metric (forward layer); train: configs[4] forward + backward; "
                          "short: cache-bound short-query cached steps (--workload short128|short512|short2048), HBM roofline; "
                          "sweep: configs[3] long-reference sweep, linear fit of time vs reference length")
@@ -744,6 +818,8 @@ def main():
         bench_short(args, w)
     elif args.mode == "sweep":
         bench_sweep(args)
+    elif args.mode == "rope":
+        bench_rope(args, w)
     else:
         bench_ours(args, w)
 
