@@ -730,6 +730,114 @@ def bench_rope(args, w):
     print(json.dumps(out), flush=True)
 
 
+def bench_ulysses(args, w):
+    """--mode ulysses: one cached denoising step of a SEQUENCE-SHARDED layer -
+    all-to-all to head shards, sra_forward per head chunk, all-to-all back, pipelined on a communication stream
+    (paper_2606_13872_b200/ulysses.py).  Strong scaling over heads: total work is fixed, rank r owns H / N heads.
+    With N = 1 (all this run can measure) the exchange is a self-exchange through NCCL plus the pack / unpack copies;
+    the line also reports the un-pipelined pieces (`direct_ms` = sra_forward alone on this rank's heads,
+    `exchange_ms` = the exchanges alone) so that the overlap is visible: pipelined ~ direct, not direct + exchange."""
+    import torch
+    import torch.distributed as dist
+    from paper_2606_13872_b200 import binding as B
+    from paper_2606_13872_b200 import dp, ulysses
+    from paper_2606_13872_b200 import inputs as I
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the SRA path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    else:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29577")
+        dist.init_process_group("nccl", rank=0, world_size=1, device_id=dev)
+    n_chunks = args.chunks
+    u = ulysses.UlyssesSRA(w.batch, w.heads, w.head_dim, w.n_gen, w.ref_block_offsets, n_chunks=n_chunks)
+    g0, gn = u.gen_shard()
+    r0, rn = u.ref_shard()
+    # every rank draws the whole tensor with the same seed and keeps its token shard (synthetic; no file, no exchange)
+    def shard(name, t0, n):
+        return I.make_tensor_device(w, name, dev)[:, t0:t0 + n].contiguous()
+    kr, vr = shard("k_ref", r0, rn), shard("v_ref", r0, rn)
+    u.cache_reference_kv(kr, vr)
+    del kr, vr
+    q, k, v = shard("q_gen", g0, gn), shard("k_gen", g0, gn), shard("v_gen", g0, gn)
+    torch.cuda.empty_cache()
+    fl = useful_flops(w, include_ref_rows=False)
+
+    def barrier():
+        dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, n):
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n):
+            fn()
+        e1.record()
+        barrier()
+        return dp.max_over_ranks(e0.elapsed_time(e1), dev) / n
+
+    for _ in range(max(args.warmup, 3)):
+        u.forward(q, k, v)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    launches0 = u.launches
+    ms = timed(lambda: u.forward(q, k, v), args.steps)
+    launches = u.launches - launches0
+    clocks = sampler.stop() if rank == 0 else None
+
+    # the pieces, un-pipelined, for comparison: the forwards alone first (same thermal / power state as the loop
+    # above), then the exchanges alone
+    staged = [(u._to_heads(q, w.n_gen, c), u._to_heads(k, w.n_gen, c), u._to_heads(v, w.n_gen, c)) for c in range(u.n_chunks)]
+    outs = [torch.empty_like(t[0]) for t in staged]
+
+    def direct():
+        for c in range(u.n_chunks):
+            if u.ctx[c]:
+                B.sra_forward(u.ctx[c], staged[c][0], staged[c][1], staged[c][2], outs[c])
+    direct()
+    direct_ms = timed(direct, args.steps)
+
+    def exchange_only():
+        o = torch.empty_like(q)
+        for c in range(u.n_chunks):
+            qh = u._to_heads(q, w.n_gen, c); u._to_heads(k, w.n_gen, c); u._to_heads(v, w.n_gen, c)
+            ulysses.heads_to_seq(qh, w.n_gen, w.heads, o, None, u.n_chunks, c)
+    exchange_only()
+    exchange_ms = timed(exchange_only, 5)
+    u.close()
+    dist.destroy_process_group()
+    if rank != 0:
+        return
+    peaks, peaks_kind = load_peaks()
+    value = fl / (ms * 1e-3) / 1e12
+    cfg = config_of(w, args)
+    cfg["parallelism"] = f"ulysses: {world} rank(s) x {w.heads // world if w.heads % world == 0 else w.heads / world} heads, {u.n_chunks} head chunks per rank"
+    cfg["step"] = "cached denoising step on sequence shards: all-to-all -> sra_forward per head chunk -> all-to-all, stream-pipelined"
+    cfg["l2"] = "tensors larger than L2, no flush"
+    out = {
+        "metric": "sra_ulysses_useful_tflops", "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+        "dtype": "bf16", "data": "synthetic", "config": cfg, "e2e": None, "gpu_launches": int(launches), "clocks": clocks,
+        "pieces": {"pipelined_ms": ms, "direct_ms": direct_ms, "exchange_ms": exchange_ms,
+                   "hidden_fraction_of_exchange": max(0.0, min(1.0, (direct_ms + exchange_ms - ms) / exchange_ms)) if exchange_ms > 0 else None},
+        "roofline": {"bound": "tensor", "kernel": "sra_fwd_kernel<128>", "achieved": fl / world / (direct_ms * 1e-3) / 1e12,
+                     "peak": peaks["bf16_tflops_sustained"], "unit": UNIT,
+                     "frac": fl / world / (direct_ms * 1e-3) / 1e12 / peaks["bf16_tflops_sustained"],
+                     "peak_kind": f"{peaks_kind} cuBLAS bf16, sustained", "kernel_ms": direct_ms,
+                     "algorithmic_flops_per_launch": fl / world / u.n_chunks, "traffic": None},
+        "cpu_baseline": None, "parity": None,
+    }
+    print(json.dumps(out), flush=True)
+
+
 def bench_sweep(args):
     """--mode sweep (BASELINE.json configs[3]; "linear in reference length"): one full forward
     layer (cache build + G and R rows) at 5 / 10 / 20 / 40 s of reference; fits t(N_r) = a + c N_r to the
@@ -787,7 +895,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default=None, help="default: 720p (--mode fwd), train (--mode train)")
-    ap.add_argument("--mode", default="fwd", choices=["fwd", "train", "short", "sweep", "rope"],
+    ap.add_argument("--mode", default="fwd", choices=["fwd", "train", "short", "sweep", "rope", "ulysses"],
                     help="fwd: the BASELINE metric (forward layer); train: configs[4] forward + backward; "
                          "short: cache-bound short-query cached steps (--workload short128|short512|short2048), HBM roofline; "
                          "sweep: configs[3] long-reference sweep, linear fit of time vs reference length")
@@ -795,7 +903,8 @@ def main():
                     help="--mode train: also check dQ/dK/dV of one (batch, head) against the oracle (minutes of CPU)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-oracle", action="store_true", help="skip the cpu_baseline / parity legs")
-    ap.add_argument("--oracle-rows", type=int, default=192, help="generation rows in the oracle sample")
+    ap.add_argument("--oracle-rows", type=int, default=768, help="generation rows in the oracle sample")
+    ap.add_argument("--chunks", type=int, default=4, help="--mode ulysses: head chunks per rank (pipeline depth)")
     ap.add_argument("--window", type=int, default=-1,
                     help="--mode fwd: sparse temporal attention window in latent frames (PAPER.md:143); -1 = off")
     ap.add_argument("--invalid-frac", type=float, default=0.0,
@@ -820,6 +929,8 @@ def main():
         bench_sweep(args)
     elif args.mode == "rope":
         bench_rope(args, w)
+    elif args.mode == "ulysses":
+        bench_ulysses(args, w)
     else:
         bench_ours(args, w)
 
