@@ -309,6 +309,7 @@ def bench_ours(args, w):
 
     # ---- e2e: HOST pinned buffers through sra_forward_host (H2D of q/k/v(+q_ref), D2H of o(+o_ref) timed)
     e2e = None
+    e2e_out = None
     try:
         host = {n: torch.empty(t[n].shape, dtype=torch.bfloat16).pin_memory() for n in ("q_gen", "k_gen", "v_gen")}
         for n in host:
@@ -338,11 +339,19 @@ def bench_ours(args, w):
         barrier()
         e2e_ms = dp.max_over_ranks(e0.elapsed_time(e1), dev)
         e2e_val = dp.sum_over_ranks(fl * n_e2e, dev) / (e2e_ms * 1e-3) / 1e12
-        same = bool(torch.equal(h_o_gen, o_gen.cpu()))
+        # the pipelined host path merges two fp32 partials for its reference-first slabs, so those rows may differ
+        # from the single-pass device path in the last bf16 bit; both are checked against the oracle below
+        o_dev = o_gen.cpu()
+        same = bool(torch.equal(h_o_gen, o_dev))
+        max_diff = float((h_o_gen.float() - o_dev.float()).abs().max())
+        ulp_top = float(o_dev.float().abs().max()) * 2.0 ** -7
+        del o_dev
         e2e = {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                "ms_per_step": e2e_ms / n_e2e, "steps": n_e2e, "api": "sra_forward_host (C ABI, host pointers)",
-               "matches_device_path": same}
-        del host, h_o_gen, h_q_ref, h_o_ref
+               "matches_device_path": bool(max_diff <= ulp_top), "bit_identical_to_device_path": same,
+               "max_abs_diff_vs_device_path": max_diff}
+        e2e_out = (h_o_gen, h_o_ref)
+        del host, h_q_ref
     except Exception as ex:  # pinned allocation can fail on a small box: report, do not hide
         log(f"e2e leg failed: {ex!r}")
         e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0, "error": repr(ex)}
@@ -380,6 +389,18 @@ def bench_ours(args, w):
                   "ok": bool(diff.max() <= MAX_ABS_TOL and diff.mean() <= MEAN_ABS_TOL and rel_l2 <= REL_L2_TOL
                              and np.isfinite(got).all()),
                   "rows": int(len(rows)), "heads": heads}
+        if e2e_out is not None and e2e is not None and e2e.get("value") is not None:
+            # the same sampled rows of what sra_forward_host returned, against the same oracle values
+            hg = [e2e_out[0][:, torch.as_tensor(g_rows).long()][:, :, heads].float().numpy()]
+            if len(r_rows) and e2e_out[1] is not None:
+                hg.append(e2e_out[1][:, torch.as_tensor(r_rows).long()][:, :, heads].float().numpy())
+            hg = np.concatenate(hg, axis=1).astype(np.float64)
+            hd = np.abs(hg - o_or)
+            h_rel = float(np.linalg.norm(hg - o_or) / max(np.linalg.norm(o_or), 1e-300))
+            e2e["parity"] = {"max_abs": float(hd.max()), "mean_abs": float(hd.mean()), "rel_l2": h_rel,
+                             "ok": bool(hd.max() <= MAX_ABS_TOL and hd.mean() <= MEAN_ABS_TOL and h_rel <= REL_L2_TOL
+                                        and np.isfinite(hg).all())}
+    e2e_out = None
 
     B.sra_destroy(ctx)
     if rank != 0:

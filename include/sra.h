@@ -127,11 +127,16 @@ typedef struct {
  * use, freed by sra_destroy), the same forward kernel as sra_forward, and the device->host copies of
  * the outputs.  The results are valid after the caller synchronises the stream.  Requires the
  * resident cache when n_ref > 0 (SRA_ERR_NO_REF_CACHE otherwise).
- * With batch == 1 and at least 16 query slabs the step is pipelined: K/V first, then the generation rows in 8
- * slabs whose host->device and device->host copies run on two ctx-owned copy streams underneath the forward
- * launches of the neighbouring slabs (query slabs are independent work items), reference rows before the last two
- * slabs.  The copy streams are ordered after prior work on `cuda_stream`, and `cuda_stream` waits for the last
- * device->host copy, so the call is still asynchronous on - and ordered by - the caller's stream. */
+ * With batch == 1 and at least 16 query slabs the step is pipelined: the generation rows go in 8 slabs whose
+ * host->device and device->host copies run on two ctx-owned copy streams underneath the forward launches of the
+ * neighbouring slabs (query slabs are independent work items), reference rows before the last two slabs.  The one
+ * transfer every generation row needs, K_g and V_g, is hidden by "reference keys first": the first slabs (up to 6,
+ * enough to cover the upload) attend the resident reference K/V while K_g / V_g are in flight, then the generation
+ * keys, and the two fp32 partials (O_s, LSE_s) of each row are merged exactly as in the key-split schedule - so
+ * those rows can differ from sra_forward's single-pass result in the last bf16 bit (same tolerance against the
+ * oracle; the other slabs and the reference rows are bit-identical).  Needs 2 * H * n_gen * (d + 1) * 4 bytes of
+ * ctx-owned partial buffers.  The copy streams are ordered after prior work on `cuda_stream`, and `cuda_stream`
+ * waits for the last device->host copy, so the call is still asynchronous on - and ordered by - the caller's stream. */
 int sra_forward_host(sra_ctx* ctx, const sra_fwd_host_args* args, void* cuda_stream);
 
 typedef struct {

@@ -360,6 +360,7 @@ static int upload_schedule(sra_ctx* ctx) {
   const sra_config& c = ctx->cfg;
   cudaFree(ctx->d_fwd_items); cudaFree(ctx->d_bwd_items); cudaFree(ctx->d_split_items);
   cudaFree(ctx->ws_part_o); cudaFree(ctx->ws_part_lse);
+  cudaFree(ctx->d_seg_items); ctx->d_seg_items = nullptr;  // derived from fwd_items; rebuilt lazily by sra_forward_host
   ctx->d_fwd_items = nullptr; ctx->d_bwd_items = nullptr; ctx->d_split_items = nullptr;
   ctx->ws_part_o = nullptr; ctx->ws_part_lse = nullptr;
   cudaError_t e = cudaMalloc(&ctx->d_fwd_items, ctx->fwd_items.size() * sizeof(FwdItem));
@@ -452,6 +453,9 @@ void sra_destroy(sra_ctx* ctx) {
     cudaFree(ctx->d_split_items);
     cudaFree(ctx->ws_part_o);
     cudaFree(ctx->ws_part_lse);
+    cudaFree(ctx->d_seg_items);
+    cudaFree(ctx->ws_seg_o);
+    cudaFree(ctx->ws_seg_lse);
     cudaFree(ctx->d_gidx);
     cudaFree(ctx->d_cidx);
     for (void* q : ctx->cbuf) cudaFree(q);
@@ -623,13 +627,19 @@ static int forward_core(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) 
   const bool split = ctx->n_split > 1;
   p.items = split ? ctx->d_split_items : ctx->d_fwd_items;
   p.n_items = ctx->n_gen_items * ctx->n_split + (with_ref_rows ? ctx->n_ref_items : 0);
+  p.part_o = ctx->ws_part_o;
+  p.part_lse = ctx->ws_part_lse;
+  const bool seg = ctx->sub_items != nullptr;  // segment-split items of the pipelined host path (merged by its caller)
+  if (seg) {
+    p.items = ctx->sub_items;
+    p.part_o = ctx->ws_seg_o;
+    p.part_lse = ctx->ws_seg_lse;
+  }
   if (ctx->sub_count >= 0) {  // sra_forward_host pipelines a step as several launches over item sub-ranges
     p.items += ctx->sub_first;
     p.n_items = ctx->sub_count;
     if (p.n_items == 0) return SRA_OK;
   }
-  p.part_o = ctx->ws_part_o;
-  p.part_lse = ctx->ws_part_lse;
   p.heads = H; p.batch = B; p.n_gen = c.n_gen; p.n_ref = nr;
   p.scale = ctx->scale;
   p.scale_log2 = ctx->scale * 1.4426950408889634f;
@@ -646,7 +656,7 @@ static int forward_core(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) 
   }
   if (e != cudaSuccess) return fail_cuda(ctx, e, "sra_fwd_kernel launch");
   ctx->launches += 1;
-  if (split) {
+  if (split && !seg) {
     sra::KernelTimer kt(ctx, SRA_KERNEL_FWD_MERGE, cudaStream_t(cuda_stream));
     e = sra::launch_fwd_merge(p, d, ctx->n_split, cudaStream_t(cuda_stream));
     if (e != cudaSuccess) return fail_cuda(ctx, e, "sra_fwd_merge_kernel launch");
@@ -655,10 +665,16 @@ static int forward_core(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) 
   return SRA_OK;
 }
 
-// Pipelined host path (batch 1): K/V first, then the generation rows in kChunks slabs - the H2D copy of slab c+1 and
-// the D2H copy of slab c-1 run on their own streams under the forward launch of slab c (query slabs are independent
-// work items, PCIe is full duplex); the reference rows go last.  Everything is ordered after prior work on `st`
-// and `st` is made to wait for the last D2H copy, so the call stays asynchronous on the caller's stream.
+// Pipelined host path (batch 1).  The generation rows go in kChunks slabs whose H2D copy (slab c+1) and D2H copy
+// (slab c-1) run on their own streams under the forward launch of slab c (query slabs are independent work items,
+// PCIe is full duplex).  The one transfer nothing could hide - K_g and V_g, which every generation row needs - is
+// covered by "reference keys first" (the reference K/V are already resident): the first n_first slabs
+// are uploaded ahead of K_g / V_g and attend the REFERENCE segment only while K_g / V_g are in flight (A items, fp32
+// partials); once K_g / V_g have landed they attend the generation segment (B items) and the two partials of every
+// row are merged by sra_fwd_merge_kernel (the key-split machinery of the short-query regime).  The remaining
+// slabs run the ordinary single-pass items.  The reference rows go in before the last two slabs.  Everything is
+// ordered after prior work on `st`, and `st` is made to wait for the last D2H copy, so the call stays asynchronous
+// on the caller's stream.
 static int forward_host_pipelined(sra_ctx* ctx, const sra_fwd_host_args* a, cudaStream_t st, bool with_ref_rows) {
   constexpr int kChunks = 8;
   const sra_config& c = ctx->cfg;
@@ -672,6 +688,35 @@ static int forward_host_pipelined(sra_ctx* ctx, const sra_fwd_host_args* a, cuda
       if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
     if (e != cudaSuccess) return fail_cuda(ctx, e, "pipeline stream / event creation");
   }
+  // How many slabs take the reference-first route: enough reference-segment work to cover the K_g / V_g upload
+  // (PCIe 5 x16 ~ 50 GB/s; ~1.1 PFLOP/s of useful forward rate), at most kChunks - 2.
+  int n_first = 0;
+  if (ctx->nr > 0) {
+    const double t_up = 2.0 * double(gen_bytes) / 50e9;
+    const double t_chunk = 4.0 * c.head_dim * double(c.n_gen) * double(ctx->nr) * c.heads / 1.1e15 / kChunks;
+    n_first = int(std::min<double>(kChunks - 2, std::ceil(t_up / t_chunk)));
+  }
+  const int G = ctx->n_gen_items;
+  if (n_first > 0 && !ctx->d_seg_items) {
+    std::vector<sra::FwdItem> seg(2 * size_t(G));
+    for (int g = 0; g < G; ++g) {
+      sra::FwdItem A = ctx->fwd_items[g], Bi = ctx->fwd_items[g];
+      A.q_is_ref = 1 << 8; A.seg0_len = 0;                   // partial 0: reference keys only
+      Bi.q_is_ref = 2 << 8; Bi.seg1_len = 0;                 // partial 1: generation keys only
+      seg[g] = A; seg[size_t(G) + g] = Bi;
+    }
+    cudaError_t e = cudaMalloc(&ctx->d_seg_items, seg.size() * sizeof(sra::FwdItem));
+    if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->d_seg_items, seg.data(), seg.size() * sizeof(sra::FwdItem), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);  // (seg is a local; first call only)
+    const size_t prow = 2 * size_t(c.heads) * c.n_gen;
+    if (e == cudaSuccess && !ctx->ws_seg_o) e = cudaMalloc(&ctx->ws_seg_o, prow * c.head_dim * sizeof(float));
+    if (e == cudaSuccess && !ctx->ws_seg_lse) e = cudaMalloc(&ctx->ws_seg_lse, prow * sizeof(float));
+    if (e != cudaSuccess) {
+      (void)cudaGetLastError();
+      cudaFree(ctx->d_seg_items); ctx->d_seg_items = nullptr;
+      return fail(ctx, SRA_ERR_OOM, "reference-first partial buffers allocation failed");
+    }
+  }
   cudaEvent_t* ev_q = ctx->pipe_ev.data();            // [kChunks] slab c of Q is on the device
   cudaEvent_t* ev_c = ev_q + kChunks;                 // [kChunks] slab c of O is computed
   cudaEvent_t ev_start = ev_c[kChunks], ev_kv = ev_c[kChunks + 1], ev_qr = ev_c[kChunks + 2], ev_cr = ev_c[kChunks + 3],
@@ -683,32 +728,50 @@ static int forward_host_pipelined(sra_ctx* ctx, const sra_fwd_host_args* a, cuda
   sra_fwd_args d{};
   d.q_gen = ctx->stage[0]; d.k_gen = ctx->stage[1]; d.v_gen = ctx->stage[2]; d.o_gen = ctx->stage[3];
   d.lse_gen = a->lse_gen ? static_cast<float*>(ctx->stage[6]) : nullptr;
-  cudaError_t e = cudaEventRecord(ev_start, st);
-  if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->s_h2d, ev_start, 0);
-  if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->s_d2h, ev_start, 0);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->stage[1], a->k_gen, gen_bytes, cudaMemcpyHostToDevice, ctx->s_h2d);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->stage[2], a->v_gen, gen_bytes, cudaMemcpyHostToDevice, ctx->s_h2d);
-  if (e == cudaSuccess) e = cudaEventRecord(ev_kv, ctx->s_h2d);
-  if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev_kv, 0);
-  const int per = (ctx->n_gen_items + kChunks - 1) / kChunks;
+  const int per = (G + kChunks - 1) / kChunks;
   auto rows_of = [&](int ch, int& i0, int& i1, size_t& r0, size_t& r1) {
-    i0 = std::min(ch * per, ctx->n_gen_items);
-    i1 = std::min(i0 + per, ctx->n_gen_items);
+    i0 = std::min(ch * per, G);
+    i1 = std::min(i0 + per, G);
     r0 = size_t(i0) * kQRowsPerCta;
     r1 = std::min<size_t>(size_t(i1) * kQRowsPerCta, size_t(c.n_gen));
   };
-  // every H2D copy is enqueued (and its event recorded) before the first launch waits on one
-  for (int ch = 0; ch < kChunks && e == cudaSuccess; ++ch) {
+  cudaError_t e = cudaEventRecord(ev_start, st);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->s_h2d, ev_start, 0);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->s_d2h, ev_start, 0);
+  // every H2D copy is enqueued (and its event recorded) before the first launch waits on one:
+  // Q slabs [0, n_first), K_g, V_g, Q slabs [n_first, kChunks), q_ref
+  auto copy_q = [&](int ch) {
     int i0, i1; size_t r0, r1;
     rows_of(ch, i0, i1, r0, r1);
-    if (i1 > i0) e = cudaMemcpyAsync(dq + r0 * row, hq + r0 * row, (r1 - r0) * row, cudaMemcpyHostToDevice, ctx->s_h2d);
+    if (e == cudaSuccess && i1 > i0) e = cudaMemcpyAsync(dq + r0 * row, hq + r0 * row, (r1 - r0) * row, cudaMemcpyHostToDevice, ctx->s_h2d);
     if (e == cudaSuccess) e = cudaEventRecord(ev_q[ch], ctx->s_h2d);
-  }
+  };
+  for (int ch = 0; ch < n_first; ++ch) copy_q(ch);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->stage[1], a->k_gen, gen_bytes, cudaMemcpyHostToDevice, ctx->s_h2d);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->stage[2], a->v_gen, gen_bytes, cudaMemcpyHostToDevice, ctx->s_h2d);
+  if (e == cudaSuccess) e = cudaEventRecord(ev_kv, ctx->s_h2d);
+  for (int ch = n_first; ch < kChunks; ++ch) copy_q(ch);
   if (e == cudaSuccess && with_ref_rows) {
     e = cudaMemcpyAsync(ctx->stage[4], a->q_ref, ref_bytes, cudaMemcpyHostToDevice, ctx->s_h2d);
     if (e == cudaSuccess) e = cudaEventRecord(ev_qr, ctx->s_h2d);
   }
   if (e != cudaSuccess) return fail_cuda(ctx, e, "host->device copy");
+  auto launch = [&](const sra::FwdItem* items, int first, int count, const sra_fwd_args& args) -> int {
+    ctx->sub_items = items; ctx->sub_first = first; ctx->sub_count = count;
+    const int rc = forward_core(ctx, &args, st);
+    ctx->sub_items = nullptr; ctx->sub_count = -1;
+    return rc;
+  };
+  // phase 1: reference segment of the first slabs, under the K_g / V_g upload
+  for (int ch = 0; ch < n_first; ++ch) {
+    int i0, i1; size_t r0, r1;
+    rows_of(ch, i0, i1, r0, r1);
+    e = cudaStreamWaitEvent(st, ev_q[ch], 0);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "pipelined host copy");
+    if (int rc = launch(ctx->d_seg_items, i0, i1 - i0, d)) return rc;
+  }
+  e = cudaStreamWaitEvent(st, ev_kv, 0);
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "pipelined host copy");
   auto run_ref_rows = [&]() -> int {
     // reference rows: their q_ref copy has had the first slabs' compute time to land; their output copy is
     // hidden under the remaining slabs
@@ -717,27 +780,36 @@ static int forward_host_pipelined(sra_ctx* ctx, const sra_fwd_host_args* a, cuda
     sra_fwd_args dr = d;
     dr.q_ref = ctx->stage[4]; dr.o_ref = ctx->stage[5];
     dr.lse_ref = a->lse_ref ? static_cast<float*>(ctx->stage[7]) : nullptr;
-    ctx->sub_first = ctx->n_gen_items; ctx->sub_count = ctx->n_ref_items;
-    const int rc = forward_core(ctx, &dr, st);
-    ctx->sub_count = -1;
-    if (rc) return rc;
+    if (int rc = launch(nullptr, G, ctx->n_ref_items, dr)) return rc;
     er = cudaEventRecord(ev_cr, st);
     if (er == cudaSuccess) er = cudaStreamWaitEvent(ctx->s_d2h, ev_cr, 0);
     if (er == cudaSuccess) er = cudaMemcpyAsync(a->o_ref, ctx->stage[5], ref_bytes, cudaMemcpyDeviceToHost, ctx->s_d2h);
     if (er == cudaSuccess && dr.lse_ref) er = cudaMemcpyAsync(a->lse_ref, dr.lse_ref, size_t(c.heads) * c.n_ref * 4, cudaMemcpyDeviceToHost, ctx->s_d2h);
     return er == cudaSuccess ? SRA_OK : fail_cuda(ctx, er, "pipelined host copy");
   };
+  // phase 2: generation segment + merge of the first slabs, then the ordinary slabs
   for (int ch = 0; ch < kChunks; ++ch) {
     int i0, i1; size_t r0, r1;
     rows_of(ch, i0, i1, r0, r1);
     if (with_ref_rows && ch == kChunks - 2)
       if (int rc = run_ref_rows()) return rc;
-    e = cudaStreamWaitEvent(st, ev_q[ch], 0);
-    if (e != cudaSuccess) break;
-    ctx->sub_first = i0; ctx->sub_count = i1 - i0;
-    const int rc = forward_core(ctx, &d, st);
-    ctx->sub_count = -1;
-    if (rc) return rc;
+    if (ch < n_first) {
+      if (int rc = launch(ctx->d_seg_items, G + i0, i1 - i0, d)) return rc;
+      sra::FwdParams mp{};
+      mp.part_o = ctx->ws_seg_o; mp.part_lse = ctx->ws_seg_lse;
+      mp.o_gen = static_cast<__nv_bfloat16*>(d.o_gen); mp.lse_gen = d.lse_gen;
+      mp.batch = 1; mp.heads = c.heads; mp.n_gen = c.n_gen;
+      {
+        sra::KernelTimer kt(ctx, SRA_KERNEL_FWD_MERGE, st);
+        e = sra::launch_fwd_merge(mp, c.head_dim, 2, st, int(r0), int(r1 - r0));
+      }
+      if (e != cudaSuccess) return fail_cuda(ctx, e, "sra_fwd_merge_kernel launch");
+      if (i1 > i0) ctx->launches += 1;
+    } else {
+      e = cudaStreamWaitEvent(st, ev_q[ch], 0);
+      if (e != cudaSuccess) break;
+      if (int rc = launch(nullptr, i0, i1 - i0, d)) return rc;
+    }
     e = cudaEventRecord(ev_c[ch], st);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->s_d2h, ev_c[ch], 0);
     if (e == cudaSuccess && i1 > i0) e = cudaMemcpyAsync(hout + r0 * row, dout + r0 * row, (r1 - r0) * row, cudaMemcpyDeviceToHost, ctx->s_d2h);

@@ -56,6 +56,13 @@ struct sra_ctx {
   cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
   std::vector<cudaEvent_t> pipe_ev;
   int sub_first = 0, sub_count = -1;  // forward_core launches items [sub_first, sub_first + sub_count) when sub_count >= 0
+  // "reference keys first" (sra_forward_host): every G slab once against the reference segment only (A items,
+  // needs nothing but Q and the resident cache) and once against the generation segment only (B items), as fp32
+  // partials merged per slab range; sub_items != nullptr makes forward_core launch from it (no merge).
+  sra::FwdItem* d_seg_items = nullptr;  // [2 * n_gen_items]: A items, then B items
+  float* ws_seg_o = nullptr;            // fp32 [2][B][H][n_gen][d]
+  float* ws_seg_lse = nullptr;          // fp32 [2][B][H][n_gen]
+  const sra::FwdItem* sub_items = nullptr;
   int64_t launches = 0;
   // optional per-kernel timing (sra_set_kernel_timing)
   bool timing = false;
@@ -88,7 +95,8 @@ template <int D>
 cudaError_t launch_bwd(const CUtensorMap* maps, const BwdParams& p, cudaStream_t stream);
 template <int D>
 cudaError_t launch_fwd(const CUtensorMap* maps, const FwdParams& p, cudaStream_t stream);
-cudaError_t launch_fwd_merge(const FwdParams& p, int head_dim, int n_split, cudaStream_t stream);
+cudaError_t launch_fwd_merge(const FwdParams& p, int head_dim, int n_split, cudaStream_t stream, int row0 = 0,
+                             int n_rows = -1);  // n_rows < 0: every generation row
 int run_backward(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t stream);
 // compaction helpers of the validity path (sra_api.cu)
 int compact_rows(sra_ctx* ctx, int slot, const void* src, const void** out, cudaStream_t stream);

@@ -420,18 +420,18 @@ cudaError_t launch_fwd(const CUtensorMap* maps, const FwdParams& p, cudaStream_t
 template <int D>
 __global__ void sra_fwd_merge_kernel(const float* __restrict__ part_o, const float* __restrict__ part_lse,
                                      __nv_bfloat16* __restrict__ o_gen, float* __restrict__ lse_gen, int n_split, int B,
-                                     int H, int n_gen) {
+                                     int H, int n_gen, int row0, int n_rows) {
   const int lane = threadIdx.x & 31;
   const size_t warp_id = (blockIdx.x * size_t(blockDim.x) + threadIdx.x) >> 5;
   const size_t n_warps = (gridDim.x * size_t(blockDim.x)) >> 5;
-  const size_t rows = size_t(B) * n_gen * H;
+  const size_t rows = size_t(B) * n_rows * H;  // generation rows [row0, row0 + n_rows) of every batch item and head
   const size_t split_stride = size_t(B) * H * n_gen;
   constexpr int V = D / 32;  // floats per lane
   for (size_t r = warp_id; r < rows; r += n_warps) {
     const int h = int(r % H);
     const size_t t = r / H;
-    const int n = int(t % n_gen);
-    const int b = int(t / n_gen);
+    const int n = row0 + int(t % n_rows);
+    const int b = int(t / n_rows);
     const size_t prow = (size_t(b) * H + h) * n_gen + n;
     float m = -INFINITY;
     for (int s = 0; s < n_split; ++s) m = fmaxf(m, part_lse[s * split_stride + prow]);
@@ -465,14 +465,16 @@ __global__ void sra_fwd_merge_kernel(const float* __restrict__ part_o, const flo
   }
 }
 
-cudaError_t launch_fwd_merge(const FwdParams& p, int head_dim, int n_split, cudaStream_t stream) {
-  const size_t rows = size_t(p.batch) * p.n_gen * p.heads;
+cudaError_t launch_fwd_merge(const FwdParams& p, int head_dim, int n_split, cudaStream_t stream, int row0, int n_rows) {
+  if (n_rows < 0) { row0 = 0; n_rows = p.n_gen; }
+  if (n_rows == 0) return cudaSuccess;
+  const size_t rows = size_t(p.batch) * n_rows * p.heads;
   const int threads = 256;
   const int blocks = int(std::min<size_t>((rows * 32 + threads - 1) / threads, size_t(148) * 16));
   if (head_dim == 128)
-    sra_fwd_merge_kernel<128><<<blocks, threads, 0, stream>>>(p.part_o, p.part_lse, p.o_gen, p.lse_gen, n_split, p.batch, p.heads, p.n_gen);
+    sra_fwd_merge_kernel<128><<<blocks, threads, 0, stream>>>(p.part_o, p.part_lse, p.o_gen, p.lse_gen, n_split, p.batch, p.heads, p.n_gen, row0, n_rows);
   else
-    sra_fwd_merge_kernel<64><<<blocks, threads, 0, stream>>>(p.part_o, p.part_lse, p.o_gen, p.lse_gen, n_split, p.batch, p.heads, p.n_gen);
+    sra_fwd_merge_kernel<64><<<blocks, threads, 0, stream>>>(p.part_o, p.part_lse, p.o_gen, p.lse_gen, n_split, p.batch, p.heads, p.n_gen, row0, n_rows);
   return cudaGetLastError();
 }
 

@@ -152,16 +152,38 @@ def test_480p_sampled_rows():
 
 @pytest.mark.parametrize("name", ["host_pipe", "ragged"])
 def test_forward_host_matches_device_path(name):
-    """sra_forward_host (HOST pointers; the e2e leg of bench.py): the pipelined path (batch 1, >= 16 query slabs: K/V
-    first, then query slabs with copies overlapped on their own streams) and the plain path (everything else) must
-    return exactly the bytes sra_forward returns for the same inputs."""
+    """sra_forward_host (HOST pointers; the e2e leg of bench.py).  The plain path (everything small) must return exactly
+    the bytes sra_forward returns.  The pipelined path (batch 1, >= 16 query slabs) runs its first slabs "reference
+    keys first" - two fp32 partials per row (reference segment, generation segment) merged afterwards - so those rows
+    may differ from the single-pass result in the last bf16 bit: every element within one bf16 ulp of the row's scale,
+    the single-pass slabs and the reference rows bit-identical, and the whole output within the contract tolerance of
+    the fp64 oracle (max-abs <= 2e-2, mean-abs <= 2e-3, rel_l2 <= 1e-2, LSE <= 2e-3)."""
     from paper_2606_13872_b200 import binding as B
-    w = (sra_inputs.SRAWorkload("host_pipe", 1, 2, 128, 4200, (700, 300), "B", 0) if name == "host_pipe"
+    from oracle import sra_oracle
+    w = (sra_inputs.SRAWorkload("host_pipe", 1, 2, 128, 6000, (700, 300), "B", 0) if name == "host_pipe"
          else sra_inputs.WORKLOADS[name])
+    pipelined = name == "host_pipe"
     t = sra_inputs.make_inputs(w)
     dev_out = run_gpu_forward(w, t, use_cache=True)
     dev = torch.device("cuda:0")
     ctx = B.sra_create(w.batch, w.heads, w.head_dim, w.n_gen, w.ref_block_offsets)
+
+    def check_gen(o, lse):
+        o = o.float().numpy()
+        if not pipelined:
+            assert np.array_equal(o, dev_out["o_gen"])
+            assert lse is None or np.array_equal(lse.numpy(), dev_out["lse_gen"])
+            return
+        ulp = 2.0 ** -7 * np.abs(dev_out["o_gen"]).max(axis=-1, keepdims=True)   # one bf16 ulp at the row's largest element
+        assert np.all(np.abs(o - dev_out["o_gen"]) <= ulp)
+        differs = np.flatnonzero((o != dev_out["o_gen"]).any(axis=(0, 2, 3)))
+        n_items = -(-w.n_gen // 256)                                               # 256-row query slabs (kQRowsPerCta)
+        tail = 6 * (-(-n_items // 8)) * 256                                        # the last two of 8 slab groups are never split
+        assert tail < w.n_gen
+        assert differs.size == 0 or differs.max() < tail, "single-pass slabs must be bit-identical to sra_forward"
+        if lse is not None:
+            assert np.abs(lse.numpy() - dev_out["lse_gen"]).max() <= 1e-5
+
     try:
         B.sra_cache_reference_kv(ctx, t["k_ref"].to(dev), t["v_ref"].to(dev))
         h = {k: t[k].pin_memory() for k in ("q_gen", "k_gen", "v_gen", "q_ref")}
@@ -173,13 +195,19 @@ def test_forward_host_matches_device_path(name):
             B.sra_forward_host(ctx, h["q_gen"], h["k_gen"], h["v_gen"], o_gen, q_ref=h["q_ref"], o_ref=o_ref,
                                lse_gen=lse_gen, lse_ref=lse_ref)
             torch.cuda.synchronize()
-            assert np.array_equal(o_gen.float().numpy(), dev_out["o_gen"])
+            check_gen(o_gen, lse_gen)
             assert np.array_equal(o_ref.float().numpy(), dev_out["o_ref"])
-            assert np.array_equal(lse_gen.numpy(), dev_out["lse_gen"]) and np.array_equal(lse_ref.numpy(), dev_out["lse_ref"])
+            assert np.array_equal(lse_ref.numpy(), dev_out["lse_ref"])
+            if pipelined:  # the host path on its own against the oracle, every row
+                tb = bits(t)
+                ref = sra_oracle.sra_forward(tb["q_gen"], tb["k_gen"], tb["v_gen"], tb["q_ref"], tb["k_ref"], tb["v_ref"],
+                                             w.ref_block_offsets, 1.0 / math.sqrt(w.head_dim))
+                assert_parity(o_gen.float().numpy(), ref["o_gen"], "host_pipe O_g through sra_forward_host")
+                assert np.abs(lse_gen.numpy() - ref["lse_gen"]).max() <= LSE_TOL
             o_gen.fill_(float("nan")); o_ref.fill_(float("nan"))
         # cached denoising step through the host entry point (no reference rows)
         B.sra_forward_host(ctx, h["q_gen"], h["k_gen"], h["v_gen"], o_gen, lse_gen=lse_gen)
         torch.cuda.synchronize()
-        assert np.array_equal(o_gen.float().numpy(), dev_out["o_gen"])
+        check_gen(o_gen, lse_gen)
     finally:
         B.sra_destroy(ctx)
