@@ -732,8 +732,10 @@ static int forward_host_pipelined(sra_ctx* ctx, const sra_fwd_host_args* a, cuda
   auto rows_of = [&](int ch, int& i0, int& i1, size_t& r0, size_t& r1) {
     i0 = std::min(ch * per, G);
     i1 = std::min(i0 + per, G);
-    r0 = size_t(i0) * kQRowsPerCta;
-    r1 = std::min<size_t>(size_t(i1) * kQRowsPerCta, size_t(c.n_gen));
+    // G items are ordered by row and tile [0, n_gen) (with a temporal window they are cut at frame boundaries, so
+    // an item is not always kQRowsPerCta rows)
+    r0 = i0 < G ? size_t(ctx->fwd_items[i0].q_row0) : size_t(c.n_gen);
+    r1 = i1 < G ? size_t(ctx->fwd_items[i1].q_row0) : size_t(c.n_gen);
   };
   cudaError_t e = cudaEventRecord(ev_start, st);
   if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->s_h2d, ev_start, 0);
