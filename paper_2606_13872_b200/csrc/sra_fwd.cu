@@ -3,14 +3,15 @@
 // One CTA = one work item (a 256-row query slab of G or of one R block) x one (batch, head).
 // The slab is two 128-row Q tiles that ping-pong on the tensor core:
 //
-//   warps 0-3   softmax warpgroup of Q tile 0   (thread = one query row, TMEM lane = row)
-//   warps 4-7   softmax warpgroup of Q tile 1
-//   warp  8     MMA issuer (one thread): S_i = Q_i K_j^T (SS), O_i += P_i V_j (A = P from TMEM)
-//   warp  9     TMA loader (one thread): Q once, then the K/V tile ring
+//   warps 0-7   softmax: warps w and w + 4 share the 32 query rows (TMEM lanes) of sub-partition w & 3; warp w takes
+//               key columns [0, 64) of every score tile, warp w + 4 columns [64, 128), for both Q tiles in turn
+//   warp  8     MMA issuer (one elected thread): S_i = Q_i K_j^T (SS), O_i += P_i V_j (A = P from TMEM)
+//   warp  9     TMA loader (one elected thread): Q once, then the K/V tile ring
 //   warps 10-11 idle (they only pad the third warpgroup for setmaxnreg)
 //
-// TMEM (512 columns x 128 lanes x fp32): S0 @0, S1 @128, O0 @256, O1 @256+D; P_i (bf16, 64
-// columns) aliases the first 64 columns of S_i once the softmax thread holds S_i in registers.
+// TMEM (512 columns x 128 lanes x fp32): S0 @0, S1 @128, O0 @256, O1 @256+D.  P_i (bf16) overwrites S_i in two
+// pieces, each written by the warp that read the scores underneath it: keys [0, 64) -> columns [0, 32) of S_i,
+// keys [64, 128) -> columns [64, 96); the PV MMA takes its K steps from there.
 // Masked tiles are never visited: the key-tile loop walks only the item's visible segments;
 // only the last tile of a segment pays for a column mask (n_valid < 128).
 #include <algorithm>
@@ -34,7 +35,7 @@ struct FwdCfg {
   static constexpr int kBoxes = D / 64;                      // 64-column (128 B) TMA boxes per tile
   static constexpr int kBoxBytes = kTile * 128;              // 16 KB
   static constexpr int kStages = (D == 128) ? 5 : 10;        // K/V ring depth (tiles)
-  static constexpr int kNumBars = 1 + 2 * kStages + 6;
+  static constexpr int kNumBars = 1 + 2 * kStages + 6 + 4;
   static constexpr int kXchBytes = 2 * 2 * kTile * 4;       // (slot, half, row) floats swapped by the two threads of a row
   static constexpr int kSmemBytes = (2 + kStages) * kTileBytes + kNumBars * 8 + 16 + kXchBytes;
   static constexpr int kTmemCols = 512;
@@ -72,7 +73,8 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
   const uint32_t bar_s_full = bar_kv_empty + 8 * C::kStages;
   const uint32_t bar_p_full = bar_s_full + 16;
   const uint32_t bar_o_full = bar_p_full + 16;
-  const uint32_t s_tmem_ptr = bar_o_full + 16;
+  const uint32_t bar_x = bar_o_full + 16;                // [4] one per row group: the two warps of a row swap a float
+  const uint32_t s_tmem_ptr = bar_x + 32;
   const uint32_t sXch = s_tmem_ptr + 16;
   uint32_t* tmem_ptr_generic = reinterpret_cast<uint32_t*>(smem_raw + (s_tmem_ptr - smem_u32(smem_raw)));
 
@@ -100,6 +102,7 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
       mbar_init(bar_p_full + 8 * i, 256);
       mbar_init(bar_o_full + 8 * i, 1);
     }
+    for (int g = 0; g < 4; ++g) mbar_init(bar_x + 8 * g, 64);
     fence_mbar_init();
   }
   if (warp == 9 && lane == 0) {
@@ -137,16 +140,25 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
     float m_ref[2] = {-INFINITY, -INFINITY};
     float m_seen[2] = {-INFINITY, -INFINITY};  // max raw score over the tiles processed so far
     float l[2] = {0.f, 0.f};                   // this thread's half of sum exp2((s - m_ref) * sl2)
-    uint32_t slot = 0;                         // exchange-buffer parity, toggles at every named barrier
-    // One float per (slot, half, row): the two threads of a row swap their half-row maxima (and, at the
-    // end, their half-row sums) across a 64-thread named barrier (one per pair of warps).  A slot is rewritten two barriers later.
-    auto exchange = [&](float mine) -> float {
+    uint32_t slot = 0;                         // exchange-buffer parity, toggles at every swap
+    // One float per (slot, half, row): the two threads of a row swap their half-row maxima (and, at the end, their
+    // half-row sums) through shared memory.  The swap is split: post() publishes this thread's value and arrives on the
+    // row group's mbarrier (64 arrivals) without blocking - it is called as soon as the half-row max is known, in the
+    // middle of the tile's exponentials - and fetch() waits for the partner's arrival only when the value is needed,
+    // at the end of the pass, by when the partner has normally long arrived.  (A blocking 64-thread barrier here
+    // made the two warps of a row run in lock-step.)  Slots alternate; a slot is rewritten two swaps later, which the
+    // partner cannot reach before this thread's next arrival, i.e. after this thread has read the slot.
+    const uint32_t bx = bar_x + 8 * (warp & 3);
+    uint32_t xphase = 0;
+    auto post = [&](float mine) {
       st_shared_f32(sXch + ((slot * 2 + hh) * kTile + row_in_tile) * 4, mine);
-      tc_fence_before();
-      named_bar_sync(1 + (warp & 3), 64);  // only the two warps of this row group: pass counts differ between groups
-      tc_fence_after();
+      mbar_arrive(bx);
+    };
+    auto fetch = [&]() -> float {
+      mbar_wait(bx, xphase);
       const float other = ld_shared_f32(sXch + ((slot * 2 + (hh ^ 1)) * kTile + row_in_tile) * 4);
       slot ^= 1;
+      xphase ^= 1;
       return other;
     };
     for (int j = 0; j < n_kv; ++j) {
@@ -187,6 +199,7 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
             const uint64_t sl2_2 = pack2(sl2, sl2), neg_m2 = pack2(neg_m, neg_m);
             uint64_t la = pack2(0.f, 0.f), lb = pack2(0.f, 0.f);
             float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+            float mt_h = -INFINITY;
             tmem_ld32(tS + hh * 64, s[0]);
 #pragma unroll
             for (int c = 0; c < 2; ++c) {
@@ -199,9 +212,15 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
                   if (c * 32 + k >= n_valid_h) sc[k] = 0xff800000u;  // -inf
               }
 #pragma unroll
+              for (int k = 0; k < 16; ++k)
+                mx[k & 3] = fmaxf(mx[k & 3], fmaxf(__uint_as_float(sc[2 * k]), __uint_as_float(sc[2 * k + 1])));
+              if (c == 1) {  // half-row max known: publish it now, the exponentials of this chunk follow
+                mt_h = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3]));
+                post(mt_h);
+              }
+#pragma unroll
               for (int k = 0; k < 16; ++k) {
                 const float s0 = __uint_as_float(sc[2 * k]), s1 = __uint_as_float(sc[2 * k + 1]);
-                mx[k & 3] = fmaxf(mx[k & 3], fmaxf(s0, s1));
                 // x = s * scale * log2(e) - m_ref * scale * log2(e) for a pair of columns (one FFMA2)
                 const uint64_t x = fma2(pack2(s0, s1), sl2_2, neg_m2);
                 float p0, p1;
@@ -221,10 +240,8 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
             unpack2(la, l0, l1);
             unpack2(lb, l2, l3);
             l_tile = (l0 + l1) + (l2 + l3);
-            // Full-row tile max = max of the two halves.  The barrier also orders every tcgen05.ld of S_i
-            // (both halves) before any tcgen05.st of P_i, which overwrites columns [0, 64) of S_i.
-            const float mt_h = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3]));
-            mt = fmaxf(mt_h, exchange(mt_h));
+            // Full-row tile max = max of the two halves.
+            mt = fmaxf(mt_h, fetch());
             // exact unless the tile leads m_ref by more than 2^64 (or m_ref is still -inf); the decision is
             // the same in both warps of a row (same mt, same m_ref)
             if (pass == 1 || !__any_sync(0xffffffffu, !((mt - m_ref[i]) * sl2 <= 64.0f))) break;
@@ -244,9 +261,11 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
                 else if (col + 1 >= n_valid_h) pk[c][k] &= 0xffffu;
               }
           }
-          // P_i: bf16 pairs; this half's 64 keys are columns [32 hh, 32 hh + 32) of the S_i region
+          // P_i: bf16 pairs; this half's 64 keys go over the first 32 columns of the 64 score columns this same warp
+          // has read (columns [64 hh, 64 hh + 32) of the S_i region), so neither warp of a row ever overwrites
+          // scores its partner may still be loading and no barrier is needed between the loads and this store.
 #pragma unroll
-          for (int c = 0; c < 2; ++c) tmem_st16(tS + hh * 32 + c * 16, pk[c]);
+          for (int c = 0; c < 2; ++c) tmem_st16(tS + hh * 64 + c * 16, pk[c]);
           tmem_wait_st();
           tc_fence_before();
           mbar_arrive(bar_p_full + 8 * i);
@@ -260,7 +279,8 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
         const uint32_t tO = tO0 + i * D + lane_off + hh * (D / 2);
         mbar_wait(bar_o_full + 8 * i, 0);
         tc_fence_after();
-        const float l_row = l[i] + exchange(l[i]);
+        post(l[i]);
+        const float l_row = l[i] + fetch();
         const int row = i * kTile + row_in_tile;
         const bool valid = row < item.q_rows;
         const int n_tok = q_is_ref ? p.n_ref : p.n_gen;
@@ -352,7 +372,7 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
         const uint32_t v = v_lo + stage * kStageStep;
 #pragma unroll
         for (int kk = 0; kk < kTile / 16; ++kk)
-          umma_ts(tO0 + i * D, tS0 + i * 128 + kk * 8, desc64(v + kk * (2048 >> 4), kDescHi), idesc_pv,
+          umma_ts(tO0 + i * D, tS0 + i * 128 + (kk / 4) * 64 + (kk % 4) * 8, desc64(v + kk * (2048 >> 4), kDescHi), idesc_pv,
                   (acc || kk > 0) ? 1u : 0u);
       };
       auto stage_of = [&](int it) { return it % C::kStages; };
