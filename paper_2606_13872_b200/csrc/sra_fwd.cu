@@ -99,10 +99,10 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
     }
     for (int i = 0; i < 2; ++i) {
       mbar_init(bar_s_full + 8 * i, 1);
-      mbar_init(bar_p_full + 8 * i, 256);
+      mbar_init(bar_p_full + 8 * i, 8);  // one elected arrive per softmax warp
       mbar_init(bar_o_full + 8 * i, 1);
     }
-    for (int g = 0; g < 4; ++g) mbar_init(bar_x + 8 * g, 64);
+    for (int g = 0; g < 4; ++g) mbar_init(bar_x + 8 * g, 2);  // one elected arrive per warp of the pair
     fence_mbar_init();
   }
   if (warp == 9 && lane == 0) {
@@ -152,7 +152,8 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
     uint32_t xphase = 0;
     auto post = [&](float mine) {
       st_shared_f32(sXch + ((slot * 2 + hh) * kTile + row_in_tile) * 4, mine);
-      mbar_arrive(bx);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bx);
     };
     auto fetch = [&]() -> float {
       mbar_wait(bx, xphase);
@@ -268,7 +269,8 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
           for (int c = 0; c < 2; ++c) tmem_st16(tS + hh * 64 + c * 16, pk[c]);
           tmem_wait_st();
           tc_fence_before();
-          mbar_arrive(bar_p_full + 8 * i);
+          __syncwarp();
+          if (lane == 0) mbar_arrive(bar_p_full + 8 * i);
         }
       }
     }
