@@ -50,6 +50,29 @@ def log(*a):
     print(*a, file=sys.stderr, flush=True)
 
 
+_RESULT_FD = None
+
+
+def claim_stdout():
+    """The contract is ONE JSON line on stdout.  Native libraries print there too (NCCL's version banner at the first
+    communicator), so the real stdout is set aside for the result line and fd 1 is pointed at stderr for everything
+    else."""
+    global _RESULT_FD
+    if _RESULT_FD is None:
+        sys.stdout.flush()
+        _RESULT_FD = os.dup(1)
+        os.dup2(2, 1)
+
+
+def emit(out):
+    line = (json.dumps(out) + "\n").encode()
+    if _RESULT_FD is None:
+        sys.stdout.write(line.decode())
+        sys.stdout.flush()
+    else:
+        os.write(_RESULT_FD, line)
+
+
 def load_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -207,7 +230,7 @@ def bench_reference(args, w):
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
-    print(json.dumps(out), flush=True)
+    emit(out)
 
 
 def config_of(w, args, extra=None):
@@ -432,7 +455,7 @@ def bench_ours(args, w):
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
         "cpu_baseline": cpu_baseline, "parity": parity,
     }
-    print(json.dumps(out), flush=True)
+    emit(out)
     if world > 1:
         dist.destroy_process_group()
 
@@ -547,7 +570,7 @@ def bench_train(args, w):
         "e2e": None, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": None,
         "parity": parity,
     }
-    print(json.dumps(out), flush=True)
+    emit(out)
     if world > 1:
         dist.destroy_process_group()
 
@@ -674,7 +697,7 @@ def bench_short(args, w):
                      "algorithmic_bytes_per_launch": alg_bytes, "traffic": None},
         "cpu_baseline": None, "parity": None,
     }
-    print(json.dumps(out), flush=True)
+    emit(out)
 
 
 def bench_rope(args, w):
@@ -748,7 +771,7 @@ def bench_rope(args, w):
         "fused_over_unfused_time": med["fused"] / med["unfused"],
         "cpu_baseline": None, "parity": None,
     }
-    print(json.dumps(out), flush=True)
+    emit(out)
 
 
 def bench_ulysses(args, w):
@@ -856,7 +879,7 @@ def bench_ulysses(args, w):
                      "algorithmic_flops_per_launch": fl / world / u.n_chunks, "traffic": None},
         "cpu_baseline": None, "parity": None,
     }
-    print(json.dumps(out), flush=True)
+    emit(out)
 
 
 def bench_sweep(args):
@@ -907,7 +930,7 @@ def bench_sweep(args):
                    "useful_flop_ratio_40_over_5": pts[-1]["useful_tflop"] / pts[0]["useful_tflop"],
                    "dense_concat_ratio_40_over_5": float(((32760 + x[-1]) / (32760 + x[0])) ** 2)},
            "points": pts, "peak_sustained_tflops": peaks["bf16_tflops_sustained"], "peak_kind": peaks_kind}
-    print(json.dumps(out), flush=True)
+    emit(out)
 
 
 def main():
@@ -931,6 +954,7 @@ def main():
     ap.add_argument("--invalid-frac", type=float, default=0.0,
                     help="--mode fwd: fraction of reference tokens marked invalid (sparse validity masking, PAPER.md:225)")
     args = ap.parse_args()
+    claim_stdout()
     if args.warmup < 3 and args.impl == "ours":
         log("note: W < 3 warm-up steps breaks the timing rules; use --warmup >= 3 for a reportable number")
     from paper_2606_13872_b200 import inputs as I
