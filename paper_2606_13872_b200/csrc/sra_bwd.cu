@@ -284,7 +284,7 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
       for (int x = 0; x < 2; ++x)
 #pragma unroll
         for (int c = 0; c < 32; ++c)
-          if (x * 32 + c < qt.valid) red_add_f32(dq_row + (x * 32 + c) * D, __uint_as_float(r[x][c]));
+          if (drow < D && x * 32 + c < qt.valid) red_add_f32(dq_row + (x * 32 + c) * D, __uint_as_float(r[x][c]));
     }
     // ---------------------------------------------------- epilogue: dK = scale * acc (lanes = keys)
     mbar_wait(bar_acc_full, 0);
@@ -351,7 +351,10 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
       // ================================================= MMA issuer
       constexpr uint32_t idesc_st = make_idesc_bf16(kTile, QT, 0, 0);   // S^T, dP^T : [128 x 64], K = d
       constexpr uint32_t idesc_acc = make_idesc_bf16(kTile, D, 0, 1);   // dV, dK    : [128 x D],  K = 64 queries
-      constexpr uint32_t idesc_dq = make_idesc_bf16(D, QT, 1, 1);       // dQ^T      : [D x 64],    K = 128 keys
+      // dQ^T : [D x 64], K = 128 keys.  With D = 64 the MMA is still issued with M = 128 (the M = 64 accumulator layout
+      // differs): its A operand then runs on from the K tile into the V tile behind it, TMEM lanes [64, 128) receive
+      // finite garbage (V^T dS^T) and the drain ignores them.
+      constexpr uint32_t idesc_dq = make_idesc_bf16(kTile, QT, 1, 1);
       const uint32_t tS0 = tmem + C::kColS, tDP0 = tmem + C::kColDP;
       const uint32_t tDV = tmem + C::kColDV, tDK = tmem + C::kColDK;
       // Descriptor low words (start address, LBO); stepping along K or to another stage is one 32-bit add.
@@ -522,6 +525,7 @@ cudaError_t launch_bwd(const CUtensorMap* m, const BwdParams& p, cudaStream_t st
   return cudaGetLastError();
 }
 
+template cudaError_t launch_bwd<64>(const CUtensorMap*, const BwdParams&, cudaStream_t);
 template cudaError_t launch_bwd<128>(const CUtensorMap*, const BwdParams&, cudaStream_t);
 
 // ------------------------------------------------------------------------------------------------ host driver
@@ -530,7 +534,6 @@ static int run_backward_core(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t s
 int run_backward(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t stream) {
   const sra_config& c = ctx->cfg;
   const int B = c.batch, H = c.heads, d = c.head_dim;
-  if (d != 128) return ctx_fail(ctx, SRA_ERR_UNSUPPORTED, "sra_backward: head_dim 128 only (head_dim 64 is forward-only)");
   if (!a->q_gen || !a->k_gen || !a->v_gen || !a->o_gen || !a->lse_gen || !a->do_gen || !a->dq_gen || !a->dk_gen || !a->dv_gen)
     return ctx_fail(ctx, SRA_ERR_INVALID_ARG, "sra_backward: generation tensors (q,k,v,o,lse,do,dq,dk,dv) are required");
   const bool has_ref = c.n_ref > 0;
@@ -598,10 +601,13 @@ static int run_backward_core(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t s
     const int threads = 256;
     const int blocks = int(std::min<size_t>((rows * 32 + threads - 1) / threads, size_t(148) * 32));
     KernelTimer kt(ctx, SRA_KERNEL_BWD_PREPROCESS, stream);
-    sra_bwd_preprocess_kernel<128><<<blocks, threads, 0, stream>>>(
-        static_cast<const __nv_bfloat16*>(a->o_gen), static_cast<const __nv_bfloat16*>(a->do_gen), a->lse_gen,
-        static_cast<const __nv_bfloat16*>(a->o_ref), static_cast<const __nv_bfloat16*>(a->do_ref), a->lse_ref,
-        ctx->ws_delta, ctx->ws_lse2, B, H, c.n_gen, nr, n_pad);
+    auto launch = [&](auto kernel) {
+      kernel<<<blocks, threads, 0, stream>>>(
+          static_cast<const __nv_bfloat16*>(a->o_gen), static_cast<const __nv_bfloat16*>(a->do_gen), a->lse_gen,
+          static_cast<const __nv_bfloat16*>(a->o_ref), static_cast<const __nv_bfloat16*>(a->do_ref), a->lse_ref,
+          ctx->ws_delta, ctx->ws_lse2, B, H, c.n_gen, nr, n_pad);
+    };
+    if (d == 128) launch(sra_bwd_preprocess_kernel<128>); else launch(sra_bwd_preprocess_kernel<64>);
     if ((e = cudaGetLastError()) != cudaSuccess) return ctx_fail_cuda(ctx, e, "bwd preprocess launch");
     ctx->launches += 1;
   }
@@ -634,7 +640,7 @@ static int run_backward_core(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t s
   p.ref_kv_head_major = use_cache ? 1 : 0;
   {
     KernelTimer kt(ctx, SRA_KERNEL_BWD_MAIN, stream);
-    e = launch_bwd<128>(m, p, stream);
+    e = d == 128 ? launch_bwd<128>(m, p, stream) : launch_bwd<64>(m, p, stream);
   }
   if (e != cudaSuccess) return ctx_fail_cuda(ctx, e, "sra_bwd_kernel launch");
   ctx->launches += 1;
@@ -644,9 +650,11 @@ static int run_backward_core(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t s
     const int threads = 256;
     const int blocks = int(std::min<size_t>((total + threads - 1) / threads, size_t(148) * 32));
     KernelTimer kt(ctx, SRA_KERNEL_BWD_DQ_FINALIZE, stream);
-    sra_bwd_dq_finalize_kernel<128><<<blocks, threads, 0, stream>>>(ctx->ws_dq, static_cast<__nv_bfloat16*>(a->dq_gen),
-                                                                   static_cast<__nv_bfloat16*>(a->dq_ref), B, H, c.n_gen,
-                                                                   nr, n_pad, ctx->scale);
+    auto launch = [&](auto kernel) {
+      kernel<<<blocks, threads, 0, stream>>>(ctx->ws_dq, static_cast<__nv_bfloat16*>(a->dq_gen),
+                                             static_cast<__nv_bfloat16*>(a->dq_ref), B, H, c.n_gen, nr, n_pad, ctx->scale);
+    };
+    if (d == 128) launch(sra_bwd_dq_finalize_kernel<128>); else launch(sra_bwd_dq_finalize_kernel<64>);
     if ((e = cudaGetLastError()) != cudaSuccess) return ctx_fail_cuda(ctx, e, "dQ finalize launch");
     ctx->launches += 1;
   }
