@@ -149,6 +149,7 @@ class UlyssesSRA:
                     for _, cc in self.chunk_heads]
         self.comm = torch.cuda.Stream()
         self.launches = 0
+        self.saved = None
 
     def close(self) -> None:
         for c in self.ctx:
@@ -175,11 +176,15 @@ class UlyssesSRA:
         torch.cuda.current_stream().synchronize()  # the head-major copies have consumed the temporaries
 
     def forward(self, q_gen: torch.Tensor, k_gen: torch.Tensor, v_gen: torch.Tensor,
-                q_ref: Optional[torch.Tensor] = None):
+                q_ref: Optional[torch.Tensor] = None, save_for_backward: bool = False):
         """One attention layer on sequence shards ([B, n_local, H, d] each; q_ref = this rank's reference shard on
         step 0 / training, None on cached denoising steps).  Returns (o_gen, o_ref or None) as sequence shards.
-        Requires `cache_reference_kv` when n_ref > 0."""
+        Requires `cache_reference_kv` when n_ref > 0.  `save_for_backward` keeps the head-sharded tensors and the LSE
+        of every chunk for `backward` (training: PAPER.md:173, :231)."""
         B = self.B
+        if save_for_backward and self.n_ref > 0 and q_ref is None:
+            raise ValueError("training needs the reference rows (q_ref)")
+        self.saved = [None] * self.n_chunks if save_for_backward else None
         cur = torch.cuda.current_stream()
         comm = self.comm
         o_gen = torch.empty_like(q_gen)
@@ -207,9 +212,15 @@ class UlyssesSRA:
             cur.wait_event(ev)
             oh = torch.empty_like(qh)
             orh = torch.empty_like(qrh) if qrh is not None else None
+            lg = lr = None
+            if save_for_backward:
+                lg = torch.empty((self.batch, qh.shape[2], self.n_gen), device=qh.device, dtype=torch.float32)
+                lr = torch.empty((self.batch, qh.shape[2], self.n_ref), device=qh.device, dtype=torch.float32) if qrh is not None else None
             if self.ctx[c]:  # (an empty chunk only relays its tokens)
-                B.sra_forward(self.ctx[c], qh, kh, vh, oh, q_ref=qrh, o_ref=orh)
+                B.sra_forward(self.ctx[c], qh, kh, vh, oh, q_ref=qrh, o_ref=orh, lse_gen=lg, lse_ref=lr)
                 self.launches += 1
+            if save_for_backward:
+                self.saved[c] = (qh, kh, vh, qrh, oh, orh, lg, lr)
             done = torch.cuda.Event()
             done.record(cur)
             with torch.cuda.stream(comm):
@@ -225,3 +236,60 @@ class UlyssesSRA:
                     x.record_stream(cur)
                     x.record_stream(comm)
         return o_gen, o_ref
+
+    def backward(self, do_gen: torch.Tensor, do_ref: Optional[torch.Tensor] = None):
+        """Gradients of the last `forward(..., save_for_backward=True)`.  do_gen / do_ref: this rank's sequence shards of
+        the upstream gradient.  Returns (dq_gen, dk_gen, dv_gen, dq_ref, dk_ref, dv_ref) as sequence shards (the last
+        three None when n_ref == 0).  Reference K/V come from the resident caches, their gradients are returned like
+        everything else.  Same pipeline as forward: the exchange of chunk c + 1's dO and the return of chunk c - 1's
+        gradients run on the communication stream underneath `sra_backward` of chunk c."""
+        if getattr(self, "saved", None) is None:
+            raise RuntimeError("backward() needs forward(..., save_for_backward=True) first")
+        B = self.B
+        has_ref = self.n_ref > 0
+        if has_ref and do_ref is None:
+            raise ValueError("do_ref is required when n_ref > 0")
+        cur = torch.cuda.current_stream()
+        comm = self.comm
+        outs_seq = [torch.empty_like(do_gen) for _ in range(3)] + ([torch.empty_like(do_ref) for _ in range(3)] if has_ref else [None] * 3)
+        comm.wait_stream(cur)
+        staged: List[Optional[tuple]] = [None] * self.n_chunks
+
+        def stage(c):
+            with torch.cuda.stream(comm):
+                t = (self._to_heads(do_gen, self.n_gen, c), self._to_heads(do_ref, self.n_ref, c) if has_ref else None)
+                ev = torch.cuda.Event()
+                ev.record(comm)
+            staged[c] = (t, ev)
+
+        keep = []
+        stage(0)
+        for c in range(self.n_chunks):
+            if c + 1 < self.n_chunks:
+                stage(c + 1)
+            (dog, dor), ev = staged[c]
+            cur.wait_event(ev)
+            qh, kh, vh, qrh, oh, orh, lg, lr = self.saved[c]
+            g = [torch.empty_like(qh) for _ in range(3)] + ([torch.empty_like(qrh) for _ in range(3)] if has_ref else [None] * 3)
+            if self.ctx[c]:
+                B.sra_backward(self.ctx[c], q_gen=qh, k_gen=kh, v_gen=vh, q_ref=qrh, k_ref=None, v_ref=None, o_gen=oh,
+                               o_ref=orh, lse_gen=lg, lse_ref=lr, do_gen=dog, do_ref=dor, dq_gen=g[0], dk_gen=g[1],
+                               dv_gen=g[2], dq_ref=g[3], dk_ref=g[4], dv_ref=g[5])
+                self.launches += 3
+            done = torch.cuda.Event()
+            done.record(cur)
+            with torch.cuda.stream(comm):
+                comm.wait_event(done)
+                for k in range(3):
+                    heads_to_seq(g[k], self.n_gen, self.heads, outs_seq[k], self.group, self.n_chunks, c)
+                    if has_ref:
+                        heads_to_seq(g[3 + k], self.n_ref, self.heads, outs_seq[3 + k], self.group, self.n_chunks, c)
+            keep.append((dog, dor, *g))
+        cur.wait_stream(comm)
+        for t in keep:
+            for x in t:
+                if x is not None:
+                    x.record_stream(cur)
+                    x.record_stream(comm)
+        self.saved = None
+        return tuple(outs_seq)
