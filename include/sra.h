@@ -128,8 +128,9 @@ typedef struct {
  * the outputs.  The results are valid after the caller synchronises the stream.  Requires the
  * resident cache when n_ref > 0 (SRA_ERR_NO_REF_CACHE otherwise).
  * With batch == 1 and at least 16 query slabs the step is pipelined: the generation rows go in 8 slabs whose
- * host->device and device->host copies run on two ctx-owned copy streams underneath the forward launches of the
- * neighbouring slabs (query slabs are independent work items), reference rows before the last two slabs.  The one
+ * host->device and device->host copies run on two ctx-owned copy streams underneath the forward launches of other
+ * slabs (query slabs are independent work items; launches cover several slabs where the copies allow), reference
+ * rows before the last slab.  The one
  * transfer every generation row needs, K_g and V_g, is hidden by "reference keys first": the first slabs (up to 6,
  * enough to cover the upload) attend the resident reference K/V while K_g / V_g are in flight, then the generation
  * keys, and the two fp32 partials (O_s, LSE_s) of each row are merged exactly as in the key-split schedule - so

@@ -672,7 +672,7 @@ static int forward_core(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) 
 // are uploaded ahead of K_g / V_g and attend the REFERENCE segment only while K_g / V_g are in flight (A items, fp32
 // partials); once K_g / V_g have landed they attend the generation segment (B items) and the two partials of every
 // row are merged by sra_fwd_merge_kernel (the key-split machinery of the short-query regime).  The remaining
-// slabs run the ordinary single-pass items.  The reference rows go in before the last two slabs.  Everything is
+// slabs run the ordinary single-pass items.  The reference rows go in before the last slab; launches cover several slabs where the copies allow.  Everything is
 // ordered after prior work on `st`, and `st` is made to wait for the last D2H copy, so the call stays asynchronous
 // on the caller's stream.
 static int forward_host_pipelined(sra_ctx* ctx, const sra_fwd_host_args* a, cudaStream_t st, bool with_ref_rows) {
@@ -764,19 +764,36 @@ static int forward_host_pipelined(sra_ctx* ctx, const sra_fwd_host_args* a, cuda
     ctx->sub_items = nullptr; ctx->sub_count = -1;
     return rc;
   };
-  // phase 1: reference segment of the first slabs, under the K_g / V_g upload
-  for (int ch = 0; ch < n_first; ++ch) {
+  // Launches are grouped over several slabs wherever the copies allow it: every kernel boundary drains the GPU
+  // through a partially filled last wave (~0.6 ms at 720p), so fewer, larger launches.
+  auto span = [&](int c0, int c1, int& i0, int& i1, size_t& r0, size_t& r1) {  // slabs [c0, c1)
+    int x; size_t y;
+    rows_of(c0, i0, x, r0, y);
+    rows_of(c1 - 1, x, i1, y, r1);
+  };
+  auto copy_out = [&](int c0, int c1) {  // rows of slabs [c0, c1) are final in the staging buffer: send them home
     int i0, i1; size_t r0, r1;
-    rows_of(ch, i0, i1, r0, r1);
-    e = cudaStreamWaitEvent(st, ev_q[ch], 0);
-    if (e != cudaSuccess) return fail_cuda(ctx, e, "pipelined host copy");
+    span(c0, c1, i0, i1, r0, r1);
+    if (e == cudaSuccess) e = cudaEventRecord(ev_c[c0], st);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->s_d2h, ev_c[c0], 0);
+    if (e == cudaSuccess && r1 > r0) e = cudaMemcpyAsync(hout + r0 * row, dout + r0 * row, (r1 - r0) * row, cudaMemcpyDeviceToHost, ctx->s_d2h);
+  };
+  // phase 1: reference segment of the first slabs, under the K_g / V_g upload (slab 0 as soon as it has landed, the
+  // others together: their copies are long done when slab 0's launch ends)
+  for (int g = 0; g < 2 && e == cudaSuccess; ++g) {
+    const int c0 = g == 0 ? 0 : 1, c1 = g == 0 ? std::min(1, n_first) : n_first;
+    if (c1 <= c0) continue;
+    int i0, i1; size_t r0, r1;
+    span(c0, c1, i0, i1, r0, r1);
+    e = cudaStreamWaitEvent(st, ev_q[c1 - 1], 0);
+    if (e != cudaSuccess) break;
     if (int rc = launch(ctx->d_seg_items, i0, i1 - i0, d)) return rc;
   }
-  e = cudaStreamWaitEvent(st, ev_kv, 0);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev_kv, 0);
   if (e != cudaSuccess) return fail_cuda(ctx, e, "pipelined host copy");
   auto run_ref_rows = [&]() -> int {
     // reference rows: their q_ref copy has had the first slabs' compute time to land; their output copy is
-    // hidden under the remaining slabs
+    // hidden under the last slab
     cudaError_t er = cudaStreamWaitEvent(st, ev_qr, 0);
     if (er != cudaSuccess) return fail_cuda(ctx, er, "pipelined host copy");
     sra_fwd_args dr = d;
@@ -789,33 +806,40 @@ static int forward_host_pipelined(sra_ctx* ctx, const sra_fwd_host_args* a, cuda
     if (er == cudaSuccess && dr.lse_ref) er = cudaMemcpyAsync(a->lse_ref, dr.lse_ref, size_t(c.heads) * c.n_ref * 4, cudaMemcpyDeviceToHost, ctx->s_d2h);
     return er == cudaSuccess ? SRA_OK : fail_cuda(ctx, er, "pipelined host copy");
   };
-  // phase 2: generation segment + merge of the first slabs, then the ordinary slabs
-  for (int ch = 0; ch < kChunks; ++ch) {
+  // phase 2: generation segment of the first slabs in one launch, one merge of their partials
+  if (n_first > 0) {
     int i0, i1; size_t r0, r1;
-    rows_of(ch, i0, i1, r0, r1);
-    if (with_ref_rows && ch == kChunks - 2)
-      if (int rc = run_ref_rows()) return rc;
-    if (ch < n_first) {
-      if (int rc = launch(ctx->d_seg_items, G + i0, i1 - i0, d)) return rc;
-      sra::FwdParams mp{};
-      mp.part_o = ctx->ws_seg_o; mp.part_lse = ctx->ws_seg_lse;
-      mp.o_gen = static_cast<__nv_bfloat16*>(d.o_gen); mp.lse_gen = d.lse_gen;
-      mp.batch = 1; mp.heads = c.heads; mp.n_gen = c.n_gen;
-      {
-        sra::KernelTimer kt(ctx, SRA_KERNEL_FWD_MERGE, st);
-        e = sra::launch_fwd_merge(mp, c.head_dim, 2, st, int(r0), int(r1 - r0));
-      }
-      if (e != cudaSuccess) return fail_cuda(ctx, e, "sra_fwd_merge_kernel launch");
-      if (i1 > i0) ctx->launches += 1;
-    } else {
-      e = cudaStreamWaitEvent(st, ev_q[ch], 0);
+    span(0, n_first, i0, i1, r0, r1);
+    if (int rc = launch(ctx->d_seg_items, G + i0, i1 - i0, d)) return rc;
+    sra::FwdParams mp{};
+    mp.part_o = ctx->ws_seg_o; mp.part_lse = ctx->ws_seg_lse;
+    mp.o_gen = static_cast<__nv_bfloat16*>(d.o_gen); mp.lse_gen = d.lse_gen;
+    mp.batch = 1; mp.heads = c.heads; mp.n_gen = c.n_gen;
+    {
+      sra::KernelTimer kt(ctx, SRA_KERNEL_FWD_MERGE, st);
+      e = sra::launch_fwd_merge(mp, c.head_dim, 2, st, int(r0), int(r1 - r0));
+    }
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "sra_fwd_merge_kernel launch");
+    if (r1 > r0) ctx->launches += 1;
+    copy_out(0, n_first);
+  }
+  // phase 3: the ordinary slabs - all but the last in one launch (without a reference-first phase slab 0 goes alone,
+  // as soon as it has landed), the reference rows, then the last slab, under which the other outputs go home
+  {
+    const int mid0 = n_first > 0 ? n_first : 1;
+    const int groups[3][2] = {{n_first, n_first > 0 ? n_first : 1}, {mid0, kChunks - 1}, {kChunks - 1, kChunks}};
+    for (int g = 0; g < 3 && e == cudaSuccess; ++g) {
+      const int c0 = groups[g][0], c1 = groups[g][1];
+      if (g == 2 && with_ref_rows)
+        if (int rc = run_ref_rows()) return rc;
+      if (c1 <= c0) continue;
+      int i0, i1; size_t r0, r1;
+      span(c0, c1, i0, i1, r0, r1);
+      e = cudaStreamWaitEvent(st, ev_q[c1 - 1], 0);
       if (e != cudaSuccess) break;
       if (int rc = launch(nullptr, i0, i1 - i0, d)) return rc;
+      copy_out(c0, c1);
     }
-    e = cudaEventRecord(ev_c[ch], st);
-    if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->s_d2h, ev_c[ch], 0);
-    if (e == cudaSuccess && i1 > i0) e = cudaMemcpyAsync(hout + r0 * row, dout + r0 * row, (r1 - r0) * row, cudaMemcpyDeviceToHost, ctx->s_d2h);
-    if (e != cudaSuccess) break;
   }
   if (e == cudaSuccess && d.lse_gen)
     e = cudaMemcpyAsync(a->lse_gen, d.lse_gen, size_t(c.heads) * c.n_gen * 4, cudaMemcpyDeviceToHost, ctx->s_d2h);
