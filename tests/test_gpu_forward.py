@@ -211,3 +211,15 @@ def test_forward_host_matches_device_path(name):
         check_gen(o_gen, lse_gen)
     finally:
         B.sra_destroy(ctx)
+
+
+@pytest.mark.parametrize("name", ["short_mini", "ragged"])
+def test_optional_lse_outputs_do_not_change_o(name):
+    """lse_gen / lse_ref are nullable (include/sra.h): leaving them out must not change a byte of O, on the single-pass
+    schedule and on the key-split schedule (whose merge kernel also writes the LSE)."""
+    w = sra_inputs.WORKLOADS[name]
+    t = sra_inputs.make_inputs(w)
+    a = run_gpu_forward(w, t, use_cache=True, want_lse=True)
+    b = run_gpu_forward(w, t, use_cache=True, want_lse=False)
+    assert np.array_equal(a["o_gen"], b["o_gen"]) and np.array_equal(a["o_ref"], b["o_ref"])
+    assert "lse_gen" not in b
