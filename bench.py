@@ -766,7 +766,8 @@ def bench_rope(args, w):
         "roofline": {"bound": "hbm", "kernel": "relayout_rope_head_major_kernel", "achieved": gbs["fused"],
                      "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": gbs["fused"] / peaks["hbm_gbs"],
                      "peak_kind": f"{peaks_kind} copy bandwidth", "kernel_ms": med["fused"],
-                     "algorithmic_bytes_per_launch": alg["fused"], "traffic": None},
+                     "algorithmic_bytes_per_launch": alg["fused"],
+                     "traffic": (load_traffic_all().get(w.name, {}) or {}).get("relayout_rope_head_major_kernel_dram_bytes")},
         "rope": {k: {"ms": med[k], "algorithmic_bytes": alg[k], "gbs": gbs[k]} for k in med},
         "fused_over_unfused_time": med["fused"] / med["unfused"],
         "cpu_baseline": None, "parity": None,
