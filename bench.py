@@ -694,7 +694,9 @@ def bench_short(args, w):
         "roofline": {"bound": "hbm", "kernel": "sra_fwd_kernel<128>" + (" + sra_fwd_merge_kernel<128>" if n_split > 1 else ""),
                      "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
                      "peak_kind": f"{peaks_kind} copy bandwidth", "kernel_ms": kernel_ms,
-                     "algorithmic_bytes_per_launch": alg_bytes, "traffic": None},
+                     "algorithmic_bytes_per_launch": alg_bytes,
+                     "traffic": (lambda t: (t.get("sra_fwd_kernel_dram_bytes", 0) + t.get("sra_fwd_merge_kernel_dram_bytes", 0)) or None)(
+                         load_traffic_all().get(w.name, {}) or {})},
         "cpu_baseline": None, "parity": None,
     }
     emit(out)
