@@ -23,6 +23,8 @@ section 8f #1): with an optional per-reference-token flag valid[t],
     M[i][j] = 0 if j in R and not valid[j]     (an invalid token is nobody's key)
     M[i][:] = 0 if i in R and not valid[i]     (an invalid token's own row is empty)
     a row with no visible key has O = 0, P = 0, LSE = -inf (the convention of reading A8).
+Per-sample masks (reading A12; "validity masks are precomputed per-rank"): `valid` of shape
+[B, n_ref] gives batch item b its own mask valid[b] - each item is the problem above with its own flags.
 
 Sparse temporal attention of the SR refiner ("restricts each frame's receptive field to a local
 neighborhood"; no window size or mask is given - reading A17 of DESIGN.md): with generation frame offsets fr[] and a
@@ -145,6 +147,14 @@ def _concat_head(x_gen, x_ref, b, h):
     return np.concatenate(parts, axis=0)
 
 
+def _valid_of(valid, b):
+    """Mask of batch item b: `valid` is None, [n_ref] (shared by the batch) or [B, n_ref] (per sample, A12)."""
+    if valid is None:
+        return None
+    v = np.asarray(valid)
+    return v[b] if v.ndim == 2 else v
+
+
 def sra_forward(q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, ref_block_offsets, scale, valid=None,
                 gen_frame_offsets=None, window=-1):
     """SRA forward on bf16-bit inputs [B, N, H, d].
@@ -159,10 +169,10 @@ def sra_forward(q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, ref_block_offsets, sca
     Nr = kr.shape[1]
     have_qr = q_ref is not None
     qr = f(q_ref) if have_qr else np.zeros((B, Nr, H, d))
-    M = sra_mask(Ng, ref_block_offsets, valid, gen_frame_offsets, window)
     o = np.zeros((B, Ng + Nr, H, d))
     lse = np.zeros((B, H, Ng + Nr))
     for b in range(B):
+        M = sra_mask(Ng, ref_block_offsets, _valid_of(valid, b), gen_frame_offsets, window)
         for h in range(H):
             Q = _concat_head(qg, qr, b, h)
             K = _concat_head(kg, kr, b, h)
@@ -185,11 +195,11 @@ def sra_backward(q_gen, k_gen, v_gen, q_ref, k_ref, v_ref, do_gen, do_ref, ref_b
     dog, dor = f(do_gen), f(do_ref)
     B, Ng, H, d = qg.shape
     Nr = kr.shape[1]
-    M = sra_mask(Ng, ref_block_offsets, valid, gen_frame_offsets, window)
     dq = np.zeros((B, Ng + Nr, H, d))
     dk = np.zeros_like(dq)
     dv = np.zeros_like(dq)
     for b in range(B):
+        M = sra_mask(Ng, ref_block_offsets, _valid_of(valid, b), gen_frame_offsets, window)
         for h in range(H):
             Q = _concat_head(qg, qr, b, h)
             K = _concat_head(kg, kr, b, h)

@@ -534,6 +534,138 @@ def test_temporal_window_mask_and_gradients(seed, frames, blocks, w):
             np.testing.assert_allclose(fwd["o_gen"][0, sl].transpose(1, 0, 2), of.numpy(), rtol=0, atol=1e-12)
 
 
+# ------------------------------------------------------------------ per-sample validity (reading A12)
+@pytest.mark.parametrize("seed,Ng,blocks", [(3, 6, (4, 7, 2)), (4, 2, (5,))])
+def test_per_sample_validity_equals_per_item_deletion(seed, Ng, blocks):
+    """valid of shape [B, n_ref]: batch item b must equal the UNMASKED oracle run on item b alone with ITS invalid
+    tokens physically deleted (forward, LSE and all six gradients) - numpy oracle and C oracle (every row / column)."""
+    rng = np.random.default_rng(seed)
+    off = [0]
+    for b in blocks:
+        off.append(off[-1] + b)
+    Nr, B, H, d = off[-1], 3, 2, 8
+    t = {k: rand_bits(rng, (B, Ng if k.endswith("gen") else Nr, H, d)) for k in
+         ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref", "do_gen", "do_ref")}
+    valid = rng.random((B, Nr)) < 0.6
+    valid[0, :] = True                       # item 0: nothing masked
+    valid[1, off[0]:off[1]] = False          # item 1: its first block disappears
+    valid[np.arange(B), rng.integers(0, Nr, B)] |= ~valid.any(axis=1)  # never all-invalid here
+    assert not np.array_equal(valid[1], valid[2])
+    scale = 0.3
+    a6 = [t[k] for k in ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref")]
+    fm = sra_oracle.sra_forward(*a6, off, scale, valid=valid)
+    bm = sra_oracle.sra_backward(*a6, t["do_gen"], t["do_ref"], off, scale, valid=valid)
+    n = Ng + Nr
+    oc, lc = c_oracle.forward_rows(*a6, off, scale, np.arange(n, dtype=np.int32), valid=valid)
+    for b in range(B):
+        tb = {k: v[b:b + 1] for k, v in t.items()}
+        t2, off2, keep = _delete_invalid(tb, off, valid[b])
+        b6 = [t2[k] for k in ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref")]
+        fd = sra_oracle.sra_forward(*b6, off2, scale)
+        bd = sra_oracle.sra_backward(*b6, t2["do_gen"], t2["do_ref"], off2, scale)
+        inv = np.flatnonzero(~valid[b])
+        np.testing.assert_allclose(fm["o_gen"][b], fd["o_gen"][0], rtol=0, atol=1e-13)
+        np.testing.assert_allclose(fm["o_ref"][b][keep], fd["o_ref"][0], rtol=0, atol=1e-13)
+        np.testing.assert_allclose(fm["lse_ref"][b][:, keep], fd["lse_ref"][0], rtol=0, atol=1e-13)
+        assert np.all(fm["o_ref"][b][inv] == 0.0) and np.all(np.isneginf(fm["lse_ref"][b][:, inv]))
+        # C oracle, all rows of item b
+        np.testing.assert_allclose(oc[b, :Ng], fd["o_gen"][0], rtol=0, atol=1e-13)
+        np.testing.assert_allclose(oc[b, Ng:][keep], fd["o_ref"][0], rtol=0, atol=1e-13)
+        np.testing.assert_allclose(lc[b][:, :Ng], fd["lse_gen"][0], rtol=0, atol=1e-13)
+        assert np.all(oc[b, Ng:][inv] == 0.0) and np.all(np.isneginf(lc[b][:, Ng:][:, inv]))
+        for g in ("dq", "dk", "dv"):
+            np.testing.assert_allclose(bm[g + "_gen"][b], bd[g + "_gen"][0], rtol=0, atol=1e-12)
+            np.testing.assert_allclose(bm[g + "_ref"][b][keep], bd[g + "_ref"][0], rtol=0, atol=1e-12)
+            assert np.all(bm[g + "_ref"][b][inv] == 0.0)
+        for h in range(H):
+            o, lse = c_oracle.forward_head(*a6, off, scale, b, h, valid=valid)
+            dq, dk, dv = c_oracle.backward_head(*a6, t["do_gen"], t["do_ref"], off, scale, b, h, o, lse, valid=valid)
+            for name, got in (("dq", dq), ("dk", dk), ("dv", dv)):
+                np.testing.assert_allclose(got[:Ng], bd[name + "_gen"][0, :, h], rtol=0, atol=1e-12)
+                np.testing.assert_allclose(got[Ng:][keep], bd[name + "_ref"][0, :, h], rtol=0, atol=1e-12)
+                assert np.all(got[Ng:][inv] == 0.0)
+
+
+# ------------------------------------------------------------------ C oracle under valid[] and the frame window
+@pytest.mark.parametrize("seed,frames,blocks,w,use_valid", [(5, (3, 5, 2, 4), (3, 4, 6), 1, True), (6, (4, 4, 4), (5,), 0, False),
+                                                            (7, (2, 3, 1, 5, 2), (6, 2), 2, True), (8, (9,), (4, 3), -1, True)])
+def test_c_oracle_valid_and_window(seed, frames, blocks, w, use_valid):
+    """The C oracle's optional masks (PAPER.md:225 validity, PAPER.md:143 frame window), pinned three ways:
+    (1) every row of its forward equals torch fp64 SDPA under a boolean mask built HERE from first principles
+    (frame ids by searchsorted, block ids by repeat - not the oracle's lookup); (2) its backward (all rows, all
+    columns, and a sampled subset) equals torch autograd under that mask; (3) with a validity mask, the problem with the
+    invalid tokens physically deleted, solved by the unmasked C oracle, gives the same G rows and kept R rows;
+    (4) its pair count equals the mask's sum.  The numpy oracle must agree too."""
+    rng = np.random.default_rng(seed)
+    fr = np.concatenate([[0], np.cumsum(frames)]).astype(np.int32)
+    off = np.concatenate([[0], np.cumsum(blocks)]).astype(np.int32)
+    Ng, Nr, B, H, d = int(fr[-1]), int(off[-1]), 2, 2, 8
+    t = {k: rand_bits(rng, (B, Ng if k.endswith("gen") else Nr, H, d)) for k in
+         ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref", "do_gen", "do_ref")}
+    valid = None
+    if use_valid:
+        valid = rng.random(Nr) < 0.65
+        valid[off[0]:off[1]] = valid[off[0]:off[1]] | (np.arange(off[1]) == 0)   # keep one token of block 0
+        if len(blocks) > 1:
+            valid[off[1]:off[2]] = False                                            # block 1 disappears
+    # the mask from first principles
+    fid = np.searchsorted(fr, np.arange(Ng), side="right") - 1
+    bid = np.repeat(np.arange(len(blocks)), blocks)
+    n = Ng + Nr
+    M = np.zeros((n, n), dtype=bool)
+    M[:Ng, :Ng] = (np.abs(fid[:, None] - fid[None, :]) <= w) if w >= 0 else True
+    M[:Ng, Ng:] = True
+    M[Ng:, Ng:] = bid[:, None] == bid[None, :]
+    if valid is not None:
+        M[:, Ng:] &= valid[None, :]
+        M[Ng:, :] &= valid[:, None]
+    scale = 0.4
+    a6 = [t[k] for k in ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref")]
+    kw = dict(valid=valid, gen_frame_offsets=fr, window=w)
+    assert c_oracle.count_pairs(Ng, off, **kw) == int(M.sum())
+    oc, lc = c_oracle.forward_rows(*a6, off, scale, np.arange(n, dtype=np.int32), **kw)
+    on = sra_oracle.sra_forward(*a6, off, scale, **kw)
+    bn = sra_oracle.sra_backward(*a6, t["do_gen"], t["do_ref"], off, scale, **kw)
+    empty = ~M.any(axis=1)
+    for b in range(B):
+        cat = lambda g, r: torch.tensor(np.concatenate([bits_to_f64(t[g][b]), bits_to_f64(t[r][b])], axis=0).transpose(1, 0, 2))
+        q, k, v = (cat(x, y).requires_grad_(True) for x, y in (("q_gen", "q_ref"), ("k_gen", "k_ref"), ("v_gen", "v_ref")))
+        do = cat("do_gen", "do_ref")
+        # torch SDPA returns NaN for empty rows: give them one dummy visible key and zero their dO, then compare the rest
+        Mt = M.copy()
+        Mt[empty, 0] = True
+        do_t = do.clone()
+        do_t[:, empty] = 0.0
+        o = torch.nn.functional.scaled_dot_product_attention(q, k, v, attn_mask=torch.tensor(Mt), scale=scale)
+        o.backward(do_t)
+        want = o.detach().numpy().transpose(1, 0, 2)          # [n, H, d]
+        np.testing.assert_allclose(oc[b][~empty], want[~empty], rtol=0, atol=1e-12)
+        assert np.all(oc[b][empty] == 0.0) and np.all(np.isneginf(lc[b][:, empty]))
+        np.testing.assert_allclose(np.concatenate([on["o_gen"][b], on["o_ref"][b]]), oc[b], rtol=0, atol=1e-12)
+        for h in range(H):
+            oh, lh = c_oracle.forward_head(*a6, off, scale, b, h, **kw)
+            np.testing.assert_allclose(oh, oc[b][:, h], rtol=0, atol=1e-13)
+            dq, dk, dv = c_oracle.backward_head(*a6, t["do_gen"], t["do_ref"], off, scale, b, h, oh, lh, **kw)
+            for name, got, g in (("dq", dq, q.grad), ("dk", dk, k.grad), ("dv", dv, v.grad)):
+                ref = g.numpy()[h]
+                np.testing.assert_allclose(got, ref, rtol=0, atol=1e-11)
+                nb = np.concatenate([bn[name + "_gen"][b, :, h], bn[name + "_ref"][b, :, h]])
+                np.testing.assert_allclose(got, nb, rtol=0, atol=1e-11)
+            rows = np.array(sorted(rng.choice(n, size=min(5, n), replace=False)), dtype=np.int32)
+            cols = np.array(sorted(rng.choice(n, size=min(4, n), replace=False)), dtype=np.int32)
+            dq_s, dk_s, dv_s = c_oracle.backward_head(*a6, t["do_gen"], t["do_ref"], off, scale, b, h, oh, lh,
+                                                      rows=rows, cols=cols, **kw)
+            assert np.array_equal(dq_s, dq[rows]) and np.array_equal(dk_s, dk[cols]) and np.array_equal(dv_s, dv[cols])
+    if valid is not None:
+        t2, off2, keep = _delete_invalid(t, list(off), valid)
+        b6 = [t2[k] for k in ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref")]
+        n2 = Ng + len(keep)
+        od, ld = c_oracle.forward_rows(*b6, off2, scale, np.arange(n2, dtype=np.int32), gen_frame_offsets=fr, window=w)
+        np.testing.assert_allclose(oc[:, :Ng], od[:, :Ng], rtol=0, atol=1e-13)
+        np.testing.assert_allclose(oc[:, Ng:][:, keep], od[:, Ng:], rtol=0, atol=1e-13)
+        np.testing.assert_allclose(lc[:, :, Ng:][:, :, keep], ld[:, :, Ng:], rtol=0, atol=1e-13)
+
+
 # ----------------------------------------------------------------------------- RoPE producer (reading A18, PAPER.md:223)
 def _angles(N, half, rng=None, base=10000.0):
     """theta[t, i] = t * base^(-i / half): the 1-D RoFormer table, the structure the relative-position pin needs."""
