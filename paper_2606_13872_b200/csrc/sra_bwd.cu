@@ -1,59 +1,98 @@
 // SRA backward for sm_100a (PAPER.md:173 - SFT trains through SRA).
 //
 //   a6  sra_bwd_preprocess_kernel   D_i = sum_c dO_ic O_ic and LSE_i * log2(e), rows [G ; R] concatenated
-//   a7  sra_bwd_kernel<D>           one CTA = one 128-key tile x one (batch, head); it loops over the 64-row
+//   a7  sra_bwd_kernel<D>           one CTA = one 128-key tile x one (batch, head); it loops over the 128-row
 //                                   query tiles that may see the tile (all G queries; for a reference key tile
-//                                   also the R queries of its own block - the transposed SRA mask), 5 MMAs each:
-//         S^T  = K   Q_i^T      [keys x queries]   SS, -> TMEM S[i&1]
-//         dP^T = V   dO_i^T     [keys x queries]   SS, -> TMEM dP
-//         dV  += P^T dO_i       [keys x d]         A = P^T (bf16) from TMEM, aliasing S[i&1]
+//                                   also the R queries of its own block - the transposed SRA mask), 5 MMAs each,
+//                                   every one of them M = 128, N = 128 (full tensor rate):
+//         S^T  = K   Q_i^T      [keys x queries]   SS            -> TMEM S
+//         dP^T = V   dO_i^T     [keys x queries]   SS            -> TMEM dPdQ
+//         dV  += P^T dO_i       [keys x d]         A = P^T (bf16) from TMEM, written over S^T
+//         dQ_i^T = K^T dS^T     [d x queries]      A = K (MN-major), B = dS^T (MN-major) -> TMEM dPdQ (over dP^T)
 //         dK  += dS^T Q_i       [keys x d]         A = dS^T (bf16) from shared memory
-//         dQ_i^T = K^T dS^T     [d x queries]      A = K (MN-major), B = dS^T (MN-major), -> TMEM dQ
-//       with P^T = exp2(S^T * scale*log2e - LSE*log2e) formed by one warpgroup and dS^T = P^T o (dP^T - D) by a
-//       second one (thread = key = TMEM lane; the two are pipeline stages of consecutive tiles).  dQ_i^T is
-//       drained by a third warpgroup (thread = d = TMEM lane) straight from registers into the fp32 workspace
-//       [B*H][n_pad][d] with coalesced red.global.add.f32 (many key tiles add into the same query rows; the
-//       summation order is not deterministic - SURVEY.md 8c A13).  What bounds the kernel is the tensor pipe
-//       itself: the N = 64 SS MMAs (S^T, dP^T, dQ^T) run at 2/3 rate (operand reads), see DESIGN.md 6.2.
+//       Thread = key = TMEM lane for the elementwise math.  Eight compute warps (two per SM sub-partition: warp w
+//       and w + 4 own the same 32 keys and split the 128 query columns in halves) form P^T = exp2(S^T * scale*log2e
+//       - LSE*log2e), keep it in registers, and then dS^T = P^T o (dP^T - D) of the same tile.  dQ_i^T is drained by a
+//       fourth warpgroup (thread = d = TMEM lane) straight from registers into the fp32 workspace [B*H][n_pad][d]
+//       with coalesced red.global.add.f32 (many key tiles add into the same query rows; the summation order is not
+//       deterministic - SURVEY.md 8c A13).
+//       TMEM is exactly full at d = 128 (S 128 | dPdQ 128 | dV 128 | dK 128 columns), so nothing is double-buffered
+//       there; the issue order  dV(i), S^T(i+1), dQ^T(i), dK(i), dP^T(i+1)  gives every elementwise stage the
+//       shadow of at least one other tile-sized MMA: exp(i+1) runs under dQ^T(i), dK(i), dP^T(i+1); dS(i+1) under
+//       dV(i+1), S^T(i+2); the dQ^T(i) drain under dK(i).  Shared memory (224 KB at d = 128): K, V, dS^T, a 3-stage
+//       Q ring (Q_i is read first by S^T(i) and last by dK(i)), one dO buffer (read by dP^T(i) and dV(i), both early
+//       in a tile) and two slots of {LSE_i log2e, D_i}.
 //   a8  sra_bwd_dq_finalize_kernel  workspace * scale -> bf16 dQ [B, N, H, d]
-//
-// TMEM columns (D = 128): S0 @0 (64), S1 @64 (64), dP0 @128 (64), dP1 @192 (64), dV @256 (128), dK @384 (128);
-// dQ^T(it) overwrites dP^T(it) in dP[it & 1].
+#include <type_traits>
+
 #include "ptx.cuh"
 #include "sra_common.h"
 #include "sra_ctx.h"
 
 namespace sra {
 
+// Development aid (-DSRA_BWD_TRACE): clock64 timestamps of the pipeline events of one CTA over a few iterations.
+#ifdef SRA_BWD_TRACE
+__device__ long long* g_bwd_trace = nullptr;
+#define TR(role, ev)                                                                                                 \
+  do {                                                                                                               \
+    if (tr_on && it >= 100 && it < 108 && g_bwd_trace) g_bwd_trace[((role) * 8 + (it - 100)) * 16 + (ev)] = clock64(); \
+  } while (0)
+#else
+#define TR(role, ev) do { } while (0)
+#endif
+
+#ifndef SRA_BWD_RED_GAP
+#define SRA_BWD_RED_GAP 28  // cycles per dQ reduction instruction of a drain warp (0 = unpaced)
+#endif
+#ifndef SRA_BWD_SPLIT
+#define SRA_BWD_SPLIT 1
+#endif
+#ifndef SRA_BWD_CHUNK
+#define SRA_BWD_CHUNK 32  // score columns per tcgen05.ld of the compute warps (16 or 32)
+#endif
+#ifndef SRA_BWD_EMU
+#define SRA_BWD_EMU 0  // of every 8 column pairs, this many take exp2 on the FMA/ALU pipes (ex2_emu2) instead of MUFU
+#endif
+
 template <int D>
 struct BwdCfg {
-  static constexpr int kQT = kBwdQTile;
+  static constexpr int kQT = kBwdQTile;                 // 128 query rows per iteration
   static constexpr int kKBytes = kTile * D * 2;         // K or V tile
-  static constexpr int kKBoxBytes = kTile * 128;        // one 64-column box of K/V
   static constexpr int kQBytes = kQT * D * 2;           // Q_i or dO_i tile
-  static constexpr int kQBoxBytes = kQT * 128;
-  static constexpr int kBoxes = D / 64;
-  static constexpr int kStages = 4;
-  static constexpr int kStageBytes = 2 * kQBytes;       // Q_i + dO_i
-  static constexpr int kDsBytes = kTile * kQT * 2;      // dS^T tile [128 keys][64 queries] bf16, x2 buffers
-  static constexpr int kVecBytes = kStages * 2 * kQT * 4;  // lse2[64] + delta[64] per stage
-  static constexpr int kNumBars = 1 + 2 * kStages + 2 + 2 + 2 + 2 + 2 + 2 + 2 + 1;
-  static constexpr int kSmemBytes = 2 * kKBytes + kStages * kStageBytes + 2 * kDsBytes + kVecBytes + kNumBars * 8 + 16;
-  static constexpr int kThreads = 512;  // P, dS and dQ warpgroups, MMA + TMA warps (+2 idle)
-  // TMEM columns: S0 | S1 | dP0 | dP1 (64 each) | dV | dK.  dQ^T(it) is written over dP^T(it) in dP[it & 1] once the dS
-  // warpgroup has read it, so dP^T(it+1) has a buffer of its own and does not wait for tile it's dS / dQ chain.
+  static constexpr int kBoxBytes = kTile * 128;         // one 64-column (128 B) box of a 128-row tile
+  static constexpr int kQStages = 3;                    // Q_i ring
+  static constexpr int kVecSlots = 2;                   // {-LSE_i log2e [128], D_i [128]} ring
+  static constexpr int kDsBytes = kTile * kQT * 2;      // dS^T tile: 2 boxes of [128 keys][64 queries] bf16
+  static constexpr int kVecBytes = kVecSlots * 2 * kQT * 4;
+  static constexpr int kNumBars = 1 + 2 * kQStages + 2 + 2 * kVecSlots + 8;
+  static constexpr int kSmemBytes = 2 * kKBytes + (kQStages + 1) * kQBytes + kDsBytes + kVecBytes + kNumBars * 8 + 16;
+  // kSplit compute warps per SM sub-partition share a key row's 128 query columns.  Warps [0, 4 kSplit): compute (P^T,
+  // dS^T; dV epilogue) | next 4: dQ^T drain (dK epilogue) | then the MMA issuer, the loader and 2 idle warps (the register
+  // file is allocated per 4 warps).  A drain thread holds a whole 128-column row of dQ^T, so that the TMEM columns are
+  // released before its first reduction: kSplit = 1 is a 384-thread launch (168 registers each); kSplit = 2 is a
+  // 512-thread launch whose 128 registers per thread are re-cut per warpgroup with setmaxnreg.
+  static constexpr int kSplit = SRA_BWD_SPLIT;
+  static constexpr int kCols = kQT / kSplit;            // query columns per compute thread
+  static constexpr int kComputeWarps = 4 * kSplit;
+  static constexpr int kMmaWarp = kComputeWarps + 4, kLoadWarp = kComputeWarps + 5;
+  static constexpr int kThreads = (kComputeWarps + 8) * 32;
+  static constexpr bool kRecut = kSplit == 2;
+  static constexpr int kRegsCompute = 120, kRegsDrain = 160, kRegsMisc = 80;  // kSplit = 2: (2 x 120 + 160 + 80) x 128 <= 64 K
+  // TMEM columns: S^T (P^T bf16 over it) | dP^T (later dQ^T) | dV | dK
   static constexpr int kColS = 0, kColDP = 128, kColDV = 256, kColDK = 256 + D;
+  static_assert(kSmemBytes <= 232448, "shared memory budget");
 };
 
 template <int D>
-__device__ __forceinline__ void bwd_load_tile(uint32_t dst, int box_bytes, const CUtensorMap* tm, uint32_t bar, int row,
-                                              int h, int b, bool head_major) {
+__device__ __forceinline__ void bwd_load_tile(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int row, int h, int b,
+                                              bool head_major) {
 #pragma unroll
   for (int x = 0; x < D / 64; ++x) {
     if (head_major)
-      tma_load_4d(dst + x * box_bytes, tm, bar, x * 64, row, h, b);
+      tma_load_4d(dst + x * BwdCfg<D>::kBoxBytes, tm, bar, x * 64, row, h, b);
     else
-      tma_load_4d(dst + x * box_bytes, tm, bar, x * 64, h, row, b);
+      tma_load_4d(dst + x * BwdCfg<D>::kBoxBytes, tm, bar, x * 64, h, row, b);
   }
 }
 
@@ -86,29 +125,34 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
                    const BwdParams p) {
   using C = BwdCfg<D>;
   constexpr int QT = C::kQT;
-  constexpr int ST = C::kStages;
+  constexpr int ST = C::kQStages;
+  constexpr int VS = C::kVecSlots;
   extern __shared__ __align__(1024) uint8_t smem_raw[];  // 128-byte-swizzled tiles need 1024-byte alignment
   const uint32_t smem_base = smem_u32(smem_raw);
   if ((smem_base & 1023u) != 0) __trap();
   const uint32_t sK = smem_base;
-  const uint32_t sV = sK + C::kKBytes;
-  const uint32_t sStage = sV + C::kKBytes;                      // [ST] x {Q_i, dO_i}
-  const uint32_t sDs = sStage + ST * C::kStageBytes;            // [2] dS^T
-  const uint32_t sVec = sDs + 2 * C::kDsBytes;                  // [ST] x {lse2[64], delta[64]}
+  const uint32_t sV = sK + C::kKBytes;                          // directly behind K (the d = 64 dQ^T MMA runs on into it)
+  const uint32_t sQ = sV + C::kKBytes;                          // [ST] Q_i
+  const uint32_t sDO = sQ + ST * C::kQBytes;                    // dO_i
+  const uint32_t sDs = sDO + C::kQBytes;                        // dS^T
+  const uint32_t sVec = sDs + C::kDsBytes;                      // [VS] x {-lse2[128], delta[128]}
   const uint32_t sBar = sVec + C::kVecBytes;
   const uint32_t bar_kv_full = sBar;
-  const uint32_t bar_q_full = sBar + 8;                         // [ST]
-  const uint32_t bar_q_empty = bar_q_full + 8 * ST;             // [ST]
-  const uint32_t bar_s_full = bar_q_empty + 8 * ST;             // [2]
-  const uint32_t bar_dp_full = bar_s_full + 16;                 // [2]
-  const uint32_t bar_p_full = bar_dp_full + 16;                 // [2]
-  const uint32_t bar_ds_full = bar_p_full + 16;                 // [2]
-  const uint32_t bar_ds_empty = bar_ds_full + 16;               // [2]
-  const uint32_t bar_dq_full = bar_ds_empty + 16;               // [2]
-  const uint32_t bar_dq_empty = bar_dq_full + 16;               // [1]
-  const uint32_t bar_acc_full = bar_dq_empty + 8;               // [1]
-  const uint32_t s_tmem_ptr = bar_acc_full + 8;
-  uint32_t* tmem_ptr_generic = reinterpret_cast<uint32_t*>(smem_raw + (s_tmem_ptr - smem_u32(smem_raw)));
+  const uint32_t bar_q_full = sBar + 8;                         // [ST] TMA transaction
+  const uint32_t bar_q_empty = bar_q_full + 8 * ST;             // [ST] commit after dK(i)
+  const uint32_t bar_do_full = bar_q_empty + 8 * ST;
+  const uint32_t bar_do_empty = bar_do_full + 8;                // commit after dV(i)
+  const uint32_t bar_vec_full = bar_do_empty + 8;               // [VS] loader warp
+  const uint32_t bar_vec_empty = bar_vec_full + 8 * VS;         // [VS] 8 compute warps, after dS(i)
+  const uint32_t bar_s_full = bar_vec_empty + 8 * VS;
+  const uint32_t bar_p_full = bar_s_full + 8;                   // 8 compute warps
+  const uint32_t bar_dp_full = bar_p_full + 8;
+  const uint32_t bar_ds_full = bar_dp_full + 8;                 // 8 compute warps
+  const uint32_t bar_dq_full = bar_ds_full + 8;
+  const uint32_t bar_dq_empty = bar_dq_full + 8;                // 4 drain warps
+  const uint32_t bar_acc_full = bar_dq_empty + 8;
+  const uint32_t s_tmem_ptr = bar_acc_full + 16;
+  uint32_t* tmem_ptr_generic = reinterpret_cast<uint32_t*>(smem_raw + (s_tmem_ptr - smem_base));
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
@@ -119,6 +163,14 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
   const int n0 = (item.g_len + QT - 1) / QT;  // generation query tiles that see this key tile
   const int n1 = (item.seg1_len + QT - 1) / QT;
   const int n_it = n0 + n1;
+  // Every CTA of a head walks the same query tiles and adds into the same dQ rows; starting each CTA at a different
+  // tile spreads the L2 reductions over addresses (the L2 serialises atomics per address) - the order of a
+  // CTA's query tiles is otherwise free.
+  const int rot = int((blockIdx.x * 2654435761u) >> 8) % n_it;
+  auto tile_of = [&](int i) { const int x = i + rot; return x >= n_it ? x - n_it : x; };
+#ifdef SRA_BWD_TRACE
+  const bool tr_on = blockIdx.x == 5 && blockIdx.y == 0 && blockIdx.z == 0 && (threadIdx.x & 31) == 0;
+#endif
 
   if (threadIdx.x == 0) {
     mbar_init(bar_kv_full, 1);
@@ -126,81 +178,172 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
       mbar_init(bar_q_full + 8 * s, 1);
       mbar_init(bar_q_empty + 8 * s, 1);
     }
-    for (int i = 0; i < 2; ++i) {
-      mbar_init(bar_s_full + 8 * i, 1);
-      mbar_init(bar_p_full + 8 * i, 128);
-      mbar_init(bar_ds_full + 8 * i, 128);
-      mbar_init(bar_ds_empty + 8 * i, 1);
-      mbar_init(bar_dp_full + 8 * i, 1);
-      mbar_init(bar_dq_full + 8 * i, 1);
+    mbar_init(bar_do_full, 1);
+    mbar_init(bar_do_empty, 1);
+    for (int s = 0; s < VS; ++s) {
+      mbar_init(bar_vec_full + 8 * s, 1);
+      mbar_init(bar_vec_empty + 8 * s, C::kComputeWarps);
     }
-    mbar_init(bar_dq_empty, 128);
+    mbar_init(bar_s_full, 1);
+    mbar_init(bar_p_full, C::kComputeWarps);
+    mbar_init(bar_dp_full, 1);
+    mbar_init(bar_ds_full, C::kComputeWarps);
+    mbar_init(bar_dq_full, 1);
+    mbar_init(bar_dq_empty, 4);
     mbar_init(bar_acc_full, 1);
     fence_mbar_init();
   }
-  if (warp == 13 && lane == 0) {
+  if (warp == C::kLoadWarp && lane == 0) {
     tma_prefetch_desc(&tm_q_gen);
     tma_prefetch_desc(&tm_do_gen);
     tma_prefetch_desc(item.k_is_ref ? &tm_k_ref : &tm_k_gen);
     tma_prefetch_desc(item.k_is_ref ? &tm_v_ref : &tm_v_gen);
   }
-  if (warp == 12) tmem_alloc(s_tmem_ptr, 512);
+  if (warp == C::kMmaWarp) tmem_alloc(s_tmem_ptr, 512);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = *tmem_ptr_generic;
 
-  if (warp < 4) {
-    // ================================================= P warpgroup: P^T = exp2(S^T * sl2 - LSE * log2e) (thread = key)
-    // The elementwise work of a tile is split into two pipeline stages on two warpgroups (this one and the
-    // dS warpgroup below), so each SM sub-partition always has warps in different phases (MUFU-bound exp2
-    // here, FMA/LSU-bound dS there, tcgen05.ld round trips in both) and a tile's P^T is ready for dV while
-    // the previous tile's dS^T is still being formed.
-    const int key = warp * 32 + lane;
+  if (warp < C::kComputeWarps) {
+    // ================================================= compute warps (thread = key = TMEM lane)
+    // Warps w and w + 4 sit on the same SM sub-partition and own the same 32 keys; warp w takes query columns [0, 64) of
+    // every tile, warp w + 4 columns [64, 128).  Per tile: P^T = exp2(S^T sl2 - LSE log2e) -> bf16 -> TMEM (the A operand
+    // of dV) and kept in registers; then, once dP^T has landed, dS^T = P^T o (dP^T - D) -> bf16 -> the swizzled
+    // shared-memory tile that is the A operand of dK and the B operand of dQ^T.  A single warp is dispatch-bound on its
+    // own instruction stream (MUFU.EX2 8 cycles, FFMA2 / FADD2 ~3.5, measured); two per sub-partition overlap.
+    if (C::kRecut) reg_dec<C::kRegsCompute>();
+    constexpr int NC = C::kCols;
+    const int hh = warp >> 2;
+    const int key = (warp & 3) * 32 + lane;
     const bool key_valid = key < item.k_rows;
-    const uint32_t lane_off = uint32_t(warp * 32) << 16;
+    const uint32_t lane_off = uint32_t((warp & 3) * 32) << 16;
+    const uint32_t tS = tmem + lane_off + C::kColS + hh * NC;
+    const uint32_t tDP = tmem + lane_off + C::kColDP + hh * NC;
+    uint8_t* const ds_row_g = smem_raw + (sDs - smem_base) + (hh * NC / 64) * C::kBoxBytes + key * 128;  // box x = queries [64 x, +64)
     const float sl2 = p.scale_log2;
+    const uint64_t sl2_2 = pack2(sl2, sl2);
     for (int it = 0; it < n_it; ++it) {
-      const int bf = it & 1, s = it % ST;
-      const uint32_t tS = tmem + lane_off + C::kColS + bf * QT;
-      const uint32_t vec = sVec + s * (2 * QT * 4);
-      mbar_wait(bar_q_full + 8 * s, (it / ST) & 1);  // acquire the loader's lse2 writes
-      mbar_wait(bar_s_full + 8 * bf, (it >> 1) & 1);
+      const int vs = it % VS;
+      // -lse2 of this warp's queries; delta at + QT floats.  Plain (non-volatile) shared-memory loads, so that the
+      // compiler batches them ahead of the arithmetic instead of exposing one load latency per four elements.
+      const float4* vec = reinterpret_cast<const float4*>(smem_raw + (sVec - smem_base) + vs * (2 * QT * 4) + hh * NC * 4);
+      const int tq = tile_of(it);
+      const int valid_h = (tq < n0 ? min(QT, item.g_len - tq * QT) : min(QT, item.seg1_len - (tq - n0) * QT)) - NC * hh;
+      if ((warp & 3) == 0) TR(1 + hh, 0);
+      mbar_wait(bar_vec_full + 8 * vs, (it / VS) & 1);  // acquire the loader's -lse2 / delta stores
+      mbar_wait(bar_s_full, it & 1);
+      if ((warp & 3) == 0) TR(1 + hh, 1);
       tc_fence_after();
+      // The columns stream through two 32-column register buffers: the tcgen05.ld of the next chunk is in flight
+      // while this one is exponentiated.
       uint32_t sv[2][32];
+      uint32_t pk[NC / 2];
       tmem_ld32(tS, sv[0]);
-      tmem_ld32(tS + 32, sv[1]);
-      tmem_wait_ld();
-      uint32_t pk[32];
 #pragma unroll
-      for (int c = 0; c < 2; ++c)
+      for (int c = 0; c < NC / 32; ++c) {
+        tmem_wait_ld();
+        if (c + 1 < NC / 32) tmem_ld32(tS + (c + 1) * 32, sv[(c + 1) & 1]);
+        const uint32_t(&sc)[32] = sv[c & 1];
 #pragma unroll
         for (int q4 = 0; q4 < 8; ++q4) {
-          const float4 l = ld_shared_f4(vec + (c * 32 + q4 * 4) * 4);
-          const float p0 = ex2(fmaf(__uint_as_float(sv[c][q4 * 4 + 0]), sl2, -l.x));
-          const float p1 = ex2(fmaf(__uint_as_float(sv[c][q4 * 4 + 1]), sl2, -l.y));
-          const float p2 = ex2(fmaf(__uint_as_float(sv[c][q4 * 4 + 2]), sl2, -l.z));
-          const float p3 = ex2(fmaf(__uint_as_float(sv[c][q4 * 4 + 3]), sl2, -l.w));
+#ifdef SRA_BWD_NOVEC  // (ablation builds only: no shared-memory loads of the row constants, results are wrong)
+          const float4 nl = make_float4(-8.f, -8.f, -8.f, -8.f);
+#else
+          const float4 nl = vec[c * 8 + q4];
+#endif
+          const uint64_t x01 = fma2(pack2(__uint_as_float(sc[q4 * 4 + 0]), __uint_as_float(sc[q4 * 4 + 1])), sl2_2, pack2(nl.x, nl.y));
+          const uint64_t x23 = fma2(pack2(__uint_as_float(sc[q4 * 4 + 2]), __uint_as_float(sc[q4 * 4 + 3])), sl2_2, pack2(nl.z, nl.w));
+          float p0, p1, p2, p3;
+          if ((((2 * q4) * SRA_BWD_EMU) & 7) < SRA_BWD_EMU) ex2_emu2(x01, p0, p1);
+          else { float a, bb; unpack2(x01, a, bb); p0 = ex2(a); p1 = ex2(bb); }
+          if ((((2 * q4 + 1) * SRA_BWD_EMU) & 7) < SRA_BWD_EMU) ex2_emu2(x23, p2, p3);
+          else { float a, bb; unpack2(x23, a, bb); p2 = ex2(a); p3 = ex2(bb); }
           pk[c * 16 + q4 * 2 + 0] = pack_bf16(p0, p1);
           pk[c * 16 + q4 * 2 + 1] = pack_bf16(p2, p3);
         }
-      tmem_st32(tS, pk);  // P^T: bf16 pairs in the first 32 columns of S[bf]
+      }
+      if (valid_h < NC) {
+        // ragged last query tile of a segment: the rows behind it belong to a neighbour (or are TMA zero fill);
+        // their P^T columns are forced to 0 by selection, whatever the scores were
+#pragma unroll
+        for (int k = 0; k < NC / 2; ++k) {
+          if (2 * k >= valid_h) pk[k] = 0u;
+          else if (2 * k + 1 >= valid_h) pk[k] &= 0xffffu;
+        }
+      }
+      // P^T: bf16 pairs over the first half of the score columns this warp has read (columns [kCols hh, + kCols / 2) of
+      // S), so no warp of a key row overwrites scores a partner may still be loading
+#pragma unroll
+      for (int x = 0; x < NC / 64; ++x) tmem_st32(tS + x * 32, *reinterpret_cast<uint32_t(*)[32]>(&pk[x * 32]));
       tmem_wait_st();
       tc_fence_before();
-      mbar_arrive(bar_p_full + 8 * bf);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar_p_full);
+      if ((warp & 3) == 0) TR(1 + hh, 2);
+      // ---- dS^T(it)
+      mbar_wait(bar_dp_full, it & 1);  // dP^T(it) has landed; every earlier MMA (dQ^T / dK of it-1, readers of sDs) is done
+      if ((warp & 3) == 0) TR(1 + hh, 3);
+      tc_fence_after();
+      // dS^T pair = P^T pair (bf16x2, as the dV MMA consumes it) * bf16x2(dP^T pair - D pair): one packed subtract, one
+      // conversion and one packed bf16 multiply per two elements.  (The selections of the masked form cost an
+      // instruction per pair, so the aligned interior takes the plain loop.)
+      auto form_ds = [&](auto masked) {
+        tmem_ld32(tDP, sv[0]);
+#pragma unroll
+        for (int c = 0; c < NC / 32; ++c) {
+          tmem_wait_ld();
+          if (c + 1 < NC / 32) tmem_ld32(tDP + (c + 1) * 32, sv[(c + 1) & 1]);
+          const uint32_t(&dp)[32] = sv[c & 1];
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {  // 8 queries = one 16-byte chunk of the dS^T row
+#ifdef SRA_BWD_NOVEC
+            const float4 d0 = make_float4(0.f, 0.f, 0.f, 0.f), d1 = d0;
+#else
+            const float4 d0 = vec[QT / 4 + c * 8 + e * 2];
+            const float4 d1 = vec[QT / 4 + c * 8 + e * 2 + 1];
+#endif
+            const uint64_t dl[4] = {pack2(d0.x, d0.y), pack2(d0.z, d0.w), pack2(d1.x, d1.y), pack2(d1.z, d1.w)};
+            uint32_t w[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+              const int q = c * 32 + e * 8 + 2 * k;  // query column of this half
+              float a, bb;
+              unpack2(sub2(pack2(__uint_as_float(dp[e * 8 + 2 * k]), __uint_as_float(dp[e * 8 + 2 * k + 1])), dl[k]), a, bb);
+              w[k] = mul_bf16x2(pk[q >> 1], pack_bf16(a, bb));
+              if (decltype(masked)::value) {
+                if (!key_valid || q >= valid_h) w[k] = 0u;
+                else if (q + 1 >= valid_h) w[k] &= 0xffffu;
+              }
+            }
+            const int ch16 = c * 4 + e;  // 16-byte chunk of this thread's dS^T row range
+            *reinterpret_cast<uint4*>(ds_row_g + (ch16 / 8) * C::kBoxBytes + (((ch16 & 7) ^ (key & 7)) << 4)) =
+                make_uint4(w[0], w[1], w[2], w[3]);
+          }
+        }
+      };
+      if (__any_sync(0xffffffffu, !key_valid) || valid_h < NC) form_ds(std::true_type{}); else form_ds(std::false_type{});
+      tc_fence_before();  // the dP^T columns may be overwritten by dQ^T(it) once ds_full completes
+      fence_proxy_async_smem();
+      __syncwarp();
+      if (lane == 0) {
+        mbar_arrive(bar_ds_full);
+        mbar_arrive(bar_vec_empty + 8 * vs);
+      }
+      if ((warp & 3) == 0) TR(1 + hh, 4);
     }
-    // ---------------------------------------------------- epilogue: dV (lanes = keys)
+    // ---------------------------------------------------- epilogue: dV (lanes = keys), D / kSplit columns per warp
     mbar_wait(bar_acc_full, 0);
     tc_fence_after();
     {
       const int n_tok = item.k_is_ref ? p.n_ref : p.n_gen;
       const int grow = item.k_row0 + key;
       __nv_bfloat16* base = item.k_is_ref ? p.dv_ref : p.dv_gen;
-      uint4* orow = reinterpret_cast<uint4*>(base + ((size_t(b) * n_tok + grow) * p.heads + h) * D);
+      uint4* orow = reinterpret_cast<uint4*>(base + ((size_t(b) * n_tok + grow) * p.heads + h) * D + hh * (D / C::kSplit));
 #pragma unroll
-      for (int c = 0; c < D / 32; ++c) {
+      for (int c = 0; c < D / C::kSplit / 32; ++c) {
         uint32_t o[32];
-        tmem_ld32(tmem + lane_off + C::kColDV + c * 32, o);
+        tmem_ld32(tmem + lane_off + C::kColDV + hh * (D / C::kSplit) + c * 32, o);
         tmem_wait_ld();
         if (key_valid) {
 #pragma unroll
@@ -216,82 +359,67 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
       }
     }
     tc_fence_before();
-  } else if (warp < 8) {
-    // ================================================= dS warpgroup: dS^T = P^T o (dP^T - D) (thread = key)
-    // P^T is read back from TMEM as the bf16 the dV MMA consumes (S[bf] is not overwritten before the
-    // MMA issuer has seen ds_full of this tile).
-    const int wk = warp - 4;
-    const int key = wk * 32 + lane;
+  } else if (warp < C::kComputeWarps + 4) {
+    // ================================================= drain warps: dQ^T (thread = d = TMEM lane), then the dK epilogue
+    if (C::kRecut) reg_inc<C::kRegsDrain>();
+    const int wq = warp - C::kComputeWarps;
+    const int key = wq * 32 + lane;
     const bool key_valid = key < item.k_rows;
-    const uint32_t lane_off = uint32_t(wk * 32) << 16;
-    for (int it = 0; it < n_it; ++it) {
-      const int bf = it & 1, s = it % ST;
-      const uint32_t tP = tmem + lane_off + C::kColS + bf * QT;
-      const uint32_t tDP = tmem + lane_off + C::kColDP + bf * QT;
-      const uint32_t vec = sVec + s * (2 * QT * 4) + QT * 4;  // delta[64]
-      mbar_wait(bar_q_full + 8 * s, (it / ST) & 1);  // acquire the loader's delta writes
-      mbar_wait(bar_p_full + 8 * bf, (it >> 1) & 1);
-      mbar_wait(bar_dp_full + 8 * bf, (it >> 1) & 1);
-      tc_fence_after();
-      uint32_t pb[32], dp[2][32];
-      tmem_ld32(tP, pb);
-      tmem_ld32(tDP, dp[0]);
-      tmem_ld32(tDP + 32, dp[1]);
-      tmem_wait_ld();
-      mbar_wait(bar_ds_empty + 8 * bf, ((it >> 1) & 1) ^ 1);  // dK / dQ MMAs of iteration it-2 have read sDs[bf]
-      const uint32_t ds_row = sDs + bf * C::kDsBytes + key * 128;
-#pragma unroll
-      for (int c = 0; c < 8; ++c) {  // 16-byte chunk c = queries [8c, 8c+8)
-        const float4 d0 = ld_shared_f4(vec + (c * 8) * 4);
-        const float4 d1 = ld_shared_f4(vec + (c * 8 + 4) * 4);
-        const float dl[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
-        uint32_t w[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          const int q = c * 8 + 2 * k;
-          const uint32_t pp = pb[q >> 1];
-          float a = __uint_as_float(pp << 16) * (__uint_as_float(dp[q >> 5][q & 31]) - dl[2 * k]);
-          float bb = __uint_as_float(pp & 0xffff0000u) * (__uint_as_float(dp[(q + 1) >> 5][(q + 1) & 31]) - dl[2 * k + 1]);
-          if (!key_valid) { a = 0.f; bb = 0.f; }
-          w[k] = pack_bf16(a, bb);
-        }
-        st_shared_v4(ds_row + ((c ^ (key & 7)) << 4), w[0], w[1], w[2], w[3]);
-      }
-      fence_proxy_async_smem();
-      tc_fence_before();
-      mbar_arrive(bar_ds_full + 8 * bf);
-    }
-  } else if (warp < 12) {
-    // ================================================= reduce warpgroup: dQ^T drain (thread = d), then dK epilogue
-    const int wq = warp - 8;
-    const int drow = wq * 32 + lane;  // TMEM lane = d index (dQ^T), later = key index (dK)
     const uint32_t lane_off = uint32_t(wq * 32) << 16;
     for (int it = 0; it < n_it; ++it) {
-      const QTile qt = q_tile_of(it, n0, item, p.n_gen);
-      mbar_wait(bar_dq_full + 8 * (it & 1), (it >> 1) & 1);
+      const QTile qt = q_tile_of(tile_of(it), n0, item, p.n_gen);
+      if (wq == 0) TR(3, 0);
+      mbar_wait(bar_dq_full, it & 1);
+      if (wq == 0) TR(3, 1);
       tc_fence_after();
-      uint32_t r[2][32];
-      tmem_ld32(tmem + lane_off + C::kColDP + (it & 1) * QT, r[0]);
-      tmem_ld32(tmem + lane_off + C::kColDP + (it & 1) * QT + 32, r[1]);
+      // dQ_it^T leaves the SM straight from registers: for a fixed query the 32 lanes of a warp hold 32 consecutive d,
+      // so each red.global.add.f32 is one coalesced 128-byte reduction into the fp32 workspace.  All 128 columns are
+      // taken into registers first, so that the TMEM columns are released (dq_empty) before the first reduction - the
+      // reductions run at the LSU -> L2 rate, far longer than dP^T(it+1) may wait.
+      const int drow = key;
+      float* dq_row = p.dq_ws + (size_t(bh) * p.n_pad + qt.cat0) * D + drow;
+      uint32_t r[4][32];
+#pragma unroll
+      for (int x = 0; x < 4; ++x) tmem_ld32(tmem + lane_off + C::kColDP + x * 32, r[x]);
       tmem_wait_ld();
       tc_fence_before();
-      mbar_arrive(bar_dq_empty);
-      // dQ_it^T leaves the SM straight from registers: for a fixed query the 32 lanes of a warp hold 32
-      // consecutive d, so each red.global.add.f32 is one coalesced 128-byte reduction into the fp32
-      // workspace (no shared-memory staging: the kernel is bound by shared-memory bandwidth).
-      float* dq_row = p.dq_ws + (size_t(bh) * p.n_pad + qt.cat0) * D + drow;
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar_dq_empty);  // dQ^T(it) is in registers: the columns are free for dP^T(it+1)
+      if (wq == 0) TR(3, 2);
+      if (drow < D) {
+        if (qt.valid == QT) {
+          // The reductions share each sub-partition's memory-instruction queue with the compute warp's tcgen05.ld / st and
+          // shared-memory accesses; issued back to back they fill it (the LSU -> L2 path drains ~22 B/clk/SM) and the
+          // compute warp stalls behind them.  They are paced instead: groups of 8, kRedGap cycles apart.
+          long long t_next = clock64();
 #pragma unroll
-      for (int x = 0; x < 2; ++x)
+          for (int x = 0; x < 4; ++x)
 #pragma unroll
-        for (int c = 0; c < 32; ++c)
-          if (drow < D && x * 32 + c < qt.valid) red_add_f32(dq_row + (x * 32 + c) * D, __uint_as_float(r[x][c]));
+            for (int c = 0; c < 32; ++c) {
+              if (SRA_BWD_RED_GAP > 0 && (c & 7) == 0) {
+                while (clock64() < t_next) { }
+                t_next += 8 * SRA_BWD_RED_GAP;
+              }
+#ifndef SRA_BWD_NORED  // (ablation builds only: drop the reductions, dQ is then wrong)
+              red_add_f32(dq_row + (x * 32 + c) * D, __uint_as_float(r[x][c]));
+#else
+              if (r[x][c] == 0x7fc12345u) red_add_f32(dq_row, 1.f);
+#endif
+            }
+        } else {
+#pragma unroll
+          for (int x = 0; x < 4; ++x)
+#pragma unroll
+            for (int c = 0; c < 32; ++c)
+              if (x * 32 + c < qt.valid) red_add_f32(dq_row + (x * 32 + c) * D, __uint_as_float(r[x][c]));
+        }
+      }
+      if (wq == 0) TR(3, 3);
     }
     // ---------------------------------------------------- epilogue: dK = scale * acc (lanes = keys)
     mbar_wait(bar_acc_full, 0);
     tc_fence_after();
     {
-      const int key = drow;
-      const bool key_valid = key < item.k_rows;
       const int n_tok = item.k_is_ref ? p.n_ref : p.n_gen;
       const int grow = item.k_row0 + key;
       __nv_bfloat16* base = item.k_is_ref ? p.dk_ref : p.dk_gen;
@@ -317,113 +445,146 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
     }
     tc_fence_before();
   } else {
-    if (warp == 13) {
-      // ================================================= loader: K/V once, then the {Q_i, dO_i, lse2, delta} ring
+    if (C::kRecut) reg_dec<C::kRegsMisc>();
+    if (warp == C::kLoadWarp) {
+      // ================================================= loader: K/V once, then per tile Q_i (3 stages), {-lse2, delta}
+      // (2 slots, written by the 32 lanes) and dO_i (one buffer, free once dV(i-1) is done)
       const bool k_hm = item.k_is_ref && p.ref_kv_head_major;
       if (lane == 0) {
         mbar_arrive_expect_tx(bar_kv_full, 2 * C::kKBytes);
-        bwd_load_tile<D>(sK, C::kKBoxBytes, item.k_is_ref ? &tm_k_ref : &tm_k_gen, bar_kv_full, item.k_row0, h, b, k_hm);
-        bwd_load_tile<D>(sV, C::kKBoxBytes, item.k_is_ref ? &tm_v_ref : &tm_v_gen, bar_kv_full, item.k_row0, h, b, k_hm);
+        bwd_load_tile<D>(sK, item.k_is_ref ? &tm_k_ref : &tm_k_gen, bar_kv_full, item.k_row0, h, b, k_hm);
+        bwd_load_tile<D>(sV, item.k_is_ref ? &tm_v_ref : &tm_v_gen, bar_kv_full, item.k_row0, h, b, k_hm);
       }
       const float* lse2 = p.lse2 + size_t(bh) * p.n_pad;
       const float* delta = p.delta + size_t(bh) * p.n_pad;
       for (int it = 0; it < n_it; ++it) {
-        const int s = it % ST;
-        const QTile qt = q_tile_of(it, n0, item, p.n_gen);
-        mbar_wait(bar_q_empty + 8 * s, ((it / ST) & 1) ^ 1);
-        const uint32_t vec = sVec + s * (2 * QT * 4);
+        const int s = it % ST, vs = it % VS;
+        const QTile qt = q_tile_of(tile_of(it), n0, item, p.n_gen);
+        // the tile's row constants, fetched before any wait so that their latency hides behind it
+        float nl[QT / 32], dl[QT / 32];
 #pragma unroll
-        for (int r = lane; r < QT; r += 32) {
-          const bool ok = r < qt.valid;
-          st_shared_f32(vec + r * 4, ok ? lse2[qt.cat0 + r] : INFINITY);   // +inf => P = 0 for rows outside the tile
-          st_shared_f32(vec + QT * 4 + r * 4, ok ? delta[qt.cat0 + r] : 0.f);
+        for (int r = 0; r < QT / 32; ++r) {
+          const int row = r * 32 + lane;
+          const bool ok = row < qt.valid;
+          nl[r] = ok ? -__ldg(lse2 + qt.cat0 + row) : -INFINITY;  // -inf => P = 0 for rows outside the tile
+          dl[r] = ok ? __ldg(delta + qt.cat0 + row) : 0.f;
+        }
+        TR(4, 0);
+        mbar_wait(bar_q_empty + 8 * s, ((it / ST) & 1) ^ 1);
+        TR(4, 1);
+        if (lane == 0) {
+          mbar_arrive_expect_tx(bar_q_full + 8 * s, C::kQBytes);
+          bwd_load_tile<D>(sQ + s * C::kQBytes, qt.is_ref ? &tm_q_ref : &tm_q_gen, bar_q_full + 8 * s, qt.row0, h, b, false);
+        }
+        mbar_wait(bar_vec_empty + 8 * vs, ((it / VS) & 1) ^ 1);
+        TR(4, 2);
+        const uint32_t vec = sVec + vs * (2 * QT * 4);
+#pragma unroll
+        for (int r = 0; r < QT / 32; ++r) {
+          st_shared_f32(vec + (r * 32 + lane) * 4, nl[r]);
+          st_shared_f32(vec + QT * 4 + (r * 32 + lane) * 4, dl[r]);
         }
         __syncwarp();
+        if (lane == 0) mbar_arrive(bar_vec_full + 8 * vs);
+        mbar_wait(bar_do_empty, (it & 1) ^ 1);
+        TR(4, 3);
         if (lane == 0) {
-          const uint32_t dst = sStage + s * C::kStageBytes;
-          mbar_arrive_expect_tx(bar_q_full + 8 * s, 2 * C::kQBytes);
-          bwd_load_tile<D>(dst, C::kQBoxBytes, qt.is_ref ? &tm_q_ref : &tm_q_gen, bar_q_full + 8 * s, qt.row0, h, b, false);
-          bwd_load_tile<D>(dst + C::kQBytes, C::kQBoxBytes, qt.is_ref ? &tm_do_ref : &tm_do_gen, bar_q_full + 8 * s,
-                           qt.row0, h, b, false);
+          mbar_arrive_expect_tx(bar_do_full, C::kQBytes);
+          bwd_load_tile<D>(sDO, qt.is_ref ? &tm_do_ref : &tm_do_gen, bar_do_full, qt.row0, h, b, false);
         }
       }
-    } else if (warp == 12 && elect_one()) {
+    } else if (warp == C::kMmaWarp && elect_one()) {
       // ================================================= MMA issuer
-      constexpr uint32_t idesc_st = make_idesc_bf16(kTile, QT, 0, 0);   // S^T, dP^T : [128 x 64], K = d
-      constexpr uint32_t idesc_acc = make_idesc_bf16(kTile, D, 0, 1);   // dV, dK    : [128 x D],  K = 64 queries
-      // dQ^T : [D x 64], K = 128 keys.  With D = 64 the MMA is still issued with M = 128 (the M = 64 accumulator layout
-      // differs): its A operand then runs on from the K tile into the V tile behind it, TMEM lanes [64, 128) receive
-      // finite garbage (V^T dS^T) and the drain ignores them.
+      constexpr uint32_t idesc_st = make_idesc_bf16(kTile, QT, 0, 0);   // S^T, dP^T : [128 x 128], A, B K-major, K = d
+      constexpr uint32_t idesc_acc = make_idesc_bf16(kTile, D, 0, 1);   // dV, dK    : [128 x D], B MN-major, K = 128 queries
+      // dQ^T : [D x 128], A, B MN-major, K = 128 keys.  With D = 64 the MMA is still issued with M = 128 (the M = 64
+      // accumulator layout differs): its A operand then runs on from the K tile into the V tile behind it, TMEM lanes
+      // [64, 128) receive finite garbage (V^T dS^T) and the drain ignores them.
       constexpr uint32_t idesc_dq = make_idesc_bf16(kTile, QT, 1, 1);
-      const uint32_t tS0 = tmem + C::kColS, tDP0 = tmem + C::kColDP;
-      const uint32_t tDV = tmem + C::kColDV, tDK = tmem + C::kColDK;
+      const uint32_t tS = tmem + C::kColS, tDP = tmem + C::kColDP, tDV = tmem + C::kColDV, tDK = tmem + C::kColDK;
       // Descriptor low words (start address, LBO); stepping along K or to another stage is one 32-bit add.
       constexpr uint32_t kHi = desc_hi_sw128(1024);
       const uint32_t k_km = desc_lo(sK, 16), v_km = desc_lo(sV, 16);             // K, V as K-major A operands
-      const uint32_t k_mn = desc_lo(sK, C::kKBoxBytes);                          // K as MN-major A operand (dQ^T)
-      const uint32_t st_km = desc_lo(sStage, 16);                                // Q_i / dO_i as K-major B operands
-      const uint32_t st_mn = desc_lo(sStage, C::kQBoxBytes);                     // Q_i / dO_i as MN-major B operands
-      const uint32_t ds_km = desc_lo(sDs, 16), ds_mn = desc_lo(sDs, C::kDsBytes);
-      // [128 x 64] = A[128 keys][d] (K-major) * B[64 queries][d]^T (K-major); b_off = byte offset inside sStage
-      auto issue_kq = [&](uint32_t d_tmem, uint32_t a_lo, uint32_t b_off) {
+      const uint32_t k_mn = desc_lo(sK, C::kBoxBytes);                           // K as MN-major A operand (dQ^T)
+      const uint32_t q_km = desc_lo(sQ, 16), do_km = desc_lo(sDO, 16);           // Q_i / dO_i as K-major B operands
+      const uint32_t q_mn = desc_lo(sQ, C::kBoxBytes), do_mn = desc_lo(sDO, C::kBoxBytes);  // ... as MN-major B operands
+      const uint32_t ds_km = desc_lo(sDs, 16), ds_mn = desc_lo(sDs, C::kBoxBytes);
+      // [128 keys x 128 queries] = A[keys][d] (K-major) * B[queries][d]^T (K-major)
+      auto issue_kq = [&](uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo) {
 #pragma unroll
-        for (int kk = 0; kk < D / 16; ++kk)
-          umma_ss(d_tmem, desc64(a_lo + (((kk / 4) * C::kKBoxBytes + (kk % 4) * 32) >> 4), kHi),
-                  desc64(st_km + ((b_off + (kk / 4) * C::kQBoxBytes + (kk % 4) * 32) >> 4), kHi), idesc_st, kk > 0);
+        for (int kk = 0; kk < D / 16; ++kk) {
+          const uint32_t off = ((kk / 4) * C::kBoxBytes + (kk % 4) * 32) >> 4;
+          umma_ss(d_tmem, desc64(a_lo + off, kHi), desc64(b_lo + off, kHi), idesc_st, kk > 0);
+        }
       };
       mbar_wait(bar_kv_full, 0);
       mbar_wait(bar_q_full, 0);
       tc_fence_after();
-      issue_kq(tS0, k_km, 0);
+      issue_kq(tS, k_km, q_km);
       umma_commit(bar_s_full);
-      issue_kq(tDP0, v_km, C::kQBytes);
+      mbar_wait(bar_do_full, 0);
+      tc_fence_after();
+      issue_kq(tDP, v_km, do_km);
       umma_commit(bar_dp_full);
       for (int it = 0; it < n_it; ++it) {
-        const int bf = it & 1, s = it % ST;
-        const uint32_t oQ = s * C::kStageBytes, oDO = oQ + C::kQBytes;  // byte offsets inside sStage
-        const uint32_t ods = bf * C::kDsBytes;
+        const int s = it % ST;
+        const uint32_t oQ = (s * C::kQBytes) >> 4;
         const bool more = it + 1 < n_it;
-        const int s1 = (it + 1) % ST;
-        const uint32_t oQ1 = s1 * C::kStageBytes;
-        if (more) {
-          mbar_wait(bar_q_full + 8 * s1, ((it + 1) / ST) & 1);
-          tc_fence_after();
-          issue_kq(tS0 + (bf ^ 1) * QT, k_km, oQ1);  // S^T(it+1); its buffer held P^T(it-1), consumed by dV(it-1)
-          umma_commit(bar_s_full + 8 * (bf ^ 1));
-          // dP^T(it+1) -> dP[bf ^ 1], which last held dQ^T(it-1): only the dQ warpgroup's drain of that tile gates it
-          mbar_wait(bar_dq_empty, (it & 1) ^ 1);
-          tc_fence_after();
-          issue_kq(tDP0 + (bf ^ 1) * QT, v_km, oQ1 + C::kQBytes);
-          umma_commit(bar_dp_full + 8 * (bf ^ 1));
-        }
-        // dV += P^T(it) dO_it : A = P^T from TMEM (16 queries = 8 columns per step), B = dO_it [queries][d] MN-major
-        mbar_wait(bar_p_full + 8 * bf, (it >> 1) & 1);
+        // dV += P^T(it) dO_it : A = P^T bf16 from TMEM (16 queries = 8 columns per step; the pairs of compute warp
+        // group x sit at column kCols x), B = dO_it [queries][d] MN-major
+        TR(0, 0);
+        mbar_wait(bar_p_full, it & 1);
+        TR(0, 1);
         tc_fence_after();
 #pragma unroll
         for (int kk = 0; kk < QT / 16; ++kk)
-          umma_ts(tDV, tS0 + bf * QT + kk * 8, desc64(st_mn + ((oDO + kk * 2048) >> 4), kHi), idesc_acc,
+          umma_ts(tDV, tS + ((kk * 16) / C::kCols) * C::kCols + ((kk * 16) % C::kCols) / 2, desc64(do_mn + ((kk * 2048) >> 4), kHi), idesc_acc,
                   (it > 0 || kk > 0) ? 1u : 0u);
-        mbar_wait(bar_ds_full + 8 * bf, (it >> 1) & 1);  // dS^T(it) in smem; dP^T(it) has been read out of TMEM
+        umma_commit(bar_do_empty);  // dO_it has been read by dP^T(it) and dV(it)
+        TR(0, 2);
+        if (more) {
+          // S^T(it+1) overwrites S^T / P^T(it): in order behind dV(it); the compute warps have read S^T(it) (p_full)
+          const int s1 = (it + 1) % ST;
+          mbar_wait(bar_q_full + 8 * s1, ((it + 1) / ST) & 1);
+          TR(0, 3);
+          tc_fence_after();
+          issue_kq(tS, k_km, q_km + ((s1 * C::kQBytes) >> 4));
+          umma_commit(bar_s_full);
+          TR(0, 4);
+        }
+        mbar_wait(bar_ds_full, it & 1);  // dS^T(it) in shared memory; dP^T(it) has been read out of TMEM
+        TR(0, 5);
         tc_fence_after();
-        // dK += dS^T(it) Q_it : A = dS^T [keys][queries] K-major (one 128-byte box), B = Q_it [queries][d] MN-major
-#pragma unroll
-        for (int kk = 0; kk < QT / 16; ++kk)
-          umma_ss(tDK, desc64(ds_km + ((ods + kk * 32) >> 4), kHi), desc64(st_mn + ((oQ + kk * 2048) >> 4), kHi),
-                  idesc_acc, (it > 0 || kk > 0) ? 1u : 0u);
-        // dQ_it^T = K^T dS^T(it) : A = K [keys][d] MN-major, B = dS^T [keys][queries] MN-major, K = 128 keys; written
-        // over dP^T(it), which the dS warpgroup has read (ds_full)
+        // dQ_it^T = K^T dS^T(it) : A = K [keys][d] MN-major, B = dS^T [keys][queries] MN-major, K = 128 keys; lands over
+        // dP^T(it).  Issued before dK so that its drain runs under the dK MMA.
 #pragma unroll
         for (int kk = 0; kk < kTile / 16; ++kk)
-          umma_ss(tDP0 + bf * QT, desc64(k_mn + ((kk * 2048) >> 4), kHi), desc64(ds_mn + ((ods + kk * 2048) >> 4), kHi), idesc_dq, kk > 0);
-        umma_commit(bar_dq_full + 8 * bf);
+          umma_ss(tDP, desc64(k_mn + ((kk * 2048) >> 4), kHi), desc64(ds_mn + ((kk * 2048) >> 4), kHi), idesc_dq, kk > 0);
+        umma_commit(bar_dq_full);
+        TR(0, 6);
+        // dK += dS^T(it) Q_it : A = dS^T [keys][queries] K-major (two 64-query boxes), B = Q_it [queries][d] MN-major
+#pragma unroll
+        for (int kk = 0; kk < QT / 16; ++kk)
+          umma_ss(tDK, desc64(ds_km + (((kk / 4) * C::kBoxBytes + (kk % 4) * 32) >> 4), kHi),
+                  desc64(q_mn + oQ + ((kk * 2048) >> 4), kHi), idesc_acc, (it > 0 || kk > 0) ? 1u : 0u);
         umma_commit(bar_q_empty + 8 * s);
-        umma_commit(bar_ds_empty + 8 * bf);
+        TR(0, 7);
+        if (more) {
+          mbar_wait(bar_do_full, (it + 1) & 1);
+          TR(0, 8);
+          mbar_wait(bar_dq_empty, it & 1);
+          TR(0, 9);  // dQ^T(it) is in registers: the columns are free for dP^T(it+1)
+          tc_fence_after();
+          issue_kq(tDP, v_km, do_km);
+          umma_commit(bar_dp_full);
+          TR(0, 10);
+        }
       }
       umma_commit(bar_acc_full);
     }
   }
   __syncthreads();
-  if (warp == 12) {
+  if (warp == C::kMmaWarp) {
     tc_fence_after();
     tmem_dealloc(tmem, 512);
   }
@@ -525,6 +686,9 @@ cudaError_t launch_bwd(const CUtensorMap* m, const BwdParams& p, cudaStream_t st
   return cudaGetLastError();
 }
 
+#ifdef SRA_BWD_TRACE
+extern "C" void sra_dbg_set_bwd_trace(long long* p) { cudaMemcpyToSymbol(g_bwd_trace, &p, sizeof(p)); }
+#endif
 template cudaError_t launch_bwd<64>(const CUtensorMap*, const BwdParams&, cudaStream_t);
 template cudaError_t launch_bwd<128>(const CUtensorMap*, const BwdParams&, cudaStream_t);
 

@@ -55,7 +55,7 @@ struct FwdParams {
   float* part_lse;  // fp32 [n_split][B][H][n_gen]:    LSE_s (natural log of the scaled scores)
 };
 
-constexpr int kBwdQTile = 64;  // query rows per backward iteration (keys per CTA = kTile)
+constexpr int kBwdQTile = 128;  // query rows per backward iteration (keys per CTA = kTile)
 
 struct BwdParams {
   const BwdItem* items;
