@@ -328,6 +328,33 @@ static void build_schedule(sra_ctx* ctx) {
       for (int r = 0; r < ctx->n_ref_items; ++r) ctx->split_items.push_back(ctx->fwd_items[ctx->n_gen_items + r]);
     }
   }
+  // CTA pairs (sra_fwd_kernel<128, 2>): two consecutive slabs of the same kind that see the same keys and tile 512
+  // consecutive rows run as one cluster of two CTAs sharing every K/V tile.
+  ctx->pair_items.clear();
+  ctx->pair_of_item.assign(ctx->fwd_items.size() + 1, 0);
+  ctx->n_gen_pairs = ctx->n_ref_pairs = 0;
+  for (size_t i = 0; i < ctx->fwd_items.size();) {
+    FwdItem it = ctx->fwd_items[i];
+    size_t used = 1;
+    if (i + 1 < ctx->fwd_items.size()) {
+      const FwdItem& nx = ctx->fwd_items[i + 1];
+      if (nx.q_is_ref == it.q_is_ref && it.q_rows == kQRowsPerCta && nx.q_row0 == it.q_row0 + kQRowsPerCta &&
+          nx.seg0_is_ref == it.seg0_is_ref && nx.seg0_start == it.seg0_start && nx.seg0_len == it.seg0_len &&
+          nx.seg1_start == it.seg1_start && nx.seg1_len == it.seg1_len) {
+        it.q_rows += nx.q_rows;
+        used = 2;
+      }
+    }
+    for (size_t k = 0; k < used; ++k) ctx->pair_of_item[i + k] = int32_t(ctx->pair_items.size());
+    (it.q_is_ref ? ctx->n_ref_pairs : ctx->n_gen_pairs) += 1;
+    ctx->pair_items.push_back(it);
+    i += used;
+  }
+  ctx->pair_of_item[ctx->fwd_items.size()] = int32_t(ctx->pair_items.size());
+  ctx->use_pairs = ctx->cfg.head_dim == 128 && ctx->n_split == 1;
+#ifdef SRA_NO_PAIRS  // (A/B builds: the single-CTA kernel everywhere)
+  ctx->use_pairs = false;
+#endif
   // Backward: key tiles.  G key tiles are seen by all G queries; R key tiles of block j additionally by block j's
   // R queries.  Tiles never straddle a block boundary.
   ctx->bwd_items.clear();
@@ -358,13 +385,18 @@ static void build_schedule(sra_ctx* ctx) {
 // (Re)allocates the device copies of the schedule and the key-split workspace.
 static int upload_schedule(sra_ctx* ctx) {
   const sra_config& c = ctx->cfg;
-  cudaFree(ctx->d_fwd_items); cudaFree(ctx->d_bwd_items); cudaFree(ctx->d_split_items);
+  cudaFree(ctx->d_fwd_items); cudaFree(ctx->d_bwd_items); cudaFree(ctx->d_split_items); cudaFree(ctx->d_pair_items);
+  ctx->d_pair_items = nullptr;
   cudaFree(ctx->ws_part_o); cudaFree(ctx->ws_part_lse);
   cudaFree(ctx->d_seg_items); ctx->d_seg_items = nullptr;  // derived from fwd_items; rebuilt lazily by sra_forward_host
   ctx->d_fwd_items = nullptr; ctx->d_bwd_items = nullptr; ctx->d_split_items = nullptr;
   ctx->ws_part_o = nullptr; ctx->ws_part_lse = nullptr;
   cudaError_t e = cudaMalloc(&ctx->d_fwd_items, ctx->fwd_items.size() * sizeof(FwdItem));
   if (e == cudaSuccess) e = cudaMemcpy(ctx->d_fwd_items, ctx->fwd_items.data(), ctx->fwd_items.size() * sizeof(FwdItem), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess && ctx->use_pairs) {
+    e = cudaMalloc(&ctx->d_pair_items, ctx->pair_items.size() * sizeof(FwdItem));
+    if (e == cudaSuccess) e = cudaMemcpy(ctx->d_pair_items, ctx->pair_items.data(), ctx->pair_items.size() * sizeof(FwdItem), cudaMemcpyHostToDevice);
+  }
   if (e == cudaSuccess && ctx->n_split > 1) {
     const size_t prow = size_t(ctx->n_split) * c.batch * c.heads * c.n_gen;
     e = cudaMalloc(&ctx->d_split_items, ctx->split_items.size() * sizeof(FwdItem));
@@ -451,6 +483,7 @@ void sra_destroy(sra_ctx* ctx) {
     cudaFree(ctx->d_fwd_items);
     cudaFree(ctx->d_bwd_items);
     cudaFree(ctx->d_split_items);
+    cudaFree(ctx->d_pair_items);
     cudaFree(ctx->ws_part_o);
     cudaFree(ctx->ws_part_lse);
     cudaFree(ctx->d_seg_items);
@@ -613,20 +646,24 @@ static int forward_core(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) 
   const int B = c.batch, H = c.heads, d = c.head_dim;
   int rc;
   if ((rc = sra::make_tmap_bf16(ctx, &maps[0], a->q_gen, B, c.n_gen, H, d, false, kTile))) return rc;
-  if ((rc = sra::make_tmap_bf16(ctx, &maps[1], a->k_gen, B, c.n_gen, H, d, false, kTile))) return rc;
+  // CTA pairs: each CTA loads 64 of a K tile's 128 keys (box of 64 rows); V shares are ordinary [128 x 64] boxes
+  const bool pairs = ctx->use_pairs;
+  const int k_box = pairs ? kTile / 2 : kTile;
+  if ((rc = sra::make_tmap_bf16(ctx, &maps[1], a->k_gen, B, c.n_gen, H, d, false, k_box))) return rc;
   if ((rc = sra::make_tmap_bf16(ctx, &maps[2], a->v_gen, B, c.n_gen, H, d, false, kTile))) return rc;
   maps[3] = maps[0]; maps[4] = maps[1]; maps[5] = maps[2];  // placeholders when n_ref == 0 (never dereferenced)
   if (nr > 0) {
     if (with_ref_rows && (rc = sra::make_tmap_bf16(ctx, &maps[3], a->q_ref, B, nr, H, d, false, kTile))) return rc;
     const void* kr = use_cache ? ctx->cache_k : a->k_ref;
     const void* vr = use_cache ? ctx->cache_v : a->v_ref;
-    if ((rc = sra::make_tmap_bf16(ctx, &maps[4], kr, B, nr, H, d, use_cache, kTile))) return rc;
+    if ((rc = sra::make_tmap_bf16(ctx, &maps[4], kr, B, nr, H, d, use_cache, k_box))) return rc;
     if ((rc = sra::make_tmap_bf16(ctx, &maps[5], vr, B, nr, H, d, use_cache, kTile))) return rc;
   }
   sra::FwdParams p{};
   const bool split = ctx->n_split > 1;
-  p.items = split ? ctx->d_split_items : ctx->d_fwd_items;
-  p.n_items = ctx->n_gen_items * ctx->n_split + (with_ref_rows ? ctx->n_ref_items : 0);
+  p.items = split ? ctx->d_split_items : pairs ? ctx->d_pair_items : ctx->d_fwd_items;
+  p.n_items = pairs ? ctx->n_gen_pairs + (with_ref_rows ? ctx->n_ref_pairs : 0)
+                    : ctx->n_gen_items * ctx->n_split + (with_ref_rows ? ctx->n_ref_items : 0);
   p.part_o = ctx->ws_part_o;
   p.part_lse = ctx->ws_part_lse;
   const bool seg = ctx->sub_items != nullptr;  // segment-split items of the pipelined host path (merged by its caller)
@@ -636,9 +673,18 @@ static int forward_core(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) 
     p.part_lse = ctx->ws_seg_lse;
   }
   if (ctx->sub_count >= 0) {  // sra_forward_host pipelines a step as several launches over item sub-ranges
-    p.items += ctx->sub_first;
-    p.n_items = ctx->sub_count;
-    if (p.n_items == 0) return SRA_OK;
+    // the range is given in 256-row slabs (indices into fwd_items, or into the [A ; B] segment list of the generation
+    // slabs); with pairs it starts and ends on pair boundaries (the caller snaps its chunks) and is converted
+    int first = ctx->sub_first, end = ctx->sub_first + ctx->sub_count;
+    if (pairs) {
+      const int G = ctx->n_gen_items;
+      auto pi = [&](int idx) { return seg && idx >= G ? ctx->n_gen_pairs + ctx->pair_of_item[idx - G] : int(ctx->pair_of_item[idx]); };
+      first = pi(first);
+      end = pi(end);
+    }
+    p.items += first;
+    p.n_items = end - first;
+    if (p.n_items <= 0) return SRA_OK;
   }
   p.heads = H; p.batch = B; p.n_gen = c.n_gen; p.n_ref = nr;
   p.scale = ctx->scale;
@@ -651,8 +697,9 @@ static int forward_core(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) 
   cudaError_t e;
   {
     sra::KernelTimer kt(ctx, SRA_KERNEL_FWD, cudaStream_t(cuda_stream));
-    e = (d == 128) ? sra::launch_fwd<128>(maps, p, cudaStream_t(cuda_stream))
-                   : sra::launch_fwd<64>(maps, p, cudaStream_t(cuda_stream));
+    e = pairs ? sra::launch_fwd<128, 2>(maps, p, cudaStream_t(cuda_stream))
+        : (d == 128) ? sra::launch_fwd<128, 1>(maps, p, cudaStream_t(cuda_stream))
+                     : sra::launch_fwd<64, 1>(maps, p, cudaStream_t(cuda_stream));
   }
   if (e != cudaSuccess) return fail_cuda(ctx, e, "sra_fwd_kernel launch");
   ctx->launches += 1;
@@ -698,12 +745,15 @@ static int forward_host_pipelined(sra_ctx* ctx, const sra_fwd_host_args* a, cuda
   }
   const int G = ctx->n_gen_items;
   if (n_first > 0 && !ctx->d_seg_items) {
-    std::vector<sra::FwdItem> seg(2 * size_t(G));
-    for (int g = 0; g < G; ++g) {
-      sra::FwdItem A = ctx->fwd_items[g], Bi = ctx->fwd_items[g];
+    // (with CTA pairs the two lists are built from the generation PAIR items)
+    const std::vector<sra::FwdItem>& src = ctx->use_pairs ? ctx->pair_items : ctx->fwd_items;
+    const int Gs = ctx->use_pairs ? ctx->n_gen_pairs : G;
+    std::vector<sra::FwdItem> seg(2 * size_t(Gs));
+    for (int g = 0; g < Gs; ++g) {
+      sra::FwdItem A = src[g], Bi = src[g];
       A.q_is_ref = 1 << 8; A.seg0_len = 0;                   // partial 0: reference keys only
       Bi.q_is_ref = 2 << 8; Bi.seg1_len = 0;                 // partial 1: generation keys only
-      seg[g] = A; seg[size_t(G) + g] = Bi;
+      seg[g] = A; seg[size_t(Gs) + g] = Bi;
     }
     cudaError_t e = cudaMalloc(&ctx->d_seg_items, seg.size() * sizeof(sra::FwdItem));
     if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->d_seg_items, seg.data(), seg.size() * sizeof(sra::FwdItem), cudaMemcpyHostToDevice, st);
@@ -729,9 +779,14 @@ static int forward_host_pipelined(sra_ctx* ctx, const sra_fwd_host_args* a, cuda
   d.q_gen = ctx->stage[0]; d.k_gen = ctx->stage[1]; d.v_gen = ctx->stage[2]; d.o_gen = ctx->stage[3];
   d.lse_gen = a->lse_gen ? static_cast<float*>(ctx->stage[6]) : nullptr;
   const int per = (G + kChunks - 1) / kChunks;
+  auto chunk_start = [&](int ch) {  // first slab of chunk ch; never the second slab of a CTA pair
+    int i = std::min(ch * per, G);
+    if (ctx->use_pairs && i > 0 && i < G && ctx->pair_of_item[i] == ctx->pair_of_item[i - 1]) ++i;
+    return i;
+  };
   auto rows_of = [&](int ch, int& i0, int& i1, size_t& r0, size_t& r1) {
-    i0 = std::min(ch * per, G);
-    i1 = std::min(i0 + per, G);
+    i0 = chunk_start(ch);
+    i1 = chunk_start(ch + 1);
     // G items are ordered by row and tile [0, n_gen) (with a temporal window they are cut at frame boundaries, so
     // an item is not always kQRowsPerCta rows)
     r0 = i0 < G ? size_t(ctx->fwd_items[i0].q_row0) : size_t(c.n_gen);

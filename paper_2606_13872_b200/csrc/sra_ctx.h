@@ -34,6 +34,14 @@ struct sra_ctx {
   int n_gen_items = 0, n_ref_items = 0;
   std::vector<sra::BwdItem> bwd_items;
   sra::FwdItem* d_fwd_items = nullptr;
+  // CTA-pair launch list (head_dim 128, no key split): consecutive slabs that see the same keys are merged into
+  // 512-row pair items (a slab without such a neighbour stays alone, q_rows <= 256); G pairs first, then R pairs.
+  // pair_of_item[i] = pair holding fwd_items[i]; pair_of_item[n_items] = n_pairs.
+  std::vector<sra::FwdItem> pair_items;
+  std::vector<int32_t> pair_of_item;
+  int n_gen_pairs = 0, n_ref_pairs = 0;
+  sra::FwdItem* d_pair_items = nullptr;
+  bool use_pairs = false;
   // Short-query regime (few G slabs): every G slab is cut into n_split key ranges so that all SMs stream the
   // K/V cache; split_items = the n_gen_items * n_split split slabs followed by the R items.
   int n_split = 1;
@@ -59,7 +67,7 @@ struct sra_ctx {
   // "reference keys first" (sra_forward_host): every G slab once against the reference segment only (A items,
   // needs nothing but Q and the resident cache) and once against the generation segment only (B items), as fp32
   // partials merged per slab range; sub_items != nullptr makes forward_core launch from it (no merge).
-  sra::FwdItem* d_seg_items = nullptr;  // [2 * n_gen_items]: A items, then B items
+  sra::FwdItem* d_seg_items = nullptr;  // [2 * n_gen_items]: A items, then B items (with use_pairs: [2 * n_gen_pairs] pair items)
   float* ws_seg_o = nullptr;            // fp32 [2][B][H][n_gen][d]
   float* ws_seg_lse = nullptr;          // fp32 [2][B][H][n_gen]
   const sra::FwdItem* sub_items = nullptr;
@@ -93,7 +101,7 @@ int make_tmap_bf16(sra_ctx* ctx, CUtensorMap* out, const void* ptr, int B, int N
                    int box_rows);
 template <int D>
 cudaError_t launch_bwd(const CUtensorMap* maps, const BwdParams& p, cudaStream_t stream);
-template <int D>
+template <int D, int CG>
 cudaError_t launch_fwd(const CUtensorMap* maps, const FwdParams& p, cudaStream_t stream);
 cudaError_t launch_fwd_merge(const FwdParams& p, int head_dim, int n_split, cudaStream_t stream, int row0 = 0,
                              int n_rows = -1);  // n_rows < 0: every generation row

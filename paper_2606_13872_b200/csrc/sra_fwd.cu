@@ -14,6 +14,16 @@
 // keys [64, 128) -> columns [64, 96); the PV MMA takes its K steps from there.
 // Masked tiles are never visited: the key-tile loop walks only the item's visible segments;
 // only the last tile of a segment pays for a column mask (n_valid < 128).
+//
+// CG = 2 (head_dim 128, the default wherever two consecutive slabs see the same keys): a CTA PAIR - a cluster of two
+// CTAs on one TPC - works on a 512-row slab (128-row tile t of the slab belongs to CTA t & 1, slot t >> 1) with
+// tcgen05.mma.cta_group::2, M = 256: each MMA drives both SMs' tensor cores, rows [0, 128) of A / D in CTA 0's shared
+// memory / TMEM, rows [128, 256) in CTA 1's.  The B operand is split between the two: CTA r loads keys [64 r, 64 r + 64)
+// of every K tile (QK^T: N = 128 keys) and head-dim columns [64 r, 64 r + 64) of every V tile (PV: N = 128 columns), so
+// each SM pulls HALF of the K/V bytes out of L2 and reads half of the B operand from shared memory; the hardware
+// exchanges the halves inside the TPC.  Only the leader (CTA 0) issues MMAs; its tcgen05.commit is multicast to both
+// CTAs' mbarriers, both CTAs' TMA loads report their bytes to the leader's kv_full barriers, and CTA 1's softmax
+// warps arrive remotely on the leader's p_full barriers.
 #include <algorithm>
 
 #include "ptx.cuh"
@@ -29,44 +39,71 @@ namespace sra {
 #endif
 constexpr int kEmuPairsPer8 = SRA_FWD_EMU;
 
-template <int D>
+template <int D, int CG>
 struct FwdCfg {
-  static constexpr int kTileBytes = kTile * D * 2;          // one Q/K/V tile in smem
+  static_assert(CG == 1 || (CG == 2 && D == 128), "the CTA-pair kernel is built for head_dim 128");
+  static constexpr int kTileBytes = kTile * D * 2;          // one Q tile in smem
+  static constexpr int kStageBytes = kTileBytes / CG;       // this CTA's share of a K or V tile
   static constexpr int kBoxes = D / 64;                      // 64-column (128 B) TMA boxes per tile
-  static constexpr int kBoxBytes = kTile * 128;              // 16 KB
-  static constexpr int kStages = (D == 128) ? 5 : 10;        // K/V ring depth (tiles)
+  static constexpr int kBoxBytes = kTile * 128;              // 16 KB: [128 rows][64 columns]
+  static constexpr int kKRows = kTile / CG;                  // key rows of a K tile held by this CTA
+  static constexpr int kKBoxBytes = kKRows * 128;            // [kKRows][64 columns]
+  static constexpr int kStages = (D == 128) ? 5 * CG : 10;   // K/V ring depth (tiles)
   static constexpr int kNumBars = 1 + 2 * kStages + 6 + 4;
   static constexpr int kXchBytes = 2 * 2 * kTile * 4;       // (slot, half, row) floats swapped by the two threads of a row
-  static constexpr int kSmemBytes = (2 + kStages) * kTileBytes + kNumBars * 8 + 16 + kXchBytes;
+  static constexpr int kSmemBytes = 2 * kTileBytes + kStages * kStageBytes + kNumBars * 8 + 16 + kXchBytes;
   static constexpr int kTmemCols = 512;
   static constexpr int kThreads = 384;
+  static_assert(kSmemBytes <= 232448, "shared memory budget");
 };
 
-template <int D>
+// One 128-row tile of a [.., d] tensor (Q; with CG = 1 also K and V): D / 64 boxes of [128 rows][64 columns].
+template <int D, int CG>
 __device__ __forceinline__ void load_tile(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int row, int h, int b,
                                           bool head_major) {
 #pragma unroll
-  for (int x = 0; x < FwdCfg<D>::kBoxes; ++x) {
-    if (head_major)
-      tma_load_4d(dst + x * FwdCfg<D>::kBoxBytes, tm, bar, x * 64, row, h, b);
-    else
-      tma_load_4d(dst + x * FwdCfg<D>::kBoxBytes, tm, bar, x * 64, h, row, b);
+  for (int x = 0; x < D / 64; ++x) {
+    const uint32_t dx = dst + x * FwdCfg<D, CG>::kBoxBytes;
+    if (CG == 1) {
+      if (head_major) tma_load_4d(dx, tm, bar, x * 64, row, h, b); else tma_load_4d(dx, tm, bar, x * 64, h, row, b);
+    } else {
+      if (head_major) tma_load_4d_pair(dx, tm, bar, x * 64, row, h, b); else tma_load_4d_pair(dx, tm, bar, x * 64, h, row, b);
+    }
   }
 }
-
+// CTA-pair shares of a key tile.  K (B operand of QK^T, N = keys): this CTA's 64 keys, all of d, as two
+// [64 rows][64 columns] boxes (the tensor map's box is 64 rows).  V (B operand of PV, N = head-dim columns): all
+// 128 keys, this CTA's 64 columns - one ordinary [128 rows][64 columns] box.
 template <int D>
-__global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
+__device__ __forceinline__ void load_k_half(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int row, int h, int b,
+                                            bool head_major, int rank) {
+#pragma unroll
+  for (int x = 0; x < D / 64; ++x) {
+    const uint32_t dx = dst + x * FwdCfg<D, 2>::kKBoxBytes;
+    if (head_major) tma_load_4d_pair(dx, tm, bar, x * 64, row + 64 * rank, h, b);
+    else tma_load_4d_pair(dx, tm, bar, x * 64, h, row + 64 * rank, b);
+  }
+}
+template <int D>
+__device__ __forceinline__ void load_v_half(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int row, int h, int b,
+                                            bool head_major, int rank) {
+  if (head_major) tma_load_4d_pair(dst, tm, bar, 64 * rank, row, h, b);
+  else tma_load_4d_pair(dst, tm, bar, 64 * rank, h, row, b);
+}
+
+template <int D, int CG>
+__global__ void __launch_bounds__(FwdCfg<D, CG>::kThreads, 1)
     sra_fwd_kernel(const __grid_constant__ CUtensorMap tm_q_gen, const __grid_constant__ CUtensorMap tm_k_gen,
                    const __grid_constant__ CUtensorMap tm_v_gen, const __grid_constant__ CUtensorMap tm_q_ref,
                    const __grid_constant__ CUtensorMap tm_k_ref, const __grid_constant__ CUtensorMap tm_v_ref,
                    const FwdParams p) {
-  using C = FwdCfg<D>;
+  using C = FwdCfg<D, CG>;
   extern __shared__ __align__(1024) uint8_t smem_raw[];  // 128-byte-swizzled tiles need 1024-byte alignment
   const uint32_t smem_base = smem_u32(smem_raw);
   if ((smem_base & 1023u) != 0) __trap();
   const uint32_t sQ = smem_base;                         // 2 tiles
   const uint32_t sKV = smem_base + 2 * C::kTileBytes;    // kStages tiles
-  const uint32_t sBar = sKV + C::kStages * C::kTileBytes;
+  const uint32_t sBar = sKV + C::kStages * C::kStageBytes;
   const uint32_t bar_q_full = sBar;
   const uint32_t bar_kv_full = sBar + 8;
   const uint32_t bar_kv_empty = bar_kv_full + 8 * C::kStages;
@@ -81,7 +118,9 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
 
-  const FwdItem item = p.items[blockIdx.x];
+  // CG = 2: blockIdx.x = 2 * (pair item) + rank; 128-row tile t of the pair's slab belongs to CTA t & 1, slot t >> 1
+  const int rank = CG == 2 ? int(cluster_ctarank()) : 0;
+  const FwdItem item = p.items[CG == 2 ? blockIdx.x >> 1 : blockIdx.x];
   const bool q_is_ref = (item.q_is_ref & 1) != 0;
   const int split = item.q_is_ref >> 8;  // 0: final output; s + 1: key split s of a short-query G slab
   const int h = blockIdx.y;
@@ -89,7 +128,8 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
   const int n0 = (item.seg0_len + kTile - 1) / kTile;
   const int n1 = (item.seg1_len + kTile - 1) / kTile;
   const int n_kv = n0 + n1;
-  const int n_qt = item.q_rows > kTile ? 2 : 1;  // Q tiles that hold at least one valid row
+  const int n_qt = item.q_rows > kTile * CG ? 2 : 1;  // Q tile slots in use (the same in both CTAs of a pair)
+  auto slot_row = [&](int i) { return (CG * i + rank) * kTile; };  // first slab row of this CTA's Q tile slot i
 
   if (threadIdx.x == 0) {
     mbar_init(bar_q_full, 1);
@@ -99,7 +139,7 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
     }
     for (int i = 0; i < 2; ++i) {
       mbar_init(bar_s_full + 8 * i, 1);
-      mbar_init(bar_p_full + 8 * i, 8);  // one elected arrive per softmax warp
+      mbar_init(bar_p_full + 8 * i, 8 * CG);  // one elected arrive per softmax warp (of both CTAs of a pair)
       mbar_init(bar_o_full + 8 * i, 1);
     }
     for (int g = 0; g < 4; ++g) mbar_init(bar_x + 8 * g, 2);  // one elected arrive per warp of the pair
@@ -110,10 +150,12 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
     tma_prefetch_desc(item.seg0_is_ref ? &tm_k_ref : &tm_k_gen);
     tma_prefetch_desc(item.seg0_is_ref ? &tm_v_ref : &tm_v_gen);
   }
-  if (warp == 8) tmem_alloc(s_tmem_ptr, C::kTmemCols);
+  if (warp == 8) tmem_alloc<CG>(s_tmem_ptr, C::kTmemCols);
   tc_fence_before();
-  __syncthreads();
+  if (CG == 2) cluster_sync(); else __syncthreads();  // (pair: the peer's mbarriers are initialised before anything signals them)
   tc_fence_after();
+  // p_full lives in the leader CTA (its MMA thread waits for the P tiles of both CTAs)
+  const uint32_t bar_p_full_leader = CG == 2 ? mapa_cluster(bar_p_full, 0) : bar_p_full;
   const uint32_t tmem = *tmem_ptr_generic;
   const uint32_t tS0 = tmem, tO0 = tmem + 256;
 
@@ -187,6 +229,7 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
           };
           mbar_wait(bar_s_full + 8 * i, j & 1);
           tc_fence_after();
+#ifndef SRA_FWD_SKEL  // (ablation builds only: MMAs, TMA and barriers without the softmax arithmetic; results are wrong)
           // s_full(j) completed => every earlier MMA, including O_i += P_i V_{j-1}, is complete.
           if (j > 0 && __any_sync(0xffffffffu, (m_seen[i] - m_ref[i]) * sl2 > 8.0f)) rescale_to(fmaxf(m_ref[i], m_seen[i]));
           uint32_t pk[2][16];
@@ -268,9 +311,12 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
 #pragma unroll
           for (int c = 0; c < 2; ++c) tmem_st16(tS + hh * 64 + c * 16, pk[c]);
           tmem_wait_st();
+#endif
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive(bar_p_full + 8 * i);
+          if (lane == 0) {
+            if (CG == 2) mbar_arrive_cluster(bar_p_full_leader + 8 * i); else mbar_arrive(bar_p_full + 8 * i);
+          }
         }
       }
     }
@@ -283,7 +329,7 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
         tc_fence_after();
         post(l[i]);
         const float l_row = l[i] + fetch();
-        const int row = i * kTile + row_in_tile;
+        const int row = slot_row(i) + row_in_tile;
         const bool valid = row < item.q_rows;
         const int n_tok = q_is_ref ? p.n_ref : p.n_gen;
         const int grow = item.q_row0 + row;
@@ -335,9 +381,13 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
     reg_dec<56>();
     if (warp == 9 && elect_one()) {
       // ===================================================== TMA loader
+      // Pair: every load of either CTA reports its bytes to the LEADER's barriers (the leader's MMA thread is the
+      // only consumer); the leader alone arrives, expecting the bytes of both CTAs.
       const CUtensorMap* tq = q_is_ref ? &tm_q_ref : &tm_q_gen;
-      mbar_arrive_expect_tx(bar_q_full, n_qt * C::kTileBytes);
-      for (int i = 0; i < n_qt; ++i) load_tile<D>(sQ + i * C::kTileBytes, tq, bar_q_full, item.q_row0 + i * kTile, h, b, false);
+      const uint32_t q_full_l = CG == 2 ? mapa_cluster(bar_q_full, 0) : bar_q_full;
+      const uint32_t kv_full_l = CG == 2 ? mapa_cluster(bar_kv_full, 0) : bar_kv_full;
+      if (rank == 0) mbar_arrive_expect_tx(bar_q_full, n_qt * C::kTileBytes * CG);
+      for (int i = 0; i < n_qt; ++i) load_tile<D, CG>(sQ + i * C::kTileBytes, tq, q_full_l, item.q_row0 + slot_row(i), h, b, false);
       int it = 0;
       for (int j = 0; j < n_kv; ++j) {
         const bool first = j < n0;
@@ -350,32 +400,39 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
           const uint32_t ph = (it / C::kStages) & 1;
           const CUtensorMap* tm = kv == 0 ? (is_ref ? &tm_k_ref : &tm_k_gen) : (is_ref ? &tm_v_ref : &tm_v_gen);
           mbar_wait(bar_kv_empty + 8 * s, ph ^ 1);
-          mbar_arrive_expect_tx(bar_kv_full + 8 * s, C::kTileBytes);
-          load_tile<D>(sKV + s * C::kTileBytes, tm, bar_kv_full + 8 * s, row, h, b, hm);
+          if (rank == 0) mbar_arrive_expect_tx(bar_kv_full + 8 * s, C::kTileBytes);
+          const uint32_t dst = sKV + s * C::kStageBytes;
+          if constexpr (CG == 1) {
+            load_tile<D, 1>(dst, tm, kv_full_l + 8 * s, row, h, b, hm);
+          } else {
+            if (kv == 0) load_k_half<D>(dst, tm, kv_full_l + 8 * s, row, h, b, hm, rank);
+            else load_v_half<D>(dst, tm, kv_full_l + 8 * s, row, h, b, hm, rank);
+          }
         }
       }
-    } else if (warp == 8 && elect_one()) {
-      // ===================================================== MMA issuer
-      constexpr uint32_t idesc_qk = make_idesc_bf16(kTile, kTile, 0, 0);
-      constexpr uint32_t idesc_pv = make_idesc_bf16(kTile, D, 0, 1);
+    } else if (warp == 8 && rank == 0 && elect_one()) {
+      // ===================================================== MMA issuer (pair: the leader CTA only, M = 256)
+      constexpr uint32_t idesc_qk = make_idesc_bf16(kTile * CG, kTile, 0, 0);
+      constexpr uint32_t idesc_pv = make_idesc_bf16(kTile * CG, D, 0, 1);
       // Descriptor low words: Q/K tiles are K-major (LBO unused), V is MN-major (LBO = one 64-column box).
       constexpr uint32_t kDescHi = desc_hi_sw128(1024);
-      constexpr uint32_t kStageStep = C::kTileBytes >> 4;
+      constexpr uint32_t kQStep = C::kTileBytes >> 4, kStageStep = C::kStageBytes >> 4;
       const uint32_t q_lo = desc_lo(sQ, 16), k_lo = desc_lo(sKV, 16), v_lo = desc_lo(sKV, C::kBoxBytes);
       auto issue_qk = [&](int i, int stage) {
-        const uint32_t q = q_lo + i * kStageStep, k = k_lo + stage * kStageStep;
+        const uint32_t q = q_lo + i * kQStep, k = k_lo + stage * kStageStep;
 #pragma unroll
         for (int kk = 0; kk < D / 16; ++kk) {
-          const uint32_t off = ((kk / 4) * C::kBoxBytes + (kk % 4) * 32) >> 4;
-          umma_ss(tS0 + i * 128, desc64(q + off, kDescHi), desc64(k + off, kDescHi), idesc_qk, kk > 0);
+          const uint32_t qoff = ((kk / 4) * C::kBoxBytes + (kk % 4) * 32) >> 4;
+          const uint32_t koff = ((kk / 4) * C::kKBoxBytes + (kk % 4) * 32) >> 4;
+          umma_ss<CG>(tS0 + i * 128, desc64(q + qoff, kDescHi), desc64(k + koff, kDescHi), idesc_qk, kk > 0);
         }
       };
       auto issue_pv = [&](int i, int stage, bool acc) {
         const uint32_t v = v_lo + stage * kStageStep;
 #pragma unroll
         for (int kk = 0; kk < kTile / 16; ++kk)
-          umma_ts(tO0 + i * D, tS0 + i * 128 + (kk / 4) * 64 + (kk % 4) * 8, desc64(v + kk * (2048 >> 4), kDescHi), idesc_pv,
-                  (acc || kk > 0) ? 1u : 0u);
+          umma_ts<CG>(tO0 + i * D, tS0 + i * 128 + (kk / 4) * 64 + (kk % 4) * 8, desc64(v + kk * (2048 >> 4), kDescHi), idesc_pv,
+                      (acc || kk > 0) ? 1u : 0u);
       };
       auto stage_of = [&](int it) { return it % C::kStages; };
       auto phase_of = [&](int it) { return uint32_t((it / C::kStages) & 1); };
@@ -386,9 +443,9 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
       tc_fence_after();
       for (int i = 0; i < n_qt; ++i) {
         issue_qk(i, stage_of(it));
-        umma_commit(bar_s_full + 8 * i);
+        umma_commit<CG>(bar_s_full + 8 * i);
       }
-      umma_commit(bar_kv_empty + 8 * stage_of(it));
+      umma_commit<CG>(bar_kv_empty + 8 * stage_of(it));
       ++it;
       for (int j = 0; j < n_kv; ++j) {
         const int sv = stage_of(it);
@@ -397,44 +454,64 @@ __global__ void __launch_bounds__(FwdCfg<D>::kThreads, 1)
         const bool more = j + 1 < n_kv;
         const int sk = stage_of(it);
         for (int i = 0; i < n_qt; ++i) {
-          mbar_wait(bar_p_full + 8 * i, j & 1);
+          if (CG == 2) mbar_wait_cluster(bar_p_full + 8 * i, j & 1); else mbar_wait(bar_p_full + 8 * i, j & 1);
           tc_fence_after();
           issue_pv(i, sv, j > 0);
-          if (!more) umma_commit(bar_o_full + 8 * i);
-          if (i == n_qt - 1) umma_commit(bar_kv_empty + 8 * sv);
+          if (!more) umma_commit<CG>(bar_o_full + 8 * i);
+          if (i == n_qt - 1) umma_commit<CG>(bar_kv_empty + 8 * sv);
           if (more) {
             if (i == 0) {
               mbar_wait(bar_kv_full + 8 * sk, phase_of(it));
               tc_fence_after();
             }
             issue_qk(i, sk);
-            umma_commit(bar_s_full + 8 * i);
-            if (i == n_qt - 1) umma_commit(bar_kv_empty + 8 * sk);
+            umma_commit<CG>(bar_s_full + 8 * i);
+            if (i == n_qt - 1) umma_commit<CG>(bar_kv_empty + 8 * sk);
           }
         }
         if (more) ++it;
       }
     }
   }
-  __syncthreads();
+  // Pair: neither CTA may leave (or free its TMEM) while the other can still read its shared memory / TMEM or signal
+  // its mbarriers.
+  tc_fence_before();
+  if (CG == 2) cluster_sync(); else __syncthreads();
   if (warp == 8) {
     tc_fence_after();
-    tmem_dealloc(tmem, C::kTmemCols);
+    tmem_dealloc<CG>(tmem, C::kTmemCols);
   }
 }
 
-template <int D>
+// The dynamic shared-memory opt-in is a per-device function attribute: remembered per device ordinal.
+static bool* configured_flag(int which) {
+  static bool flags[4][64] = {};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) dev = 0;
+  return &flags[which][dev];
+}
+
+template <int D, int CG>
 cudaError_t launch_fwd(const CUtensorMap* maps, const FwdParams& p, cudaStream_t stream) {
-  using C = FwdCfg<D>;
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(sra_fwd_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes);
+  using C = FwdCfg<D, CG>;
+  bool* configured = configured_flag((D == 128 ? 0 : 1) + 2 * (CG - 1));
+  if (!*configured) {
+    cudaError_t e = cudaFuncSetAttribute(sra_fwd_kernel<D, CG>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes);
     if (e != cudaSuccess) return e;
-    configured = true;
+    *configured = true;
   }
-  dim3 grid(p.n_items, p.heads, p.batch);
-  sra_fwd_kernel<D><<<grid, C::kThreads, C::kSmemBytes, stream>>>(maps[0], maps[1], maps[2], maps[3], maps[4], maps[5], p);
-  return cudaGetLastError();
+  // p.n_items counts launched items: 256-row slabs (CG = 1) or 512-row pair slabs, two CTAs each (CG = 2)
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(p.n_items * CG, p.heads, p.batch);
+  cfg.blockDim = dim3(C::kThreads);
+  cfg.dynamicSmemBytes = C::kSmemBytes;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = CG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = CG == 2 ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, sra_fwd_kernel<D, CG>, maps[0], maps[1], maps[2], maps[3], maps[4], maps[5], p);
 }
 
 // a5' (short-query schedules only): O = sum_s exp(LSE_s - LSE) O_s with LSE = log sum_s exp(LSE_s); one warp per
@@ -500,7 +577,8 @@ cudaError_t launch_fwd_merge(const FwdParams& p, int head_dim, int n_split, cuda
   return cudaGetLastError();
 }
 
-template cudaError_t launch_fwd<64>(const CUtensorMap*, const FwdParams&, cudaStream_t);
-template cudaError_t launch_fwd<128>(const CUtensorMap*, const FwdParams&, cudaStream_t);
+template cudaError_t launch_fwd<64, 1>(const CUtensorMap*, const FwdParams&, cudaStream_t);
+template cudaError_t launch_fwd<128, 1>(const CUtensorMap*, const FwdParams&, cudaStream_t);
+template cudaError_t launch_fwd<128, 2>(const CUtensorMap*, const FwdParams&, cudaStream_t);
 
 }  // namespace sra
