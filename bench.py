@@ -167,29 +167,61 @@ def oracle_sample_rows(w, n_gen_rows, n_ref_rows, seed=0):
     return np.asarray(rows, dtype=np.int32)
 
 
-def sample_flops(w, rows, n_heads):
+def sample_flops(w, rows, n_heads, valid=None, frames=None, window=-1):
+    """Useful FLOPs of the sampled rows: 4 d per visible (query, key) pair under the same mask options the oracle gets."""
+    import bisect
     fl = 0.0
     off = w.ref_block_offsets
+    n_valid = w.n_ref if valid is None else int(sum(1 for v in valid if v))
     for r in rows:
         if r < w.n_gen:
-            vis = w.n_gen + w.n_ref
+            vis = w.n_gen
+            if frames is not None and window >= 0:
+                f = bisect.bisect_right(frames, int(r)) - 1
+                n_fr = len(frames) - 1
+                vis = frames[min(n_fr, f + window + 1)] - frames[max(0, f - window)]
+            vis += n_valid
         else:
             t = r - w.n_gen
             j = max(k for k in range(len(off) - 1) if off[k] <= t)
-            vis = off[j + 1] - off[j]
+            if valid is None:
+                vis = off[j + 1] - off[j]
+            else:
+                vis = int(sum(1 for v in valid[off[j]:off[j + 1]] if v)) if valid[t] else 0
         fl += 4.0 * w.head_dim * vis
     return fl * n_heads * w.batch
 
 
-def run_oracle_sample(w, bits_h, heads, rows):
+def run_oracle_sample(w, bits_h, heads, rows, valid=None, frames=None, window=-1):
     """Times oracle/ (plain C fp64, OpenMP over rows) on `rows` x `heads`.  bits_h: uint16 arrays already
-    restricted to `heads`.  Returns (seconds, o [B, n_rows, len(heads), d], lse)."""
+    restricted to `heads`.  valid / frames + window: the optional mask restrictions, which the
+    oracle materialises in its visibility predicate.  Returns (seconds, o [B, n_rows, len(heads), d], lse)."""
     from oracle import c_oracle
     t0 = time.perf_counter()
     o, lse = c_oracle.forward_rows(bits_h["q_gen"], bits_h["k_gen"], bits_h["v_gen"], bits_h.get("q_ref"),
                                    bits_h.get("k_ref"), bits_h.get("v_ref"), w.ref_block_offsets,
-                                   1.0 / math.sqrt(w.head_dim), rows)
+                                   1.0 / math.sqrt(w.head_dim), rows, valid=valid, gen_frame_offsets=frames,
+                                   window=window if frames is not None else -1)
     return time.perf_counter() - t0, o, lse
+
+
+def parity_record(got, ref, got_lse=None, ref_lse=None):
+    """GPU vs oracle on the same sampled outputs: the contract gates + rel_l2; empty rows (invalid reference tokens:
+    O = 0, LSE = -inf on both sides) are compared as such."""
+    import numpy as np
+    diff = np.abs(got - ref)
+    rel_l2 = float(np.linalg.norm(got - ref) / max(np.linalg.norm(ref), 1e-300))
+    rec = {"max_abs": float(diff.max()), "mean_abs": float(diff.mean()), "rel_l2": rel_l2,
+           "tolerance": {"max_abs": MAX_ABS_TOL, "mean_abs": MEAN_ABS_TOL, "rel_l2": REL_L2_TOL}}
+    ok = bool(diff.max() <= MAX_ABS_TOL and diff.mean() <= MEAN_ABS_TOL and rel_l2 <= REL_L2_TOL and np.isfinite(got).all())
+    if got_lse is not None:
+        empty = np.isneginf(ref_lse)
+        same_empty = bool(np.array_equal(np.isneginf(got_lse), empty))
+        rec["lse_max_abs"] = float(np.abs(got_lse[~empty] - ref_lse[~empty]).max()) if (~empty).any() else 0.0
+        rec["empty_rows"] = int(empty.sum())
+        ok = ok and same_empty and rec["lse_max_abs"] <= 2e-3
+    rec["ok"] = ok
+    return rec
 
 
 def bench_reference(args, w):
@@ -264,9 +296,19 @@ def bench_ours(args, w):
         dist.init_process_group("nccl", device_id=dev)
     peaks, peaks_kind = load_peaks()
 
-    # weak scaling: this rank owns global batch items [b0, b0 + w.batch)
+    # weak scaling (default): this rank owns global batch items [b0, b0 + w.batch).
+    # --shard heads (strong scaling of a B = 1 config; what Ulysses SP leaves each GPU with,
+    # PAPER.md:231): the job is ONE item, rank r owns a contiguous slice of its heads - still no data-path collective.
     b0, _ = dp.shard_batch(w.batch, world, rank)
     seed_off = dp.unit_seed(0, b0)
+    scaling = "weak"
+    if args.shard == "heads":
+        h0, hn = dp.shard_heads(w.heads, world, rank)
+        if hn == 0:
+            raise SystemExit(f"bench.py --shard heads: rank {rank} of {world} owns no head of {w.heads}")
+        w = w.replace(heads=hn)
+        seed_off = 7919 * h0  # (synthetic data: each head slice is drawn on its own)
+        scaling = "strong"
     names = ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref") if w.n_ref else ("q_gen", "k_gen", "v_gen")
     t = {n: I.make_tensor_device(w, n, dev, seed_offset=seed_off) for n in names}
     o_gen = torch.empty_like(t["q_gen"])
@@ -276,20 +318,19 @@ def bench_ours(args, w):
     ctx = B.sra_create(w.batch, w.heads, w.head_dim, w.n_gen, w.ref_block_offsets)
     fl = useful_flops(w)
     assert abs(B.sra_useful_flops(ctx, True) - fl) <= 1e-6 * fl
+    valid = frames = None
     if args.window >= 0:
         # refiner-style sparse temporal attention: 21 latent frames, generation keys of frames within
-        # the window only.  Parity for this path is in tests/test_gpu_temporal.py (numpy oracle).
+        # the window only; the C oracle applies the same frame rule in its visibility predicate
         n_frames = 21 if w.n_gen % 21 == 0 else 1
-        B.sra_set_temporal_window(ctx, [i * (w.n_gen // n_frames) for i in range(n_frames + 1)], args.window)
+        frames = [i * (w.n_gen // n_frames) for i in range(n_frames + 1)]
+        B.sra_set_temporal_window(ctx, frames, args.window)
         fl = B.sra_useful_flops(ctx, True)
-        args.no_oracle = True
     if args.invalid_frac > 0 and w.n_ref:
-        # sparse validity masking: a seeded per-token mask; useful FLOPs follow the valid tokens only.
-        # Parity for this path is in tests/test_gpu_validity.py (numpy oracle); the C-oracle legs are skipped here.
+        # sparse validity masking: a seeded per-token mask; useful FLOPs follow the valid tokens only
         valid = np.random.default_rng(w.seed).random(w.n_ref) >= args.invalid_frac
         B.sra_set_reference_validity(ctx, valid)
         fl = B.sra_useful_flops(ctx, True)
-        args.no_oracle = True
 
     def step():
         if w.n_ref:
@@ -388,8 +429,8 @@ def bench_ours(args, w):
         rows = oracle_sample_rows(w, args.oracle_rows, max(2, args.oracle_rows // 4))
         bits_h = {n: I.bf16_bits(t[n][:, :, heads].contiguous().cpu()) for n in names}
         wh = w.replace(heads=len(heads))
-        dt, o_or, lse_or = run_oracle_sample(wh, bits_h, heads, rows)
-        sfl = sample_flops(w, rows, len(heads))
+        dt, o_or, lse_or = run_oracle_sample(wh, bits_h, heads, rows, valid, frames, args.window)
+        sfl = sample_flops(w, rows, len(heads), valid, frames, args.window)
         sample = (f"{len(rows)} query rows ({int((rows < w.n_gen).sum())} G + {int((rows >= w.n_gen).sum())} R) x heads {heads} "
                   f"of the same {w.name} inputs, all visible keys; {sfl / 1e9:.1f} GFLOP fp64 in {dt:.1f} s")
         cpu_baseline = {"value": sfl / dt / 1e12, "unit": UNIT, "cores": c_oracle.num_threads(), "kind": "oracle",
@@ -404,25 +445,15 @@ def bench_ours(args, w):
             got_lse.append(lse_ref[:, heads][:, :, torch.as_tensor(r_rows, device=dev).long()].cpu().numpy())
         got = np.concatenate(got, axis=1).astype(np.float64)
         got_lse = np.concatenate(got_lse, axis=2).astype(np.float64)
-        diff = np.abs(got - o_or)
-        rel_l2 = float(np.linalg.norm(got - o_or) / max(np.linalg.norm(o_or), 1e-300))
-        parity = {"max_abs": float(diff.max()), "mean_abs": float(diff.mean()), "rel_l2": rel_l2,
-                  "lse_max_abs": float(np.abs(got_lse - lse_or).max()),
-                  "tolerance": {"max_abs": MAX_ABS_TOL, "mean_abs": MEAN_ABS_TOL, "rel_l2": REL_L2_TOL},
-                  "ok": bool(diff.max() <= MAX_ABS_TOL and diff.mean() <= MEAN_ABS_TOL and rel_l2 <= REL_L2_TOL
-                             and np.isfinite(got).all()),
-                  "rows": int(len(rows)), "heads": heads}
+        parity = parity_record(got, o_or, got_lse, lse_or)
+        parity.update(rows=int(len(rows)), heads=heads)
         if e2e_out is not None and e2e is not None and e2e.get("value") is not None:
             # the same sampled rows of what sra_forward_host returned, against the same oracle values
             hg = [e2e_out[0][:, torch.as_tensor(g_rows).long()][:, :, heads].float().numpy()]
             if len(r_rows) and e2e_out[1] is not None:
                 hg.append(e2e_out[1][:, torch.as_tensor(r_rows).long()][:, :, heads].float().numpy())
             hg = np.concatenate(hg, axis=1).astype(np.float64)
-            hd = np.abs(hg - o_or)
-            h_rel = float(np.linalg.norm(hg - o_or) / max(np.linalg.norm(o_or), 1e-300))
-            e2e["parity"] = {"max_abs": float(hd.max()), "mean_abs": float(hd.mean()), "rel_l2": h_rel,
-                             "ok": bool(hd.max() <= MAX_ABS_TOL and hd.mean() <= MEAN_ABS_TOL and h_rel <= REL_L2_TOL
-                                        and np.isfinite(hg).all())}
+            e2e["parity"] = parity_record(hg, o_or)
     e2e_out = None
 
     B.sra_destroy(ctx)
@@ -430,6 +461,20 @@ def bench_ours(args, w):
         if world > 1:
             dist.destroy_process_group()
         return
+    # ---- legs (N == 1, the default 720p line only): the rest of SURVEY.md 8 on the same line, same run
+    legs = None
+    if world == 1 and args.legs and w.name == "720p" and args.window < 0 and args.invalid_frac == 0:
+        del t, o_gen, o_ref, lse_gen, lse_ref
+        torch.cuda.empty_cache()
+        legs = {}
+        for name, fn in (("denoise8", lambda: leg_denoise8(args, w, dev, peaks, peaks_kind)),
+                         ("train", lambda: leg_train(args)), ("short128", lambda: leg_short(args))):
+            try:
+                legs[name] = fn()
+            except Exception as ex:  # a failed leg is reported, never hidden
+                log(f"leg {name} failed: {ex!r}")
+                legs[name] = {"error": repr(ex)}
+            torch.cuda.empty_cache()
     k_ms = statistics.mean(kernel_ms)
     achieved = fl / (k_ms * 1e-3) / 1e12
     peak = peaks["bf16_tflops_sustained"]
@@ -444,9 +489,11 @@ def bench_ours(args, w):
     }
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": scaling, "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
-        "config": config_of(w, args, {**({"invalid_ref_frac": args.invalid_frac} if args.invalid_frac > 0 else {}),
+        "config": config_of(w, args, {**({"parallelism": f"heads{world} (one item, {w.heads} heads per rank, no collective)",
+                                          "global_batch": w.batch} if scaling == "strong" else {}),
+                                      **({"invalid_ref_frac": args.invalid_frac} if args.invalid_frac > 0 else {}),
                                       **({"temporal_window_frames": args.window} if args.window >= 0 else {})} or None),
         "pct_of_peak": {"measured_sustained": 100 * value / world / peaks["bf16_tflops_sustained"],
                         "measured_burst": 100 * value / world / peaks["bf16_tflops"],
@@ -455,12 +502,106 @@ def bench_ours(args, w):
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
         "cpu_baseline": cpu_baseline, "parity": parity,
     }
+    if legs is not None:
+        out["legs"] = legs
     emit(out)
     if world > 1:
         dist.destroy_process_group()
 
 
-def bench_train(args, w):
+def leg_denoise8(args, w, dev, peaks, peaks_kind):
+    """BASELINE.json configs[2] as written ("reuse cached ref KV over 8 denoising steps") with the
+    protocol of SURVEY.md 8d: step 0 = sra_cache_reference_kv + sra_forward over G and R rows; steps 1-7 = cached
+    steps (q_ref = k_ref = v_ref = NULL: G rows only, reference K/V from the resident cache), FRESH generation
+    tensors every step (seed + 1000 * step).  Every step is bracketed by CUDA events on the launching stream."""
+    import numpy as np
+    import torch
+    from paper_2606_13872_b200 import binding as B
+    from paper_2606_13872_b200 import inputs as I
+    n_steps = 8
+    ref = {n: I.make_tensor_device(w, n, dev) for n in ("q_ref", "k_ref", "v_ref")}
+    gens = [{n: I.make_tensor_device(w, n, dev, step=s) for n in ("q_gen", "k_gen", "v_gen")} for s in range(n_steps)]
+    o_gen = torch.empty_like(gens[0]["q_gen"])
+    o_ref = torch.empty_like(ref["q_ref"])
+    lse_gen = torch.empty((w.batch, w.heads, w.n_gen), device=dev, dtype=torch.float32)
+    ctx = B.sra_create(w.batch, w.heads, w.head_dim, w.n_gen, w.ref_block_offsets)
+    fl0, flc = B.sra_useful_flops(ctx, True), B.sra_useful_flops(ctx, False)
+
+    def run(s):
+        g = gens[s]
+        if s == 0:
+            B.sra_cache_reference_kv(ctx, ref["k_ref"], ref["v_ref"])
+            B.sra_forward(ctx, g["q_gen"], g["k_gen"], g["v_gen"], o_gen, q_ref=ref["q_ref"], o_ref=o_ref, lse_gen=lse_gen)
+        else:
+            B.sra_forward(ctx, g["q_gen"], g["k_gen"], g["v_gen"], o_gen, lse_gen=lse_gen)
+
+    for s in (0, 1, 2):  # warm-up: a full step and two cached steps
+        run(s)
+    torch.cuda.synchronize()
+    cache_bytes = B.sra_cache_bytes(ctx)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(n_steps + 1)]
+    launches = []
+    ev[0].record()
+    for s in range(n_steps):
+        l0 = B.sra_launch_count(ctx)
+        run(s)
+        ev[s + 1].record()
+        launches.append(B.sra_launch_count(ctx) - l0)
+    torch.cuda.synchronize()
+    ms = [ev[s].elapsed_time(ev[s + 1]) for s in range(n_steps)]
+    # parity of the LAST cached step (fresh tensors of step 7, resident cache) on sampled generation rows
+    from oracle import c_oracle
+    c_oracle.build()
+    heads = [0, w.heads - 1]
+    rows = oracle_sample_rows(w, 96, 0)
+    g = gens[n_steps - 1]
+    bits_h = {n: I.bf16_bits(x[:, :, heads].contiguous().cpu()) for n, x in {**g, **ref}.items()}
+    _, o_or, lse_or = run_oracle_sample(w.replace(heads=len(heads)), bits_h, heads, rows)
+    idx = torch.as_tensor(rows, device=dev).long()
+    got = o_gen[:, idx][:, :, heads].float().cpu().numpy().astype(np.float64)
+    got_lse = lse_gen[:, heads][:, :, idx].cpu().numpy().astype(np.float64)
+    parity = parity_record(got, o_or, got_lse, lse_or)
+    parity.update(rows=int(len(rows)), heads=heads, step=n_steps - 1)
+    same_cache = B.sra_cache_bytes(ctx) == cache_bytes
+    B.sra_destroy(ctx)
+    cached = ms[1:]
+    peak = peaks["bf16_tflops_sustained"]
+    return {
+        "workload": w.name, "protocol": "step 0 = cache build + G and R rows; steps 1-7 = cached (q_ref NULL), fresh G tensors per step",
+        "step0_ms": ms[0], "cached_step_ms": cached, "cached_step_ms_mean": statistics.mean(cached),
+        "mean_ms_over_8_steps": statistics.mean(ms), "launches_per_step": launches,
+        "cache_bytes": int(cache_bytes), "cache_unchanged_over_cached_steps": bool(same_cache),
+        "step0_useful_tflops": fl0 / (ms[0] * 1e-3) / 1e12,
+        "cached_step_useful_tflops": flc / (statistics.mean(cached) * 1e-3) / 1e12,
+        "cached_step_frac_of_sustained_peak": flc / (statistics.mean(cached) * 1e-3) / 1e12 / peak,
+        "useful_tflops_over_8_steps": (fl0 + 7 * flc) / (sum(ms) * 1e-3) / 1e12,
+        "peak": peak, "peak_kind": f"{peaks_kind} cuBLAS bf16, sustained", "parity": parity,
+    }
+
+
+def leg_train(args):
+    """BASELINE.json configs[4] (rows a6-a8): the --mode train measurement, shortened, with its oracle check."""
+    from paper_2606_13872_b200 import inputs as I
+    a = argparse.Namespace(**{**vars(args), "steps": 4, "warmup": 3, "train_parity": not args.no_oracle})
+    out = bench_train(a, I.WORKLOADS["train"], emit_line=False)
+    keep = ("metric", "value", "unit", "ms_per_step", "steps", "warmup", "gpu_launches", "clocks", "roofline", "parity")
+    leg = {k: out[k] for k in keep}
+    leg["workload"] = out["config"]["workload"]
+    return leg
+
+
+def leg_short(args):
+    """north_star's cache-bound short-query case (128 rows against the 40 s cache): the --mode short measurement."""
+    from paper_2606_13872_b200 import inputs as I
+    a = argparse.Namespace(**{**vars(args), "steps": 20, "warmup": 3})
+    out = bench_short(a, I.WORKLOADS["short128"], emit_line=False)
+    keep = ("metric", "value", "unit", "ms_per_step", "steps", "useful_tflops", "gpu_launches", "roofline", "parity")
+    leg = {k: out[k] for k in keep}
+    leg["workload"] = out["config"]["workload"]
+    return leg
+
+
+def bench_train(args, w, emit_line=True):
     """--mode train (BASELINE.json configs[4]): one step = sra_forward (fresh reference K/V, LSE written) +
     sra_backward (a6 + a7 + a8) on the workload; value = useful fwd+bwd TFLOP/s (3.5 x forward FLOPs)."""
     import numpy as np
@@ -570,9 +711,11 @@ def bench_train(args, w):
         "e2e": None, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": None,
         "parity": parity,
     }
-    emit(out)
+    if emit_line:
+        emit(out)
     if world > 1:
         dist.destroy_process_group()
+    return out
 
 
 def train_parity(w, t, grads, dev, b=0, h=0, n_rows=48, n_cols=48):
@@ -625,7 +768,7 @@ def load_traffic_all():
         return {}
 
 
-def bench_short(args, w):
+def bench_short(args, w, emit_line=True):
     """--mode short (north_star "cache-bound short-query cases", SURVEY.md 8d auxiliary sweep): cached denoising
     steps of a few generation rows against the resident reference cache.  Arithmetic intensity ~ N_g FLOP/B is
     below the ridge (~250 FLOP/B) for N_g <= 256, so the step is judged on HBM GB/s: algorithmic bytes = the
@@ -679,9 +822,33 @@ def bench_short(args, w):
         k_ms.append(ms)
     clocks = sampler.stop()
     launches = B.sra_launch_count(ctx) - launches0
+    parity = None
+    if not args.no_oracle:
+        # the last step's output (set (steps - 1) % 4 ... the per-kernel loop above ran sets 0 .. min(steps, 8) - 1)
+        import numpy as np
+        from oracle import c_oracle
+        c_oracle.build()
+        last = (min(args.steps, 8) - 1) % 4
+        step(last)
+        torch.cuda.synchronize()
+        heads = [0, w.heads - 1]
+        rows = oracle_sample_rows(w, 48, 0)
+        gs = sets[last]
+        bits_h = {n: I.bf16_bits(x[:, :, heads].contiguous().cpu()) for n, x in {**gs, **ref}.items()}
+        bits_h["q_ref"] = None
+        _, o_or, lse_or = run_oracle_sample(w.replace(heads=len(heads)), bits_h, heads, rows)
+        idx = torch.as_tensor(rows, device=dev).long()
+        parity = parity_record(o_gen[:, idx][:, :, heads].float().cpu().numpy().astype(np.float64), o_or,
+                               lse_gen[:, heads][:, :, idx].cpu().numpy().astype(np.float64), lse_or)
+        parity.update(rows=int(len(rows)), heads=heads)
     B.sra_destroy(ctx)
     kernel_ms = statistics.median(k_ms)
     achieved = alg_bytes / (kernel_ms * 1e-3) / 1e9
+    # which roofline: arithmetic intensity of the step against the ridge of the two measured peaks
+    intensity = fl / alg_bytes
+    ridge = peaks["bf16_tflops_sustained"] * 1e12 / (peaks["hbm_gbs"] * 1e9)
+    tensor_bound = intensity > ridge
+    achieved_tf = fl / (kernel_ms * 1e-3) / 1e12
     cfg = config_of(w, args)
     cfg["step"] = "sra_forward, cached denoising step (q_ref = k_ref = v_ref = NULL): G rows against gen K/V + resident reference cache"
     cfg["n_split"] = n_split
@@ -691,15 +858,23 @@ def bench_short(args, w):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
         "config": cfg, "useful_tflops": fl * args.steps / (elapsed_ms * 1e-3) / 1e12, "e2e": None,
         "gpu_launches": int(launches), "clocks": clocks,
-        "roofline": {"bound": "hbm", "kernel": "sra_fwd_kernel<128>" + (" + sra_fwd_merge_kernel<128>" if n_split > 1 else ""),
-                     "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
-                     "peak_kind": f"{peaks_kind} copy bandwidth", "kernel_ms": kernel_ms,
-                     "algorithmic_bytes_per_launch": alg_bytes,
+        "roofline": {"bound": "tensor" if tensor_bound else "hbm",
+                     "kernel": "sra_fwd_kernel<128>" + (" + sra_fwd_merge_kernel<128>" if n_split > 1 else ""),
+                     "achieved": achieved_tf if tensor_bound else achieved,
+                     "peak": peaks["bf16_tflops_sustained"] if tensor_bound else peaks["hbm_gbs"],
+                     "unit": UNIT if tensor_bound else "GB/s",
+                     "frac": achieved_tf / peaks["bf16_tflops_sustained"] if tensor_bound else achieved / peaks["hbm_gbs"],
+                     "peak_kind": f"{peaks_kind} cuBLAS bf16, sustained" if tensor_bound else f"{peaks_kind} copy bandwidth",
+                     "intensity_flop_per_byte": intensity, "ridge_flop_per_byte": ridge,
+                     "hbm_gbs": achieved, "hbm_frac": achieved / peaks["hbm_gbs"], "kernel_ms": kernel_ms,
+                     "algorithmic_bytes_per_launch": alg_bytes, "algorithmic_flops_per_launch": fl,
                      "traffic": (lambda t: (t.get("sra_fwd_kernel_dram_bytes", 0) + t.get("sra_fwd_merge_kernel_dram_bytes", 0)) or None)(
                          load_traffic_all().get(w.name, {}) or {})},
-        "cpu_baseline": None, "parity": None,
+        "cpu_baseline": None, "parity": parity,
     }
-    emit(out)
+    if emit_line:
+        emit(out)
+    return out
 
 
 def bench_rope(args, w):
@@ -950,6 +1125,10 @@ def main():
                     help="--mode train: also check dQ/dK/dV of one (batch, head) against the oracle (minutes of CPU)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-oracle", action="store_true", help="skip the cpu_baseline / parity legs")
+    ap.add_argument("--shard", default="batch", choices=["batch", "heads"],
+                    help="--mode fwd, N > 1: batch = weak scaling (one item per rank), heads = strong scaling (one item, H / N heads per rank)")
+    ap.add_argument("--no-legs", dest="legs", action="store_false",
+                    help="--mode fwd on 720p: skip the extra legs (8-step cached protocol, training step, short-query step)")
     ap.add_argument("--oracle-rows", type=int, default=768, help="generation rows in the oracle sample")
     ap.add_argument("--chunks", type=int, default=4, help="--mode ulysses: head chunks per rank (pipeline depth)")
     ap.add_argument("--window", type=int, default=-1,
@@ -957,14 +1136,26 @@ def main():
     ap.add_argument("--invalid-frac", type=float, default=0.0,
                     help="--mode fwd: fraction of reference tokens marked invalid (sparse validity masking, PAPER.md:225)")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # `python bench.py --gpus N` without a launcher: start the N ranks ourselves, exactly as the driver's
+        # torchrun line would (one process per GPU, rendezvous on 127.0.0.1); rank 0 of that job prints the line
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        sys.stdout.flush()
+        os.execv(sys.executable, cmd)
     claim_stdout()
     if args.warmup < 3 and args.impl == "ours":
         log("note: W < 3 warm-up steps breaks the timing rules; use --warmup >= 3 for a reportable number")
     from paper_2606_13872_b200 import inputs as I
     w = I.WORKLOADS[args.workload or {"train": "train", "short": "short128"}.get(args.mode, "720p")]
     world = int(os.environ.get("WORLD_SIZE", "1"))
-    if world != args.gpus and world > 1:
-        log(f"note: --gpus {args.gpus} but WORLD_SIZE={world}; using WORLD_SIZE")
+    if world != args.gpus:
+        log(f"note: --gpus {args.gpus} but WORLD_SIZE={world}; the job has WORLD_SIZE ranks and reports that")
+        args.gpus = world
     if args.impl == "reference":
         if int(os.environ.get("RANK", "0")) != 0:
             return

@@ -120,3 +120,20 @@ def test_head_chunks_partition_the_heads():
                 h0, hc = ulysses.head_chunk(H, world, r, n_chunks, c)
                 seen.extend(range(h0, h0 + hc))
         assert sorted(seen) == list(range(H))
+
+
+def test_bench_gpus2_starts_two_ranks_itself():
+    """`python bench.py --gpus 2` without a launcher starts its own 2-rank job (torchrun re-exec on 127.0.0.1), rank 0
+    alone prints the line and it says n_gpus = 2.  Run with --impl reference (the oracle arm: no GPU needed)."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1",
+                        "--warmup", "0", "--workload", "tiny"], capture_output=True, text=True, timeout=600, env=env, cwd=root)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, r.stdout
+    out = json.loads(lines[0])
+    assert out["impl"] == "reference" and out["n_gpus"] == 2 and out["value"] > 0

@@ -39,18 +39,32 @@ def _head_bits(t, heads, b=None):
     return out
 
 
-def _forward_sampled(w, heads, n_random=8, steps=1):
+def _forward_sampled(w, heads, n_random=8, steps=1, invalid_frac=0.0, window=-1, n_frames=21):
     """Step 0 (cache build + G and R rows) and `steps - 1` cached denoising steps (G rows only, fresh G tensors,
-    resident reference K/V) of workload `w`; every step checked on sampled rows of `heads`."""
+    resident reference K/V) of workload `w`; every step checked on sampled rows of `heads`.
+    invalid_frac > 0: a seeded validity mask over the reference tokens (the mask bench.py
+    --invalid-frac draws); window >= 0: sparse temporal attention over `n_frames` equal frames (PAPER.md:143);
+    the C oracle materialises both restrictions in its visibility predicate."""
     from paper_2606_13872_b200 import binding as B
     dev = torch.device("cuda:0")
     scale = 1.0 / math.sqrt(w.head_dim)
     ref = _device_inputs(w, ("q_ref", "k_ref", "v_ref"), dev)
     ctx = B.sra_create(w.batch, w.heads, w.head_dim, w.n_gen, w.ref_block_offsets)
+    valid = frames = None
+    okw = {}
     try:
+        if invalid_frac > 0:
+            valid = np.random.default_rng(w.seed).random(w.n_ref) >= invalid_frac
+            B.sra_set_reference_validity(ctx, valid)
+            okw["valid"] = valid
+        if window >= 0:
+            frames = [i * (w.n_gen // n_frames) for i in range(n_frames)] + [w.n_gen]
+            B.sra_set_temporal_window(ctx, frames, window)
+            okw.update(gen_frame_offsets=frames, window=window)
         B.sra_cache_reference_kv(ctx, ref["k_ref"], ref["v_ref"])
         cache_bytes = B.sra_cache_bytes(ctx)
-        assert cache_bytes == 2 * w.batch * w.n_ref * w.heads * w.head_dim * 2
+        n_cached = w.n_ref if valid is None else int(valid.sum())
+        assert cache_bytes == 2 * w.batch * n_cached * w.heads * w.head_dim * 2
         o_gen = torch.empty((w.batch, w.n_gen, w.heads, w.head_dim), device=dev, dtype=torch.bfloat16)
         o_ref = torch.empty_like(ref["q_ref"])
         lse_gen = torch.empty((w.batch, w.heads, w.n_gen), device=dev)
@@ -69,12 +83,13 @@ def _forward_sampled(w, heads, n_random=8, steps=1):
                 use_rows = rows[rows < w.n_gen]
             torch.cuda.synchronize()
             n_split, _ = B.sra_split_schedule_copy(ctx)
-            assert B.sra_launch_count(ctx) - launches0 == (1 if n_split == 1 else 2), \
-                "one forward = one kernel launch (+ the partial merge of a key-split schedule), no cache re-copy"
+            if valid is None or step > 0:  # (step 0 under a validity mask also gathers Q_r and scatters O_r / LSE_r)
+                assert B.sra_launch_count(ctx) - launches0 == (1 if n_split == 1 else 2), \
+                    "one forward = one kernel launch (+ the partial merge of a key-split schedule), no cache re-copy"
             assert B.sra_cache_bytes(ctx) == cache_bytes
             assert torch.isfinite(o_gen.float()).all()
             tb = _head_bits({**gen, **ref}, heads)
-            o_or, lse_or = c_oracle.forward_rows(*[tb[n] for n in NAMES6], w.ref_block_offsets, scale, use_rows)
+            o_or, lse_or = c_oracle.forward_rows(*[tb[n] for n in NAMES6], w.ref_block_offsets, scale, use_rows, **okw)
             g = use_rows[use_rows < w.n_gen]
             r = use_rows[use_rows >= w.n_gen] - w.n_gen
             o_gpu = [o_gen[:, torch.as_tensor(g, device=dev).long()][:, :, heads].float().cpu().numpy()]
@@ -83,14 +98,38 @@ def _forward_sampled(w, heads, n_random=8, steps=1):
                 o_gpu.append(o_ref[:, torch.as_tensor(r, device=dev).long()][:, :, heads].float().cpu().numpy())
                 l_gpu.append(lse_ref[:, heads][:, :, torch.as_tensor(r, device=dev).long()].cpu().numpy())
             assert_parity(np.concatenate(o_gpu, axis=1), o_or, f"{w.name} step {step} sampled O")
-            assert np.abs(np.concatenate(l_gpu, axis=2) - lse_or).max() <= LSE_TOL
+            l_gpu = np.concatenate(l_gpu, axis=2)
+            empty = np.isneginf(lse_or)  # rows of invalid reference tokens: O = 0, LSE = -inf on both sides (A8)
+            assert np.array_equal(np.isneginf(l_gpu), empty)
+            assert np.abs(l_gpu[~empty] - lse_or[~empty]).max() <= LSE_TOL
+            if valid is not None and step == 0:
+                assert empty.any() and (~empty).any(), "the sample must hold valid and invalid reference rows"
     finally:
         B.sra_destroy(ctx)
 
 
 def test_720p_step0_and_cached_steps():
-    """BASELINE.json configs[2]: 720p, ref K/V cached once, reused by later denoising steps."""
-    _forward_sampled(sra_inputs.WORKLOADS["720p"], heads=[0, 39], n_random=8, steps=3)
+    """BASELINE.json configs[2]: 720p, "reuse cached ref KV over 8 denoising steps": step 0 builds
+    the cache and computes G and R rows, steps 1-7 are cached steps with fresh generation tensors."""
+    _forward_sampled(sra_inputs.WORKLOADS["720p"], heads=[0, 39], n_random=8, steps=8)
+
+
+def test_720p_invalid_reference_tokens():
+    """The shape `bench.py --invalid-frac 0.3` quotes: 30 % of the reference tokens invalid, the
+    resident cache holds the valid ones only; step 0 + one cached step against the validity-aware C oracle."""
+    _forward_sampled(sra_inputs.WORKLOADS["720p"], heads=[7], n_random=16, steps=2, invalid_frac=0.3)
+
+
+def test_720p_temporal_window():
+    """The shape `bench.py --window 2` quotes (reading A17): generation keys of frames within +-2."""
+    _forward_sampled(sra_inputs.WORKLOADS["720p"], heads=[31], n_random=16, steps=2, window=2)
+
+
+def test_480p_dist_a():
+    """BASELINE.json configs[1] by name, under its own distribution (reading A of A14)."""
+    w = sra_inputs.WORKLOADS["480p"]
+    assert w.dist == "A"
+    _forward_sampled(w, heads=[0, 20], n_random=16, steps=2)
 
 
 def test_720p_dist_b():
@@ -98,9 +137,9 @@ def test_720p_dist_b():
     _forward_sampled(sra_inputs.WORKLOADS["720p"].replace(dist="B"), heads=[17], n_random=8, steps=1)
 
 
-@pytest.mark.parametrize("name", ["sweep5s", "sweep40s"])
+@pytest.mark.parametrize("name", ["sweep5s", "sweep10s", "sweep20s", "sweep40s"])
 def test_long_reference_sweep_endpoints(name):
-    """BASELINE.json configs[3]: the 5 s and 40 s (174,720 reference tokens, 3.58 GB cache) ends of the sweep."""
+    """BASELINE.json configs[3]: every point of the sweep, 5 s to 40 s (174,720 reference tokens, 3.58 GB cache)."""
     _forward_sampled(sra_inputs.WORKLOADS[name], heads=[3], n_random=8, steps=2)
 
 
@@ -163,28 +202,28 @@ def test_train_config_forward_backward_sampled():
         torch.cuda.synchronize()
         for g in grads.values():
             assert torch.isfinite(g.float()).all()
-        b, h = 1, 23
-        tb = _head_bits(t, [h], b=b)
-        args6 = [tb[n] for n in NAMES6]
-        o, lse = c_oracle.forward_head(*args6, w.ref_block_offsets, scale, 0, 0)
-        n = w.n_gen + w.n_ref
-        off = w.ref_block_offsets
-        rng = np.random.default_rng(1)
-        edge = [0, 63, 64, 127, 128, w.n_gen - 1, w.n_gen, w.n_gen + off[1] - 1, w.n_gen + off[1], n - 1]
-        rows = np.asarray(sorted(set(edge) | set(int(x) for x in rng.integers(0, n, 24))), dtype=np.int32)
-        cols = np.asarray(sorted(set(edge) | set(int(x) for x in rng.integers(0, n, 24))), dtype=np.int32)
-        # forward of the sampled rows first (the backward consumes the GPU's own O and LSE, as a training step does)
-        gi, ri = rows[rows < w.n_gen], rows[rows >= w.n_gen] - w.n_gen
-        o_gpu = np.concatenate([o_gen[b, :, h][torch.as_tensor(gi, device=dev).long()].float().cpu().numpy(),
-                                o_ref[b, :, h][torch.as_tensor(ri, device=dev).long()].float().cpu().numpy()], axis=0)
-        assert_parity(o_gpu, o[rows], "train config sampled O")
-        dq, dk, dv = c_oracle.backward_head(*args6, tb["do_gen"], tb["do_ref"], off, scale, 0, 0, o, lse, rows=rows,
-                                            cols=cols)
-        for name, ref, idx in (("dq", dq, rows), ("dk", dk, cols), ("dv", dv, cols)):
-            gi, ri = idx[idx < w.n_gen], idx[idx >= w.n_gen] - w.n_gen
-            got = np.concatenate(
-                [grads[name + "_gen"][b, :, h][torch.as_tensor(gi, device=dev).long()].float().cpu().numpy(),
-                 grads[name + "_ref"][b, :, h][torch.as_tensor(ri, device=dev).long()].float().cpu().numpy()], axis=0)
-            assert_parity(got, ref, f"train config sampled {name}")
+        for b, h in ((1, 23), (0, 6)):  # both batch items (each oracle pass is a full fp64 forward of one (b, h))
+            tb = _head_bits(t, [h], b=b)
+            args6 = [tb[n] for n in NAMES6]
+            o, lse = c_oracle.forward_head(*args6, w.ref_block_offsets, scale, 0, 0)
+            n = w.n_gen + w.n_ref
+            off = w.ref_block_offsets
+            rng = np.random.default_rng(1)
+            edge = [0, 63, 64, 127, 128, w.n_gen - 1, w.n_gen, w.n_gen + off[1] - 1, w.n_gen + off[1], n - 1]
+            rows = np.asarray(sorted(set(edge) | set(int(x) for x in rng.integers(0, n, 24))), dtype=np.int32)
+            cols = np.asarray(sorted(set(edge) | set(int(x) for x in rng.integers(0, n, 24))), dtype=np.int32)
+            # forward of the sampled rows first (the backward consumes the GPU's own O and LSE, as a training step does)
+            gi, ri = rows[rows < w.n_gen], rows[rows >= w.n_gen] - w.n_gen
+            o_gpu = np.concatenate([o_gen[b, :, h][torch.as_tensor(gi, device=dev).long()].float().cpu().numpy(),
+                                    o_ref[b, :, h][torch.as_tensor(ri, device=dev).long()].float().cpu().numpy()], axis=0)
+            assert_parity(o_gpu, o[rows], "train config sampled O")
+            dq, dk, dv = c_oracle.backward_head(*args6, tb["do_gen"], tb["do_ref"], off, scale, 0, 0, o, lse, rows=rows,
+                                                cols=cols)
+            for name, ref, idx in (("dq", dq, rows), ("dk", dk, cols), ("dv", dv, cols)):
+                gi, ri = idx[idx < w.n_gen], idx[idx >= w.n_gen] - w.n_gen
+                got = np.concatenate(
+                    [grads[name + "_gen"][b, :, h][torch.as_tensor(gi, device=dev).long()].float().cpu().numpy(),
+                     grads[name + "_ref"][b, :, h][torch.as_tensor(ri, device=dev).long()].float().cpu().numpy()], axis=0)
+                assert_parity(got, ref, f"train config sampled {name}")
     finally:
         B.sra_destroy(ctx)
