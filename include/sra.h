@@ -18,7 +18,13 @@
  *     status (0 = SRA_OK, <0 = error) and never throws / aborts.
  *   - "device" pointers are CUDA device pointers on the ctx's device; "host" pointers are
  *     ordinary host memory.  The caller owns every tensor; the library owns only sra_ctx
- *     (resident reference-KV cache, tile schedule, fp32 backward workspace).
+ *     (resident reference-KV cache, tile schedule, fp32 backward workspace).  Every entry point
+ *     makes the ctx's device current for its own duration and restores the caller's device.
+ *   - Memory: sra_create allocates what sra_cache_reference_kv and sra_forward need (cache,
+ *     device schedule, key-split workspace).  The optional paths - backward workspace, host
+ *     staging of sra_forward_host, compaction buffers of a validity mask - are allocated ONCE,
+ *     sized from the config for the largest case, by sra_reserve or at the first call that needs
+ *     them; no steady-state call allocates, frees, creates a stream or synchronises the device.
  *   - Tensor layout: bf16, [batch, tokens, heads, head_dim], head_dim contiguous,
  *     16-byte aligned base pointers.  LSE: fp32 [batch, heads, tokens].
  *   - Calls are asynchronous on `cuda_stream` (a cudaStream_t passed as void*; NULL = legacy
@@ -60,10 +66,29 @@ typedef struct {
 } sra_config;
 
 /* Creates a context: validates the config, copies the block pattern, builds the tile
- * schedule (work items never enumerate a masked tile), allocates the
- * resident reference-KV cache (2 * B*n_ref*H*d bf16) and the backward workspace lazily.
- * *out is set to NULL on failure. */
+ * schedule (work items never enumerate a masked tile) and allocates, on
+ * cfg->device, the resident reference-KV cache (2 * B*n_ref*H*d bf16), the device copies of the
+ * schedule and - for short-query shapes - the key-split workspace.  The caller's current device
+ * is left unchanged.  *out is set to NULL on failure (SRA_ERR_OOM if the device allocations fail).
+ * Without a usable sm_100 device the context is host-only (schedule queries work, every compute
+ * entry point returns SRA_ERR_UNSUPPORTED). */
 int sra_create(const sra_config* cfg, sra_ctx** out);
+
+/* One-time allocation of the optional paths, so that no later call allocates (each bit is also
+ * reserved implicitly by the first call that needs it; reserving twice is a no-op):
+ *   SRA_RESERVE_BACKWARD  fp32 workspace of sra_backward: dQ accumulators B*H*n_pad*d, D and LSE*log2e
+ *                         B*H*n_pad each, n_pad = (n_gen + n_ref) rounded up to 64
+ *   SRA_RESERVE_HOST      sra_forward_host: device staging of q/k/v/o (gen), q/o (ref) and both LSE,
+ *                         two copy streams, events, the fp32 partials of its reference-first phase; measures the
+ *                         host->device copy bandwidth once (64 MB probe) to size that phase
+ *   SRA_RESERVE_VALIDITY  sra_set_reference_validity[_batched]: compacted Q_r/K_r/V_r/O_r/LSE_r (n_ref rows
+ *                         capacity) and the index arrays; with SRA_RESERVE_BACKWARD also dO_r/dQ_r/dK_r/dV_r
+ * Returns SRA_ERR_OOM if an allocation fails (nothing of that bit is kept), SRA_ERR_UNSUPPORTED
+ * without an sm_100 device. */
+#define SRA_RESERVE_BACKWARD 1u
+#define SRA_RESERVE_HOST 2u
+#define SRA_RESERVE_VALIDITY 4u
+int sra_reserve(sra_ctx* ctx, uint32_t what);
 
 /* "reference KV tensors ... computed once at the first denoising step and
  * cached in GPU memory".  k_ref / v_ref: DEVICE bf16 [B, n_ref, H, d] (post-projection,
@@ -135,9 +160,15 @@ typedef struct {
  * enough to cover the upload) attend the resident reference K/V while K_g / V_g are in flight, then the generation
  * keys, and the two fp32 partials (O_s, LSE_s) of each row are merged exactly as in the key-split schedule - so
  * those rows can differ from sra_forward's single-pass result in the last bf16 bit (same tolerance against the
- * oracle; the other slabs and the reference rows are bit-identical).  Needs 2 * H * n_gen * (d + 1) * 4 bytes of
+ * oracle; the other slabs and the reference rows are bit-identical).  Needs 2 * B * H * n_gen * (d + 1) * 4 bytes of
  * ctx-owned partial buffers.  The copy streams are ordered after prior work on `cuda_stream`, and `cuda_stream`
- * waits for the last device->host copy, so the call is still asynchronous on - and ordered by - the caller's stream. */
+ * waits for the last device->host copy, so the call is still asynchronous on - and ordered by - the caller's stream.
+ * The same pipeline runs with batch > 1 (a slab is the same row range of every batch item, copied with one strided
+ * copy), under a validity mask (the reference rows are gathered from / scattered into the staged tensors) and under
+ * a temporal window; with per-sample masks the reference-first phase is skipped.  Only shapes with fewer than 16
+ * query slabs (the short-query regime, a sub-millisecond launch) copy serially.  The number of reference-first
+ * slabs follows two measured rates: the host->device bandwidth (SRA_RESERVE_HOST) and the forward rate of the
+ * previous call on this ctx.  Staging, streams and events: see sra_reserve(SRA_RESERVE_HOST). */
 int sra_forward_host(sra_ctx* ctx, const sra_fwd_host_args* args, void* cuda_stream);
 
 typedef struct {
@@ -188,7 +219,10 @@ int sra_schedule_copy(const sra_ctx* ctx, int32_t* items, int32_t capacity, int3
  * reference key; reference rows are unchanged.  window < 0 turns it off (gen_frame_offsets may then be NULL);
  * window >= n_frames - 1 is plain SRA.  The schedule is rebuilt: forward slabs and backward key tiles never straddle
  * a frame and masked tiles are never enumerated, so cost is linear in the window.  Forward and backward are
- * supported; the key-split short-query schedule is not combined with a window.  Synchronises the device. */
+ * supported; the key-split short-query schedule is not combined with a window.  Host work only: the new schedule is
+ * uploaded by the next launching call, on that call's stream (into the second of two device buffers, so kernels
+ * already in flight keep the schedule they were launched with); calls issued on OTHER streams must be ordered after
+ * that call by the caller.  Allocates only if the new schedule has more work items than any before it. */
 int sra_set_temporal_window(sra_ctx* ctx, int32_t n_frames, const int32_t* gen_frame_offsets, int32_t window);
 
 /* Sparse validity masking of reference tokens ("skip invalid reference tokens"; SURVEY.md 8f #1,
@@ -198,9 +232,29 @@ int sra_set_temporal_window(sra_ctx* ctx, int32_t n_frames, const int32_t* gen_f
  * its gradient rows are 0.  The library compacts: the schedule, the resident cache, the workspaces and the
  * kernels only ever see the valid tokens (blocks shrink, empty blocks vanish), so invalid tokens cost nothing;
  * caller tensors keep their [B, n_ref, H, d] shape and are gathered / scattered by row.  Invalidates the
- * resident cache (call sra_cache_reference_kv again) and synchronises the device.  Usable without a GPU
- * (host schedule only). */
+ * resident cache (call sra_cache_reference_kv again).  Host work only, like sra_set_temporal_window: the schedule and
+ * the index arrays are uploaded by the next launching call on its stream.  Usable without a GPU (host schedule
+ * only). */
 int sra_set_reference_validity(sra_ctx* ctx, const uint8_t* valid);
+
+/* Per-sample validity / variable reference length ("validity masks are precomputed per-rank"; reading
+ * A12): `valid` = HOST, n_masks * n_ref bytes, n_masks = 1 (the call above) or n_masks = batch (row b = the mask of
+ * batch item b).  Every batch item is the problem of sra_set_reference_validity under its own mask: it gets its own
+ * compaction and its own work-item list (the lists of all items are stacked with a common stride and padded with
+ * empty items, which the kernels skip at once), so a batch whose references have different lengths pays for its
+ * valid tokens only.  Compacted tensors and the cache have max_b(valid_b) rows per item; the rows behind an item's
+ * last valid token are zero.  The key-split short-query schedule is not combined with per-sample masks.
+ * SRA_ERR_INVALID_ARG if n_masks is neither 1 nor batch. */
+int sra_set_reference_validity_batched(sra_ctx* ctx, const uint8_t* valid, int32_t n_masks);
+
+/* The forward schedule of ONE batch item (same 8-int32 layout as sra_schedule_copy; differs between items only under
+ * per-sample masks).  Pure host logic. */
+int sra_batch_schedule_copy(const sra_ctx* ctx, int32_t batch_item, int32_t* items, int32_t capacity, int32_t* n_items);
+
+/* CTA-pair launch list (head_dim 128 without a key split: *use_pairs = 1): the items sra_fwd_kernel<128, 2> is
+ * launched with - consecutive slabs of sra_schedule_copy that see the same keys merged into one item of up to 512
+ * rows, run by a cluster of two CTAs that share every K/V tile (same 8-int32 layout).  Pure host logic. */
+int sra_pair_schedule_copy(const sra_ctx* ctx, int32_t* use_pairs, int32_t* items, int32_t capacity, int32_t* n_items);
 
 /* Short-query schedules (north_star "cache-bound short-query cases"): when a context has fewer generation
  * slabs than about two per SM, sra_create cuts every generation slab into *n_split key ranges of whole
@@ -211,7 +265,8 @@ int sra_set_reference_validity(sra_ctx* ctx, const uint8_t* valid);
  * n_gen_items * n_split split slabs, then the reference items.  Pure host logic - usable without a GPU. */
 int sra_split_schedule_copy(const sra_ctx* ctx, int32_t* n_split, int32_t* items, int32_t capacity, int32_t* n_items);
 
-/* Device bytes held by the resident reference-KV cache (0 before the first cache call). */
+/* Bytes of reference K/V resident in the cache: 2 * sum_b valid_b * H * d * 2 (0 before the first cache call and after
+ * a validity change until the cache is rebuilt).  The allocation itself is made at sra_create for n_ref rows. */
 int64_t sra_cache_bytes(const sra_ctx* ctx);
 
 /* Optional per-kernel device timing (bench.py's roofline leg): when enabled, every launch is bracketed by

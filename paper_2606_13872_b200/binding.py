@@ -25,7 +25,10 @@ EXPORTS = (
     "sra_create", "sra_cache_reference_kv", "sra_cache_reference_kv_rope", "sra_apply_rope", "sra_forward", "sra_forward_host", "sra_backward", "sra_destroy", "sra_useful_flops",
     "sra_schedule_info", "sra_schedule_copy", "sra_cache_bytes", "sra_launch_count", "sra_status_string",
     "sra_last_error", "sra_set_kernel_timing", "sra_kernel_time_ms", "sra_split_schedule_copy", "sra_set_reference_validity", "sra_set_temporal_window",
+    "sra_reserve", "sra_set_reference_validity_batched", "sra_batch_schedule_copy", "sra_pair_schedule_copy",
 )
+
+RESERVE_BACKWARD, RESERVE_HOST, RESERVE_VALIDITY = 1, 2, 4
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(
@@ -86,6 +89,16 @@ lib.sra_schedule_info.argtypes = [_ctx_p, ctypes.POINTER(ctypes.c_int32), ctypes
 lib.sra_schedule_info.restype = ctypes.c_int
 lib.sra_set_reference_validity.argtypes = [_ctx_p, ctypes.c_char_p]
 lib.sra_set_reference_validity.restype = ctypes.c_int
+lib.sra_set_reference_validity_batched.argtypes = [_ctx_p, ctypes.c_char_p, ctypes.c_int32]
+lib.sra_set_reference_validity_batched.restype = ctypes.c_int
+lib.sra_reserve.argtypes = [_ctx_p, ctypes.c_uint32]
+lib.sra_reserve.restype = ctypes.c_int
+lib.sra_batch_schedule_copy.argtypes = [_ctx_p, ctypes.c_int32, ctypes.POINTER(ctypes.c_int32), ctypes.c_int32,
+                                        ctypes.POINTER(ctypes.c_int32)]
+lib.sra_batch_schedule_copy.restype = ctypes.c_int
+lib.sra_pair_schedule_copy.argtypes = [_ctx_p, ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32), ctypes.c_int32,
+                                       ctypes.POINTER(ctypes.c_int32)]
+lib.sra_pair_schedule_copy.restype = ctypes.c_int
 lib.sra_set_temporal_window.argtypes = [_ctx_p, ctypes.c_int32, ctypes.POINTER(ctypes.c_int32), ctypes.c_int32]
 lib.sra_set_temporal_window.restype = ctypes.c_int
 lib.sra_split_schedule_copy.argtypes = [_ctx_p, ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32), ctypes.c_int32,
@@ -150,11 +163,22 @@ def sra_create(batch: int, heads: int, head_dim: int, n_gen: int, ref_block_offs
                      arr if n_blocks > 0 else None, float(softmax_scale), device)
     ctx = _ctx_p()
     _check(lib.sra_create(ctypes.byref(cfg), ctypes.byref(ctx)))
+    _SHAPES[ctx.value] = (int(batch), int(off[-1]))
     return ctx.value
 
 
+_SHAPES = {}  # ctx handle -> (batch, n_ref): the binding checks host buffer lengths before they cross the boundary
+
+
 def sra_destroy(ctx: Optional[int]) -> None:
+    _SHAPES.pop(ctx, None)
     lib.sra_destroy(ctx)
+
+
+def sra_reserve(ctx: int, what: int) -> None:
+    """sra_reserve (include/sra.h): one-time allocation of the optional paths (RESERVE_BACKWARD | RESERVE_HOST |
+    RESERVE_VALIDITY), so that no later call allocates."""
+    _check(lib.sra_reserve(ctx, int(what)), ctx)
 
 
 def sra_cache_reference_kv(ctx: int, k_ref, v_ref, stream=None) -> None:
@@ -251,13 +275,47 @@ def sra_set_temporal_window(ctx: int, gen_frame_offsets, window: int) -> None:
     _check(lib.sra_set_temporal_window(ctx, len(off) - 1, arr, int(window)), ctx)
 
 
+def _items(buf, n):
+    keys = ("q_is_ref", "q_row0", "q_rows", "seg0_is_ref", "seg0_start", "seg0_len", "seg1_start", "seg1_len")
+    return [dict(zip(keys, buf[8 * i:8 * i + 8])) for i in range(n)]
+
+
+def sra_batch_schedule_copy(ctx: int, batch_item: int):
+    """The forward work items of one batch item (they differ between items only under per-sample validity masks)."""
+    n = ctypes.c_int32()
+    _check(lib.sra_batch_schedule_copy(ctx, int(batch_item), None, 0, ctypes.byref(n)), ctx)
+    buf = (ctypes.c_int32 * (8 * max(n.value, 1)))()
+    _check(lib.sra_batch_schedule_copy(ctx, int(batch_item), buf, n.value, ctypes.byref(n)), ctx)
+    return _items(buf, n.value)
+
+
+def sra_pair_schedule_copy(ctx: int):
+    """(use_pairs, pair items): the launch list of the CTA-pair forward kernel (items of up to 512 rows)."""
+    up, n = ctypes.c_int32(), ctypes.c_int32()
+    _check(lib.sra_pair_schedule_copy(ctx, ctypes.byref(up), None, 0, ctypes.byref(n)), ctx)
+    buf = (ctypes.c_int32 * (8 * max(n.value, 1)))()
+    _check(lib.sra_pair_schedule_copy(ctx, ctypes.byref(up), buf, n.value, ctypes.byref(n)), ctx)
+    return bool(up.value), _items(buf, n.value)
+
+
 def sra_set_reference_validity(ctx: int, valid) -> None:
-    """sra_set_reference_validity (include/sra.h): `valid` = sequence / array of n_ref truthy values, or None."""
+    """sra_set_reference_validity[_batched] (include/sra.h): `valid` = None (every token valid), a sequence / array of
+    n_ref truthy values (one mask for the batch) or a [batch, n_ref] array (one mask per batch item, reading A12).
+    The length is checked here: the C side reads exactly n_masks * n_ref bytes."""
     if valid is None:
         _check(lib.sra_set_reference_validity(ctx, None), ctx)
         return
-    buf = bytes(bytearray(1 if v else 0 for v in valid))
-    _check(lib.sra_set_reference_validity(ctx, buf), ctx)
+    import numpy as np
+    v = np.ascontiguousarray(np.asarray(valid) != 0, dtype=np.uint8)
+    batch, n_ref = _SHAPES.get(ctx, (None, None))
+    if v.ndim == 1:
+        if n_ref is not None and v.shape[0] != n_ref:
+            raise ValueError(f"valid has {v.shape[0]} entries, the context has n_ref = {n_ref}")
+        _check(lib.sra_set_reference_validity(ctx, v.tobytes()), ctx)
+        return
+    if v.ndim != 2 or (n_ref is not None and v.shape != (batch, n_ref)):
+        raise ValueError(f"valid must be [n_ref] or [batch, n_ref] = [{batch}, {n_ref}], got {v.shape}")
+    _check(lib.sra_set_reference_validity_batched(ctx, v.tobytes(), int(v.shape[0])), ctx)
 
 
 def sra_cache_bytes(ctx: int) -> int:

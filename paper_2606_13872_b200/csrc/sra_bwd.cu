@@ -156,7 +156,8 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
-  const BwdItem item = p.items[blockIdx.x];
+  const BwdItem item = p.items[blockIdx.x + size_t(blockIdx.z) * p.item_batch_stride];
+  if (item.k_rows == 0) return;  // padding of a per-sample schedule (whole CTA, nothing is set up yet)
   const int h = blockIdx.y;
   const int b = blockIdx.z;
   const int bh = b * p.heads + h;
@@ -675,11 +676,11 @@ __global__ void sra_bwd_dq_finalize_kernel(const float* __restrict__ ws, __nv_bf
 template <int D>
 cudaError_t launch_bwd(const CUtensorMap* m, const BwdParams& p, cudaStream_t stream) {
   using C = BwdCfg<D>;
-  static bool configured = false;
-  if (!configured) {
+  bool* configured = smem_configured_flag(D == 128 ? 4 : 5);  // per device
+  if (!*configured) {
     cudaError_t e = cudaFuncSetAttribute(sra_bwd_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes);
     if (e != cudaSuccess) return e;
-    configured = true;
+    *configured = true;
   }
   dim3 grid(p.n_items, p.heads, p.batch);
   sra_bwd_kernel<D><<<grid, C::kThreads, C::kSmemBytes, stream>>>(m[0], m[1], m[2], m[3], m[4], m[5], m[6], m[7], p);
@@ -745,25 +746,16 @@ static int run_backward_core(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t s
   const int n_pad = (n_cat + 63) / 64 * 64;
   const size_t vec_bytes = size_t(B) * H * n_pad * 4;
   const size_t dq_bytes = vec_bytes * d;
-  if (!ctx->ws_dq) {
-    cudaError_t e = cudaMalloc(&ctx->ws_dq, dq_bytes);
-    if (e == cudaSuccess) e = cudaMalloc(&ctx->ws_delta, vec_bytes);
-    if (e == cudaSuccess) e = cudaMalloc(&ctx->ws_lse2, vec_bytes);
-    if (e != cudaSuccess) {
-      (void)cudaGetLastError();
-      cudaFree(ctx->ws_dq); cudaFree(ctx->ws_delta); cudaFree(ctx->ws_lse2);
-      ctx->ws_dq = ctx->ws_delta = ctx->ws_lse2 = nullptr;
-      return ctx_fail(ctx, SRA_ERR_OOM, "backward workspace allocation failed");
-    }
-    ctx->ws_dq_bytes = dq_bytes;
-  }
+  // the workspace is sized once, for the unmasked reference (sra_reserve(SRA_RESERVE_BACKWARD), or here on first use)
+  if (int rc = reserve(ctx, SRA_RESERVE_BACKWARD)) return rc;
+  if (int rc = sync_schedule(ctx, stream)) return rc;
   e = cudaMemsetAsync(ctx->ws_dq, 0, dq_bytes, stream);
   if (e != cudaSuccess) return ctx_fail_cuda(ctx, e, "dQ workspace memset");
 
   {  // a6
     const size_t rows = size_t(B) * n_cat * H;
     const int threads = 256;
-    const int blocks = int(std::min<size_t>((rows * 32 + threads - 1) / threads, size_t(148) * 32));
+    const int blocks = grid_for(ctx, rows * 32, threads, 32);
     KernelTimer kt(ctx, SRA_KERNEL_BWD_PREPROCESS, stream);
     auto launch = [&](auto kernel) {
       kernel<<<blocks, threads, 0, stream>>>(
@@ -793,8 +785,9 @@ static int run_backward_core(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t s
   }
 
   BwdParams p{};
-  p.items = ctx->d_bwd_items;
-  p.n_items = int(ctx->bwd_items.size());
+  p.items = ctx->d_bwd_items[ctx->sched_buf];
+  p.n_items = ctx->bwd_stride;
+  p.item_batch_stride = ctx->n_masks > 1 ? ctx->bwd_stride : 0;
   p.heads = H; p.batch = B; p.n_gen = c.n_gen; p.n_ref = nr; p.n_pad = n_pad;
   p.scale = ctx->scale;
   p.scale_log2 = ctx->scale * 1.4426950408889634f;
@@ -812,7 +805,7 @@ static int run_backward_core(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t s
   {  // a8
     const size_t total = size_t(B) * H * n_cat * (d / 8);
     const int threads = 256;
-    const int blocks = int(std::min<size_t>((total + threads - 1) / threads, size_t(148) * 32));
+    const int blocks = grid_for(ctx, total, threads, 32);
     KernelTimer kt(ctx, SRA_KERNEL_BWD_DQ_FINALIZE, stream);
     auto launch = [&](auto kernel) {
       kernel<<<blocks, threads, 0, stream>>>(ctx->ws_dq, static_cast<__nv_bfloat16*>(a->dq_gen),

@@ -7,7 +7,6 @@
 namespace sra {
 
 constexpr int kTile = 128;         // rows per MMA tile (UMMA M = 128; key tile N = 128)
-constexpr int kNumSms = 148;       // B200
 constexpr int kQRowsPerCta = 256;  // two ping-ponged Q tiles per CTA (forward)
 
 // Forward work item: a 256-row query slab and the (up to two) key
@@ -40,6 +39,8 @@ struct BwdItem {
 struct FwdParams {
   const FwdItem* items;
   int32_t n_items;
+  int32_t item_batch_stride;  // 0: one list for every batch item; else batch item b reads items + b * stride (per-sample
+                              // validity masks: lists padded to a common length with empty items, q_rows = 0)
   int32_t heads, batch;
   int32_t n_gen, n_ref;
   float scale_log2;  // softmax_scale * log2(e)
@@ -60,6 +61,7 @@ constexpr int kBwdQTile = 128;  // query rows per backward iteration (keys per C
 struct BwdParams {
   const BwdItem* items;
   int32_t n_items;
+  int32_t item_batch_stride;  // as in FwdParams (empty item: k_rows = 0)
   int32_t heads, batch;
   int32_t n_gen, n_ref;
   int32_t n_pad;       // row length of the [G ; R]-concatenated fp32 workspaces (multiple of 64)

@@ -120,7 +120,8 @@ __global__ void __launch_bounds__(FwdCfg<D, CG>::kThreads, 1)
 
   // CG = 2: blockIdx.x = 2 * (pair item) + rank; 128-row tile t of the pair's slab belongs to CTA t & 1, slot t >> 1
   const int rank = CG == 2 ? int(cluster_ctarank()) : 0;
-  const FwdItem item = p.items[CG == 2 ? blockIdx.x >> 1 : blockIdx.x];
+  const FwdItem item = p.items[(CG == 2 ? blockIdx.x >> 1 : blockIdx.x) + size_t(blockIdx.z) * p.item_batch_stride];
+  if (item.q_rows == 0) return;  // padding of a per-sample schedule (the whole CTA / CTA pair: nothing is set up yet)
   const bool q_is_ref = (item.q_is_ref & 1) != 0;
   const int split = item.q_is_ref >> 8;  // 0: final output; s + 1: key split s of a short-query G slab
   const int h = blockIdx.y;
@@ -484,8 +485,8 @@ __global__ void __launch_bounds__(FwdCfg<D, CG>::kThreads, 1)
 }
 
 // The dynamic shared-memory opt-in is a per-device function attribute: remembered per device ordinal.
-static bool* configured_flag(int which) {
-  static bool flags[4][64] = {};
+bool* smem_configured_flag(int which) {
+  static bool flags[8][64] = {};
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) dev = 0;
   return &flags[which][dev];
@@ -494,7 +495,7 @@ static bool* configured_flag(int which) {
 template <int D, int CG>
 cudaError_t launch_fwd(const CUtensorMap* maps, const FwdParams& p, cudaStream_t stream) {
   using C = FwdCfg<D, CG>;
-  bool* configured = configured_flag((D == 128 ? 0 : 1) + 2 * (CG - 1));
+  bool* configured = smem_configured_flag((D == 128 ? 0 : 1) + 2 * (CG - 1));
   if (!*configured) {
     cudaError_t e = cudaFuncSetAttribute(sra_fwd_kernel<D, CG>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes);
     if (e != cudaSuccess) return e;
@@ -564,12 +565,13 @@ __global__ void sra_fwd_merge_kernel(const float* __restrict__ part_o, const flo
   }
 }
 
-cudaError_t launch_fwd_merge(const FwdParams& p, int head_dim, int n_split, cudaStream_t stream, int row0, int n_rows) {
+cudaError_t launch_fwd_merge(const FwdParams& p, int head_dim, int n_split, cudaStream_t stream, int n_ctas, int row0,
+                             int n_rows) {
   if (n_rows < 0) { row0 = 0; n_rows = p.n_gen; }
   if (n_rows == 0) return cudaSuccess;
   const size_t rows = size_t(p.batch) * n_rows * p.heads;
   const int threads = 256;
-  const int blocks = int(std::min<size_t>((rows * 32 + threads - 1) / threads, size_t(148) * 16));
+  const int blocks = int(std::min<size_t>((rows * 32 + threads - 1) / threads, size_t(n_ctas)));
   if (head_dim == 128)
     sra_fwd_merge_kernel<128><<<blocks, threads, 0, stream>>>(p.part_o, p.part_lse, p.o_gen, p.lse_gen, n_split, p.batch, p.heads, p.n_gen, row0, n_rows);
   else

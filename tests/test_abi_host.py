@@ -238,3 +238,87 @@ def test_no_device_means_unsupported_not_fallback():
         assert B.lib.sra_backward(ctx, ctypes.byref(bw), None) == B.SRA_ERR_UNSUPPORTED
     finally:
         B.sra_destroy(ctx)
+
+
+@pytest.mark.parametrize("heads,n_gen,blocks,frames,w", [(40, 75600 // 10, (3600,) * 2, None, -1), (2, 333, (1, 130, 257, 64, 200), None, -1),
+                                                         (2, 1200, (700, 513), (300, 300, 300, 300), 1), (2, 513, (), None, -1),
+                                                         (2, 256 * 5, (256 * 2,), None, -1)])
+def test_pair_schedule_covers_the_slab_schedule(heads, n_gen, blocks, frames, w):
+    """The CTA-pair launch list (sra_fwd_kernel<128, 2>): every 256-row slab sits in exactly one pair item, a pair item
+    holds at most 512 consecutive rows of slabs that see the SAME key segments, G pairs come first, and the pair list
+    covers exactly the pairs of the mask (the coverage matrix equals the oracle's explicit mask)."""
+    off = [0]
+    for b in blocks:
+        off.append(off[-1] + b)
+    ctx = B.sra_create(1, heads, 128, n_gen, off)  # (shapes with enough slabs per SM: no key split)
+    try:
+        fr = None
+        if frames is not None:
+            fr = [0]
+            for f in frames:
+                fr.append(fr[-1] + f)
+            B.sra_set_temporal_window(ctx, fr, w)
+        slabs = B.sra_schedule_copy(ctx)
+        use_pairs, pairs = B.sra_pair_schedule_copy(ctx)
+        assert use_pairs
+        keyset = lambda it: tuple(it[k] for k in ("q_is_ref", "seg0_is_ref", "seg0_start", "seg0_len", "seg1_start", "seg1_len"))
+        si = 0
+        seen_ref = False
+        for p in pairs:
+            assert 1 <= p["q_rows"] <= 512
+            seen_ref = seen_ref or bool(p["q_is_ref"])
+            assert bool(p["q_is_ref"]) == seen_ref, "G pairs first, then R pairs"
+            rows = 0
+            while rows < p["q_rows"]:
+                s = slabs[si]
+                assert keyset(s) == keyset(p) and s["q_row0"] == p["q_row0"] + rows
+                rows += s["q_rows"]
+                si += 1
+            assert rows == p["q_rows"]
+        assert si == len(slabs)
+        if n_gen + off[-1] <= 4000:
+            M = sra_oracle.sra_mask(n_gen, off, None, fr, w).astype(np.int32)
+            assert np.array_equal(_covered_pairs(pairs, n_gen, off[-1]), M)
+    finally:
+        B.sra_destroy(ctx)
+    ctx = B.sra_create(1, 2, 64, n_gen, off)  # head_dim 64 keeps the single-CTA kernel
+    try:
+        assert not B.sra_pair_schedule_copy(ctx)[0]
+    finally:
+        B.sra_destroy(ctx)
+
+
+def test_per_sample_validity_schedules():
+    """sra_set_reference_validity_batched (reading A12; "validity masks are precomputed per-rank"): each
+    batch item gets the schedule of its own compacted reference - mapped back through its compaction it covers exactly
+    the oracle's mask under that item's flags; useful FLOPs are the sum over the items; a [B, n_ref] array whose rows are
+    all-true is the unmasked context again; wrong lengths never reach the C side."""
+    n_gen, off = 300, [0, 77, 205, 334, 339]
+    rng = np.random.default_rng(5)
+    valid = rng.random((3, off[-1])) < 0.6
+    valid[1, :] = True            # item 1: every token valid
+    valid[2, off[2]:off[3]] = False  # item 2: one block entirely invalid
+    ctx = B.sra_create(3, 2, 64, n_gen, off)
+    try:
+        plain = B.sra_schedule_copy(ctx)
+        B.sra_set_reference_validity(ctx, valid)
+        total = 0.0
+        for b in range(3):
+            items = B.sra_batch_schedule_copy(ctx, b)
+            keep = np.flatnonzero(valid[b])
+            Cc = _covered_pairs(items, n_gen, len(keep))
+            M = sra_oracle.sra_mask(n_gen, off, valid[b]).astype(np.int32)
+            idx = np.concatenate([np.arange(n_gen), n_gen + keep])
+            assert np.array_equal(Cc, M[np.ix_(idx, idx)]) and M.sum() == Cc.sum(), b
+            total += float(M.sum())
+        assert B.sra_batch_schedule_copy(ctx, 1) == plain
+        assert B.sra_useful_flops(ctx, True) == 4.0 * 64 * 2 * total
+        B.sra_set_reference_validity(ctx, np.ones((3, off[-1]), dtype=bool))
+        assert all(B.sra_batch_schedule_copy(ctx, b) == plain for b in range(3))
+        with pytest.raises(ValueError):
+            B.sra_set_reference_validity(ctx, np.ones(off[-1] - 1, dtype=bool))
+        with pytest.raises(ValueError):
+            B.sra_set_reference_validity(ctx, np.ones((2, off[-1]), dtype=bool))
+        assert B.lib.sra_set_reference_validity_batched(ctx, valid.astype(np.uint8).tobytes(), 2) == B.SRA_ERR_INVALID_ARG
+    finally:
+        B.sra_destroy(ctx)

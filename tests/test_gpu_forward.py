@@ -213,6 +213,58 @@ def test_forward_host_matches_device_path(name):
         B.sra_destroy(ctx)
 
 
+@pytest.mark.parametrize("mask", ["none", "shared", "per_sample"])
+def test_forward_host_pipelined_batch2_and_validity(mask):
+    """The pipelined host path beyond its first case (batch 1, no mask): batch 2 (a slab = the same rows of both items,
+    strided copies), a validity mask shared by the batch (reference rows gathered from / scattered into the staged
+    tensors; reference-first still on) and per-sample masks (reference-first off).  Against sra_forward on the same
+    inputs (generation rows within one bf16 ulp of the row scale - the two-partial merge; reference rows bit-identical)
+    and against the fp64 oracle under the same flags, every row."""
+    from paper_2606_13872_b200 import binding as B
+    from oracle import sra_oracle
+    w = sra_inputs.SRAWorkload("host_pipe2", 2, 2, 128, 4200, (700, 300), "B", 0)
+    t = sra_inputs.make_inputs(w)
+    dev = torch.device("cuda:0")
+    rng = np.random.default_rng(11)
+    valid = {"none": None, "shared": rng.random(w.n_ref) < 0.7,
+             "per_sample": np.stack([rng.random(w.n_ref) < 0.8, rng.random(w.n_ref) < 0.4])}[mask]
+    g = {k: v.to(dev) for k, v in t.items()}
+    ctx = B.sra_create(w.batch, w.heads, w.head_dim, w.n_gen, w.ref_block_offsets)
+    try:
+        if valid is not None:
+            B.sra_set_reference_validity(ctx, valid)
+        B.sra_cache_reference_kv(ctx, g["k_ref"], g["v_ref"])
+        d_o_gen, d_o_ref = torch.empty_like(g["q_gen"]), torch.empty_like(g["q_ref"])
+        d_lse_gen = torch.empty((w.batch, w.heads, w.n_gen), device=dev)
+        B.sra_forward(ctx, g["q_gen"], g["k_gen"], g["v_gen"], d_o_gen, q_ref=g["q_ref"], o_ref=d_o_ref, lse_gen=d_lse_gen)
+        h = {k: t[k].pin_memory() for k in ("q_gen", "k_gen", "v_gen", "q_ref")}
+        o_gen = torch.full(t["q_gen"].shape, float("nan"), dtype=torch.bfloat16).pin_memory()
+        o_ref = torch.full(t["q_ref"].shape, float("nan"), dtype=torch.bfloat16).pin_memory()
+        lse_gen = torch.full((w.batch, w.heads, w.n_gen), float("nan")).pin_memory()
+        lse_ref = torch.full((w.batch, w.heads, w.n_ref), float("nan")).pin_memory()
+        tb = bits(t)
+        ref = sra_oracle.sra_forward(tb["q_gen"], tb["k_gen"], tb["v_gen"], tb["q_ref"], tb["k_ref"], tb["v_ref"],
+                                     w.ref_block_offsets, 1.0 / math.sqrt(w.head_dim), valid=valid)
+        for _ in range(2):  # the second call sizes its reference-first phase from the first call's measured rate
+            B.sra_forward_host(ctx, h["q_gen"], h["k_gen"], h["v_gen"], o_gen, q_ref=h["q_ref"], o_ref=o_ref,
+                               lse_gen=lse_gen, lse_ref=lse_ref)
+            torch.cuda.synchronize()
+            og, dg = o_gen.float().numpy(), d_o_gen.float().cpu().numpy()
+            assert np.all(np.abs(og - dg) <= 2.0 ** -7 * np.abs(dg).max(axis=-1, keepdims=True))
+            assert np.array_equal(o_ref.float().numpy(), d_o_ref.float().cpu().numpy())
+            assert_parity(og, ref["o_gen"], f"host_pipe2[{mask}] O_g through sra_forward_host")
+            assert np.abs(lse_gen.numpy() - ref["lse_gen"]).max() <= LSE_TOL
+            v2 = np.ones((w.batch, w.n_ref), dtype=bool) if valid is None else np.broadcast_to(valid, (w.batch, w.n_ref))
+            for b in range(w.batch):
+                keep, inv = np.flatnonzero(v2[b]), np.flatnonzero(~v2[b])
+                assert_parity(o_ref[b, keep].float().numpy(), ref["o_ref"][b, keep], f"host_pipe2[{mask}] O_r item {b}")
+                assert np.all(o_ref[b, inv].float().numpy() == 0.0) and np.all(np.isneginf(lse_ref[b][:, inv].numpy()))
+                assert np.abs(lse_ref[b][:, keep].numpy() - ref["lse_ref"][b][:, keep]).max() <= LSE_TOL
+            o_gen.fill_(float("nan")); o_ref.fill_(float("nan"))
+    finally:
+        B.sra_destroy(ctx)
+
+
 @pytest.mark.parametrize("name", ["short_mini", "ragged"])
 def test_optional_lse_outputs_do_not_change_o(name):
     """lse_gen / lse_ref are nullable (include/sra.h): leaving them out must not change a byte of O, on the single-pass
