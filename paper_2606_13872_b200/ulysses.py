@@ -39,6 +39,22 @@ def head_chunk(heads: int, world: int, rank: int, n_chunks: int, chunk: int) -> 
     return h0 + c0, cc
 
 
+_RT = False  # cuda.bindings.runtime, resolved once (None if cuda-python is not installed)
+
+
+def _cuda_runtime():
+    """The cuda-python runtime bindings, imported once at first use - never in the middle of a collective, where an
+    ImportError on one rank would leave its peers waiting inside all_to_all_single."""
+    global _RT
+    if _RT is False:
+        try:
+            from cuda.bindings import runtime as rt
+            _RT = rt
+        except Exception:
+            _RT = None
+    return _RT
+
+
 def _copy_rows(dst: torch.Tensor, src: torch.Tensor) -> None:
     """dst[...] = src[...] for [B, n, h, d] views whose (h, d) block is contiguous and whose token stride is constant
     (a head slice of a [B, n, H, d] tensor, or a token range of one).  On CUDA this is one cudaMemcpy2DAsync per batch
@@ -52,7 +68,10 @@ def _copy_rows(dst: torch.Tensor, src: torch.Tensor) -> None:
     if not (dst.is_cuda and ok):
         dst.copy_(src)
         return
-    from cuda.bindings import runtime as rt
+    rt = _cuda_runtime()
+    if rt is None:  # cuda-python absent: an SM copy kernel on the same stream (slower under a running forward, never wrong)
+        dst.copy_(src)
+        return
     es = src.element_size()
     stream = torch.cuda.current_stream().cuda_stream
     for b in range(B):
@@ -137,6 +156,7 @@ class UlyssesSRA:
         if not torch.cuda.is_available():
             raise RuntimeError("UlyssesSRA: no CUDA device; the SRA path has no CPU fallback")
         self.B = B
+        _cuda_runtime()  # resolve the optional copy-engine path now, outside any collective
         self.group = group
         self.world, self.rank = _world_rank(group)
         self.batch, self.heads, self.head_dim, self.n_gen = batch, heads, head_dim, n_gen
