@@ -30,6 +30,11 @@
  *   - Calls are asynchronous on `cuda_stream` (a cudaStream_t passed as void*; NULL = legacy
  *     default stream).  Argument / launch errors are returned synchronously; execution
  *     faults surface at the caller's next synchronisation.
+ *   - Inputs must be finite.  Masked keys never reach a softmax (scores are masked by selection, P = 0 exactly), but
+ *     the ragged last tile of a key segment multiplies P = 0 with the V rows that follow the segment in memory (the
+ *     neighbouring reference block or frame; zeros past the end of a tensor), so an Inf / NaN in such a row turns the
+ *     outputs of rows that must not see it into NaN (0 * Inf).  Finite values, however large, are isolated exactly
+ *     (tests: mask poison, bit-identical).
  *   - One ctx is used from one thread at a time.  No CPU fallback exists: on a device that
  *     is not sm_100 every compute entry point returns SRA_ERR_UNSUPPORTED.
  */
