@@ -595,7 +595,7 @@ def leg_short(args):
     from paper_2606_13872_b200 import inputs as I
     a = argparse.Namespace(**{**vars(args), "steps": 20, "warmup": 3})
     out = bench_short(a, I.WORKLOADS["short128"], emit_line=False)
-    keep = ("metric", "value", "unit", "ms_per_step", "steps", "useful_tflops", "gpu_launches", "roofline", "parity")
+    keep = ("metric", "value", "unit", "ms_per_step", "steps", "useful_tflops", "gpu_launches", "roofline", "cuda_graph", "parity")
     leg = {k: out[k] for k in keep}
     leg["workload"] = out["config"]["workload"]
     return leg
@@ -822,6 +822,29 @@ def bench_short(args, w, emit_line=True):
         k_ms.append(ms)
     clocks = sampler.stop()
     launches = B.sra_launch_count(ctx) - launches0
+    # the same loop replayed from ONE CUDA graph (a steady-state call neither allocates nor synchronises, so it can be
+    # captured): what the launch overhead of two sub-millisecond kernels per step is worth
+    graph_rec = None
+    try:
+        B.sra_set_kernel_timing(ctx, False)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            for i in range(args.steps):
+                step(i)
+        graph.replay()
+        torch.cuda.synchronize()
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g0.record()
+        graph.replay()
+        g1.record()
+        torch.cuda.synchronize()
+        g_ms = g0.elapsed_time(g1) / args.steps
+        graph_rec = {"ms_per_step": g_ms, "steps_per_graph": args.steps, "eager_ms_per_step": elapsed_ms / args.steps,
+                     "gbs": alg_bytes / (g_ms * 1e-3) / 1e9, "frac_of_copy_peak": alg_bytes / (g_ms * 1e-3) / 1e9 / peaks["hbm_gbs"]}
+        del graph
+    except Exception as ex:
+        log(f"graph replay leg failed: {ex!r}")
+        graph_rec = {"error": repr(ex)}
     parity = None
     if not args.no_oracle:
         # the last step's output (set (steps - 1) % 4 ... the per-kernel loop above ran sets 0 .. min(steps, 8) - 1)
@@ -856,7 +879,7 @@ def bench_short(args, w, emit_line=True):
         "metric": "sra_short_query_cache_gbs", "value": alg_bytes * args.steps / (elapsed_ms * 1e-3) / 1e9, "unit": "GB/s",
         "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": elapsed_ms / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-        "config": cfg, "useful_tflops": fl * args.steps / (elapsed_ms * 1e-3) / 1e12, "e2e": None,
+        "config": cfg, "useful_tflops": fl * args.steps / (elapsed_ms * 1e-3) / 1e12, "e2e": None, "cuda_graph": graph_rec,
         "gpu_launches": int(launches), "clocks": clocks,
         "roofline": {"bound": "tensor" if tensor_bound else "hbm",
                      "kernel": "sra_fwd_kernel<128>" + (" + sra_fwd_merge_kernel<128>" if n_split > 1 else ""),
