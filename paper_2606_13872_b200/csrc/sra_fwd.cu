@@ -129,8 +129,14 @@ __global__ void __launch_bounds__(FwdCfg<D, CG>::kThreads, 1)
   const int n0 = (item.seg0_len + kTile - 1) / kTile;
   const int n1 = (item.seg1_len + kTile - 1) / kTile;
   const int n_kv = n0 + n1;
-  const int n_qt = item.q_rows > kTile * CG ? 2 : 1;  // Q tile slots in use (the same in both CTAs of a pair)
-  auto slot_row = [&](int i) { return (CG * i + rank) * kTile; };  // first slab row of this CTA's Q tile slot i
+  // DUAL (single-CTA kernel, a slab of at most 128 rows - the short-query regime): with one Q tile the second slot of
+  // TMEM would idle and every key tile would wait for the S -> softmax -> P -> PV chain of the one before it.  Instead
+  // both slots work on the SAME Q tile: slot i takes the key tiles j = i (mod 2) with its own running (m_ref, l, O),
+  // and the epilogue merges the two partial softmax states.  Two key tiles are then in flight, as with two Q tiles.
+  const bool dual = CG == 1 && item.q_rows <= kTile && n_kv >= 2;
+  const int n_qt = (item.q_rows > kTile * CG || dual) ? 2 : 1;  // TMEM slots in use (the same in both CTAs of a pair)
+  const int n_steps = dual ? (n_kv + 1) / 2 : n_kv;             // iterations of the (step, slot) loops
+  auto slot_row = [&](int i) { return dual ? 0 : (CG * i + rank) * kTile; };  // first slab row of this CTA's slot i
 
   if (threadIdx.x == 0) {
     mbar_init(bar_q_full, 1);
@@ -205,12 +211,13 @@ __global__ void __launch_bounds__(FwdCfg<D, CG>::kThreads, 1)
       xphase ^= 1;
       return other;
     };
-    for (int j = 0; j < n_kv; ++j) {
-      const int n_valid = (j < n0) ? min(kTile, item.seg0_len - j * kTile) : min(kTile, item.seg1_len - (j - n0) * kTile);
-      const int n_valid_h = n_valid - 64 * hh;  // valid columns of this thread's 64-column half (may be <= 0)
+    for (int t = 0; t < n_steps; ++t) {
 #pragma unroll
       for (int i = 0; i < 2; ++i) {
-        if (i < n_qt) {
+        const int j = dual ? 2 * t + i : t;  // key tile of slot i at this step
+        if (i < n_qt && j < n_kv) {
+          const int n_valid = (j < n0) ? min(kTile, item.seg0_len - j * kTile) : min(kTile, item.seg1_len - (j - n0) * kTile);
+          const int n_valid_h = n_valid - 64 * hh;  // valid columns of this thread's 64-column half (may be <= 0)
           const uint32_t tS = tS0 + i * 128 + lane_off;
           const uint32_t tO = tO0 + i * D + lane_off + hh * (D / 2);
           auto rescale_to = [&](float m_new) {
@@ -228,11 +235,11 @@ __global__ void __launch_bounds__(FwdCfg<D, CG>::kThreads, 1)
             }
             tmem_wait_st();
           };
-          mbar_wait(bar_s_full + 8 * i, j & 1);
+          mbar_wait(bar_s_full + 8 * i, t & 1);
           tc_fence_after();
 #ifndef SRA_FWD_SKEL  // (ablation builds only: MMAs, TMA and barriers without the softmax arithmetic; results are wrong)
-          // s_full(j) completed => every earlier MMA, including O_i += P_i V_{j-1}, is complete.
-          if (j > 0 && __any_sync(0xffffffffu, (m_seen[i] - m_ref[i]) * sl2 > 8.0f)) rescale_to(fmaxf(m_ref[i], m_seen[i]));
+          // s_full completed => every earlier MMA, including this slot's previous O_i += P_i V, is complete.
+          if (t > 0 && __any_sync(0xffffffffu, (m_seen[i] - m_ref[i]) * sl2 > 8.0f)) rescale_to(fmaxf(m_ref[i], m_seen[i]));
           uint32_t pk[2][16];
           float l_tile = 0.f, mt = -INFINITY;
 #pragma unroll 1
@@ -291,7 +298,7 @@ __global__ void __launch_bounds__(FwdCfg<D, CG>::kThreads, 1)
             // the same in both warps of a row (same mt, same m_ref)
             if (pass == 1 || !__any_sync(0xffffffffu, !((mt - m_ref[i]) * sl2 <= 64.0f))) break;
             const float m_new = fmaxf(m_ref[i], mt);
-            if (j > 0) rescale_to(m_new); else m_ref[i] = m_new;
+            if (t > 0) rescale_to(m_new); else m_ref[i] = m_new;
           }
           m_seen[i] = fmaxf(m_seen[i], mt);
           l[i] += l_tile;
@@ -322,14 +329,24 @@ __global__ void __launch_bounds__(FwdCfg<D, CG>::kThreads, 1)
       }
     }
     // ---------------------------------------------------- epilogue (a5): O / l -> bf16, LSE
+    // (DUAL: one output tile from the two slots' partial states: O = a_0 O_0 + a_1 O_1, l = a_0 l_0 + a_1 l_1 with
+    //  a_i = 2^((m_ref_i - m) sl2), m = max(m_ref_0, m_ref_1))
 #pragma unroll
     for (int i = 0; i < 2; ++i) {
-      if (i < n_qt) {
+      if (i < (dual ? 1 : n_qt)) {
         const uint32_t tO = tO0 + i * D + lane_off + hh * (D / 2);
         mbar_wait(bar_o_full + 8 * i, 0);
+        if (dual) mbar_wait(bar_o_full + 8, 0);
         tc_fence_after();
-        post(l[i]);
-        const float l_row = l[i] + fetch();
+        float a0 = 1.f, a1 = 0.f, m_out = m_ref[i];
+        if (dual) {
+          m_out = fmaxf(m_ref[0], m_ref[1]);
+          a0 = ex2((m_ref[0] - m_out) * sl2);
+          a1 = ex2((m_ref[1] - m_out) * sl2);
+        }
+        const float l_mine = dual ? l[0] * a0 + l[1] * a1 : l[i];
+        post(l_mine);
+        const float l_row = l_mine + fetch();
         const int row = slot_row(i) + row_in_tile;
         const bool valid = row < item.q_rows;
         const int n_tok = q_is_ref ? p.n_ref : p.n_gen;
@@ -337,26 +354,41 @@ __global__ void __launch_bounds__(FwdCfg<D, CG>::kThreads, 1)
         __nv_bfloat16* obase = q_is_ref ? p.o_ref : p.o_gen;
         uint4* orow = reinterpret_cast<uint4*>(obase + ((size_t(b) * n_tok + grow) * p.heads + h) * D + hh * (D / 2));
         const float inv_l = 1.0f / l_row;
+        const float w0 = a0 * inv_l, w1 = a1 * inv_l;
+        // this thread's half row of O, 32 columns at a time, normalised (and merged)
+        auto load_o = [&](int c, uint32_t (&o)[32]) {
+          tmem_ld32(tO + c * 32, o);
+          tmem_wait_ld();
+          if (dual) {
+            uint32_t o1[32];
+            tmem_ld32(tO + D + c * 32, o1);
+            tmem_wait_ld();
+#pragma unroll
+            for (int k = 0; k < 32; ++k) o[k] = __float_as_uint(__uint_as_float(o[k]) * w0 + __uint_as_float(o1[k]) * w1);
+          } else {
+#pragma unroll
+            for (int k = 0; k < 32; ++k) o[k] = __float_as_uint(__uint_as_float(o[k]) * inv_l);
+          }
+        };
         if (split == 0) {
 #pragma unroll
           for (int c = 0; c < D / 64; ++c) {
             uint32_t o[32];
-            tmem_ld32(tO + c * 32, o);
-            tmem_wait_ld();
+            load_o(c, o);
             if (valid) {
 #pragma unroll
               for (int q = 0; q < 4; ++q) {
                 uint4 v;
-                v.x = pack_bf16(__uint_as_float(o[8 * q + 0]) * inv_l, __uint_as_float(o[8 * q + 1]) * inv_l);
-                v.y = pack_bf16(__uint_as_float(o[8 * q + 2]) * inv_l, __uint_as_float(o[8 * q + 3]) * inv_l);
-                v.z = pack_bf16(__uint_as_float(o[8 * q + 4]) * inv_l, __uint_as_float(o[8 * q + 5]) * inv_l);
-                v.w = pack_bf16(__uint_as_float(o[8 * q + 6]) * inv_l, __uint_as_float(o[8 * q + 7]) * inv_l);
+                v.x = pack_bf16(__uint_as_float(o[8 * q + 0]), __uint_as_float(o[8 * q + 1]));
+                v.y = pack_bf16(__uint_as_float(o[8 * q + 2]), __uint_as_float(o[8 * q + 3]));
+                v.z = pack_bf16(__uint_as_float(o[8 * q + 4]), __uint_as_float(o[8 * q + 5]));
+                v.w = pack_bf16(__uint_as_float(o[8 * q + 6]), __uint_as_float(o[8 * q + 7]));
                 orow[c * 4 + q] = v;
               }
             }
           }
           float* lse = q_is_ref ? p.lse_ref : p.lse_gen;
-          if (lse != nullptr && valid && hh == 0) lse[(size_t(b) * p.heads + h) * n_tok + grow] = m_ref[i] * p.scale + __logf(l_row);
+          if (lse != nullptr && valid && hh == 0) lse[(size_t(b) * p.heads + h) * n_tok + grow] = m_out * p.scale + __logf(l_row);
         } else {
           // key split: fp32 partial (O_s, LSE_s) of generation rows, head-major so the merge kernel streams it
           const size_t prow = ((size_t(split - 1) * p.batch + b) * p.heads + h) * p.n_gen + grow;
@@ -364,16 +396,15 @@ __global__ void __launch_bounds__(FwdCfg<D, CG>::kThreads, 1)
 #pragma unroll
           for (int c = 0; c < D / 64; ++c) {
             uint32_t o[32];
-            tmem_ld32(tO + c * 32, o);
-            tmem_wait_ld();
+            load_o(c, o);
             if (valid) {
 #pragma unroll
               for (int q = 0; q < 8; ++q)
-                dst[c * 8 + q] = make_float4(__uint_as_float(o[4 * q + 0]) * inv_l, __uint_as_float(o[4 * q + 1]) * inv_l,
-                                             __uint_as_float(o[4 * q + 2]) * inv_l, __uint_as_float(o[4 * q + 3]) * inv_l);
+                dst[c * 8 + q] = make_float4(__uint_as_float(o[4 * q + 0]), __uint_as_float(o[4 * q + 1]),
+                                             __uint_as_float(o[4 * q + 2]), __uint_as_float(o[4 * q + 3]));
             }
           }
-          if (valid && hh == 0) p.part_lse[prow] = m_ref[i] * p.scale + __logf(l_row);
+          if (valid && hh == 0) p.part_lse[prow] = m_out * p.scale + __logf(l_row);
         }
         tc_fence_before();
       }
@@ -439,6 +470,32 @@ __global__ void __launch_bounds__(FwdCfg<D, CG>::kThreads, 1)
       auto phase_of = [&](int it) { return uint32_t((it / C::kStages) & 1); };
 
       mbar_wait(bar_q_full, 0);
+      if (dual) {
+        // slot i = j & 1 takes key tile j (K_j at ring position 2 j, V_j at 2 j + 1); both Q slots hold the same tile
+        for (int i = 0; i < 2; ++i) {
+          mbar_wait(bar_kv_full + 8 * stage_of(2 * i), phase_of(2 * i));
+          tc_fence_after();
+          issue_qk(i, stage_of(2 * i));
+          umma_commit<CG>(bar_s_full + 8 * i);
+          umma_commit<CG>(bar_kv_empty + 8 * stage_of(2 * i));
+        }
+        for (int j = 0; j < n_kv; ++j) {
+          const int i = j & 1, t = j >> 1, itv = 2 * j + 1, itk = 2 * (j + 2);
+          mbar_wait(bar_kv_full + 8 * stage_of(itv), phase_of(itv));
+          mbar_wait(bar_p_full + 8 * i, t & 1);
+          tc_fence_after();
+          issue_pv(i, stage_of(itv), t > 0);
+          if (j + 2 >= n_kv) umma_commit<CG>(bar_o_full + 8 * i);
+          umma_commit<CG>(bar_kv_empty + 8 * stage_of(itv));
+          if (j + 2 < n_kv) {
+            mbar_wait(bar_kv_full + 8 * stage_of(itk), phase_of(itk));
+            tc_fence_after();
+            issue_qk(i, stage_of(itk));
+            umma_commit<CG>(bar_s_full + 8 * i);
+            umma_commit<CG>(bar_kv_empty + 8 * stage_of(itk));
+          }
+        }
+      } else {
       int it = 0;
       mbar_wait(bar_kv_full + 8 * stage_of(it), phase_of(it));
       tc_fence_after();
@@ -471,6 +528,7 @@ __global__ void __launch_bounds__(FwdCfg<D, CG>::kThreads, 1)
           }
         }
         if (more) ++it;
+      }
       }
     }
   }
