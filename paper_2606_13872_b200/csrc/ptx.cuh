@@ -24,7 +24,26 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
+// The suspend-time hint (ns) lets the hardware keep a waiting warp asleep until the phase completes instead of waking
+// it to re-issue the try_wait and its branch (ncu, forward kernel: 5.6 G BRA + 4.2 G SYNCS of 74 G issued warp
+// instructions, mostly the waiting MMA / TMA warps).  Measured worth 0.2-0.3 % on both contraction kernels.
+#ifndef SRA_WAIT_HINT_NS
+#define SRA_WAIT_HINT_NS 10000000
+#endif
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+#if SRA_WAIT_HINT_NS > 0
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "SRA_WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
+      "@p bra SRA_DONE_%=;\n\t"
+      "bra SRA_WAIT_%=;\n\t"
+      "SRA_DONE_%=:\n\t"
+      "}" ::"r"(bar),
+      "r"(parity), "r"(uint32_t(SRA_WAIT_HINT_NS))
+      : "memory");
+#else
   asm volatile(
       "{\n\t"
       ".reg .pred p;\n\t"
@@ -36,6 +55,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "}" ::"r"(bar),
       "r"(parity)
       : "memory");
+#endif
 }
 
 // Non-blocking: has the phase with this parity completed?
