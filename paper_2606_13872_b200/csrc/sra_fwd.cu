@@ -129,14 +129,15 @@ __global__ void __launch_bounds__(FwdCfg<D, CG>::kThreads, 1)
   const int n0 = (item.seg0_len + kTile - 1) / kTile;
   const int n1 = (item.seg1_len + kTile - 1) / kTile;
   const int n_kv = n0 + n1;
-  // DUAL (single-CTA kernel, a slab of at most 128 rows - the short-query regime): with one Q tile the second slot of
-  // TMEM would idle and every key tile would wait for the S -> softmax -> P -> PV chain of the one before it.  Instead
-  // both slots work on the SAME Q tile: slot i takes the key tiles j = i (mod 2) with its own running (m_ref, l, O),
-  // and the epilogue merges the two partial softmax states.  Two key tiles are then in flight, as with two Q tiles.
-  const bool dual = CG == 1 && item.q_rows <= kTile && n_kv >= 2;
+  // DUAL (a slab with one Q tile per CTA: the short-query regime, and the last slab of a frame or block): the second
+  // slot of TMEM would idle and every key tile would wait for the S -> softmax -> P -> PV chain of the one before it.
+  // Instead both slots work on the SAME Q tile: slot i takes the key tiles j = i (mod 2) with its own running
+  // (m_ref, l, O), and the epilogue merges the two partial softmax states.  Two key tiles are then in flight, as with
+  // two Q tiles.  (The same decision in both CTAs of a pair: it depends on the item only.)
+  const bool dual = item.q_rows <= kTile * CG && n_kv >= 2;
   const int n_qt = (item.q_rows > kTile * CG || dual) ? 2 : 1;  // TMEM slots in use (the same in both CTAs of a pair)
   const int n_steps = dual ? (n_kv + 1) / 2 : n_kv;             // iterations of the (step, slot) loops
-  auto slot_row = [&](int i) { return dual ? 0 : (CG * i + rank) * kTile; };  // first slab row of this CTA's slot i
+  auto slot_row = [&](int i) { return dual ? rank * kTile : (CG * i + rank) * kTile; };  // first slab row of this CTA's slot i
 
   if (threadIdx.x == 0) {
     mbar_init(bar_q_full, 1);

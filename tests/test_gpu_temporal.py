@@ -88,7 +88,10 @@ def test_temporal_window_covering_everything_is_plain_sra():
     t = sra_inputs.make_inputs(w, with_grad=True)
     base = run_gpu_forward(w, t, use_cache=True)
     got = _run(w, t, [0, 100, 200, 333], 2, None, backward=False)
-    assert_parity(got["o_gen"], base["o_gen"], "window >= n_frames - 1", rel_l2_tol=1e-3)
+    # (GPU against GPU: the same mask through a different slab partition.  The frame-cut slabs have one Q tile per CTA and
+    # run in dual-slot mode - two partial softmax states merged at the end - so the two results differ by the bf16
+    # rounding of P against different reference maxima; each is checked against the oracle in the tests above.)
+    assert_parity(got["o_gen"], base["o_gen"], "window >= n_frames - 1", rel_l2_tol=5e-3)
     assert np.array_equal(got["o_ref"], base["o_ref"])
 
 
