@@ -698,7 +698,6 @@ static int run_backward_core(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t s
 
 int run_backward(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t stream) {
   const sra_config& c = ctx->cfg;
-  const int B = c.batch, H = c.heads, d = c.head_dim;
   if (!a->q_gen || !a->k_gen || !a->v_gen || !a->o_gen || !a->lse_gen || !a->do_gen || !a->dq_gen || !a->dk_gen || !a->dv_gen)
     return ctx_fail(ctx, SRA_ERR_INVALID_ARG, "sra_backward: generation tensors (q,k,v,o,lse,do,dq,dk,dv) are required");
   const bool has_ref = c.n_ref > 0;
