@@ -39,6 +39,17 @@ namespace sra {
 #endif
 constexpr int kEmuPairsPer8 = SRA_FWD_EMU;
 
+// Development aid (-DSRA_FWD_TRACE): clock64 timestamps of the pipeline events of one CTA over a few key tiles.
+#ifdef SRA_FWD_TRACE
+__device__ long long* g_fwd_trace = nullptr;
+#define FTR(role, step, ev)                                                                                         \
+  do {                                                                                                              \
+    if (ftr_on && (step) >= 100 && (step) < 108 && g_fwd_trace) g_fwd_trace[((role) * 8 + ((step) - 100)) * 16 + (ev)] = clock64(); \
+  } while (0)
+#else
+#define FTR(role, step, ev) do { } while (0)
+#endif
+
 template <int D, int CG>
 struct FwdCfg {
   static_assert(CG == 1 || (CG == 2 && D == 128), "the CTA-pair kernel is built for head_dim 128");
@@ -139,6 +150,9 @@ __global__ void __launch_bounds__(FwdCfg<D, CG>::kThreads, 1)
   const int n_steps = dual ? (n_kv + 1) / 2 : n_kv;             // iterations of the (step, slot) loops
   auto slot_row = [&](int i) { return dual ? rank * kTile : (CG * i + rank) * kTile; };  // first slab row of this CTA's slot i
 
+#ifdef SRA_FWD_TRACE
+  const bool ftr_on = blockIdx.x == 4 && blockIdx.y == 0 && blockIdx.z == 0 && (threadIdx.x & 31) == 0;
+#endif
   if (threadIdx.x == 0) {
     mbar_init(bar_q_full, 1);
     for (int s = 0; s < C::kStages; ++s) {
@@ -236,8 +250,10 @@ __global__ void __launch_bounds__(FwdCfg<D, CG>::kThreads, 1)
             }
             tmem_wait_st();
           };
+          if ((warp & 3) == 0) FTR(2 * hh + i, t, 0);
           mbar_wait(bar_s_full + 8 * i, t & 1);
           tc_fence_after();
+          if ((warp & 3) == 0) FTR(2 * hh + i, t, 1);
 #ifndef SRA_FWD_SKEL  // (ablation builds only: MMAs, TMA and barriers without the softmax arithmetic; results are wrong)
           // s_full completed => every earlier MMA, including this slot's previous O_i += P_i V, is complete.
           if (t > 0 && __any_sync(0xffffffffu, (m_seen[i] - m_ref[i]) * sl2 > 8.0f)) rescale_to(fmaxf(m_ref[i], m_seen[i]));
@@ -293,8 +309,10 @@ __global__ void __launch_bounds__(FwdCfg<D, CG>::kThreads, 1)
             unpack2(la, l0, l1);
             unpack2(lb, l2, l3);
             l_tile = (l0 + l1) + (l2 + l3);
+            if ((warp & 3) == 0) FTR(2 * hh + i, t, 2);
             // Full-row tile max = max of the two halves.
             mt = fmaxf(mt_h, fetch());
+            if ((warp & 3) == 0) FTR(2 * hh + i, t, 3);
             // exact unless the tile leads m_ref by more than 2^64 (or m_ref is still -inf); the decision is
             // the same in both warps of a row (same mt, same m_ref)
             if (pass == 1 || !__any_sync(0xffffffffu, !((mt - m_ref[i]) * sl2 <= 64.0f))) break;
@@ -326,6 +344,7 @@ __global__ void __launch_bounds__(FwdCfg<D, CG>::kThreads, 1)
           if (lane == 0) {
             if (CG == 2) mbar_arrive_cluster(bar_p_full_leader + 8 * i); else mbar_arrive(bar_p_full + 8 * i);
           }
+          if ((warp & 3) == 0) FTR(2 * hh + i, t, 4);
         }
       }
     }
@@ -513,9 +532,12 @@ __global__ void __launch_bounds__(FwdCfg<D, CG>::kThreads, 1)
         const bool more = j + 1 < n_kv;
         const int sk = stage_of(it);
         for (int i = 0; i < n_qt; ++i) {
+          FTR(4 + i, j, 0);
           if (CG == 2) mbar_wait_cluster(bar_p_full + 8 * i, j & 1); else mbar_wait(bar_p_full + 8 * i, j & 1);
+          FTR(4 + i, j, 1);
           tc_fence_after();
           issue_pv(i, sv, j > 0);
+          FTR(4 + i, j, 2);
           if (!more) umma_commit<CG>(bar_o_full + 8 * i);
           if (i == n_qt - 1) umma_commit<CG>(bar_kv_empty + 8 * sv);
           if (more) {
@@ -525,6 +547,7 @@ __global__ void __launch_bounds__(FwdCfg<D, CG>::kThreads, 1)
             }
             issue_qk(i, sk);
             umma_commit<CG>(bar_s_full + 8 * i);
+            FTR(4 + i, j, 3);
             if (i == n_qt - 1) umma_commit<CG>(bar_kv_empty + 8 * sk);
           }
         }
@@ -638,6 +661,9 @@ cudaError_t launch_fwd_merge(const FwdParams& p, int head_dim, int n_split, cuda
   return cudaGetLastError();
 }
 
+#ifdef SRA_FWD_TRACE
+extern "C" void sra_dbg_set_fwd_trace(long long* p) { cudaMemcpyToSymbol(g_fwd_trace, &p, sizeof(p)); }
+#endif
 template cudaError_t launch_fwd<64, 1>(const CUtensorMap*, const FwdParams&, cudaStream_t);
 template cudaError_t launch_fwd<128, 1>(const CUtensorMap*, const FwdParams&, cudaStream_t);
 template cudaError_t launch_fwd<128, 2>(const CUtensorMap*, const FwdParams&, cudaStream_t);
