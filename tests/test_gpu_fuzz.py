@@ -130,3 +130,71 @@ def test_random_configuration(case):
                 if len(big):
                     assert_parity(gr[b, big], bref[n][b, big], what + f" {n} item {b} (blocks >= 16 tokens)",
                                   rel_l2_tol=rel_tol(bref[n][b, big]), **abs_tol(bref[n][b, big]))
+
+
+def _draw_host(case):
+    rng = np.random.default_rng(5000 + case)
+    B_ = int(rng.integers(1, 3))
+    H = int(rng.integers(1, 3))
+    d = int(rng.choice([64, 128]))
+    n_gen = int(rng.choice([4096, 4100, 4611, 5000, 6000]))  # >= 16 query slabs: the pipelined host path
+    blocks = tuple(int(rng.choice([1, 130, 257, 700])) for _ in range(int(rng.integers(0, 4))))
+    window, frames = -1, None
+    if rng.random() < 0.4:
+        n_fr = int(rng.integers(2, 7))
+        cuts = sorted(set(int(x) for x in rng.integers(1, n_gen, size=n_fr - 1)))
+        frames = [0] + cuts + [n_gen]
+        window = int(rng.integers(0, 3))
+    n_ref = sum(blocks)
+    valid = None
+    if n_ref and rng.random() < 0.5:
+        valid = (rng.random(n_ref) < 0.7) if rng.random() < 0.5 else (rng.random((B_, n_ref)) < 0.6)
+    with_ref_rows = bool(n_ref and rng.random() < 0.7)
+    return B_, H, d, n_gen, blocks, frames, window, valid, with_ref_rows
+
+
+@pytest.mark.parametrize("case", range(10))
+def test_random_configuration_through_the_host_path(case):
+    """sra_forward_host (pipelined: >= 16 query slabs) on random configurations: slab chunks snapped to CTA pairs and
+    frames, reference-first phase on or off, strided copies for batch 2, gathered reference rows under a mask - every
+    row against the numpy oracle, twice (the second call runs with the measured rates of the first)."""
+    from paper_2606_13872_b200 import binding as B
+    B_, H, d, n_gen, blocks, frames, window, valid, with_ref_rows = _draw_host(case)
+    w = sra_inputs.SRAWorkload(f"fuzzhost{case}", B_, H, d, n_gen, blocks, "B", 90 + case)
+    t = sra_inputs.make_inputs(w)
+    dev = torch.device("cuda:0")
+    has_ref = w.n_ref > 0
+    what = f"host case {case}: B{B_} H{H} d{d} gen {n_gen} blocks {blocks} frames {frames} w {window} valid {None if valid is None else valid.shape} ref rows {with_ref_rows}"
+    tb = bits(t)
+    a6 = [tb.get(k) for k in ("q_gen", "k_gen", "v_gen", "q_ref", "k_ref", "v_ref")]
+    ref = sra_oracle.sra_forward(*a6, w.ref_block_offsets, 1.0 / math.sqrt(d), valid=valid, gen_frame_offsets=frames, window=window)
+    ctx = B.sra_create(w.batch, w.heads, w.head_dim, w.n_gen, w.ref_block_offsets)
+    try:
+        if frames is not None:
+            B.sra_set_temporal_window(ctx, frames, window)
+        if valid is not None:
+            B.sra_set_reference_validity(ctx, valid)
+        if has_ref:
+            B.sra_cache_reference_kv(ctx, t["k_ref"].to(dev), t["v_ref"].to(dev))
+        h = {k: t[k].pin_memory() for k in ("q_gen", "k_gen", "v_gen", "q_ref")}
+        o_gen = torch.full(t["q_gen"].shape, float("nan"), dtype=torch.bfloat16).pin_memory()
+        lse_gen = torch.full((B_, H, n_gen), float("nan")).pin_memory()
+        o_ref = torch.full(t["q_ref"].shape, float("nan"), dtype=torch.bfloat16).pin_memory() if with_ref_rows else None
+        for _ in range(2):
+            B.sra_forward_host(ctx, h["q_gen"], h["k_gen"], h["v_gen"], o_gen, q_ref=h["q_ref"] if with_ref_rows else None,
+                               o_ref=o_ref, lse_gen=lse_gen)
+            torch.cuda.synchronize()
+            assert_parity(o_gen.float().numpy(), ref["o_gen"], what + " O_g")
+            assert np.abs(lse_gen.numpy() - ref["lse_gen"]).max() <= 2e-3, what
+            if with_ref_rows:
+                v2 = np.ones((B_, w.n_ref), dtype=bool) if valid is None else np.broadcast_to(valid, (B_, w.n_ref))
+                og = o_ref.float().numpy()
+                for b in range(B_):
+                    keep, inv = np.flatnonzero(v2[b]), np.flatnonzero(~v2[b])
+                    assert np.all(og[b, inv] == 0.0), what
+                    if len(keep):
+                        assert_parity(og[b, keep], ref["o_ref"][b, keep], what + f" O_r item {b}")
+                o_ref.fill_(float("nan"))
+            o_gen.fill_(float("nan"))
+    finally:
+        B.sra_destroy(ctx)
