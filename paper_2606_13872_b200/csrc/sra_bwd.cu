@@ -591,49 +591,48 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
   }
 }
 
-// a6: D_i = sum_c dO_ic O_ic and LSE_i * log2(e) for rows [G ; R]; one warp per (b, token, head) row.
+// a6: D_i = sum_c dO_ic O_ic and LSE_i * log2(e) for rows [G ; R].  A row of O or dO is D bf16 = D / 8 16-byte vectors:
+// D / 8 lanes per row (16 for d = 128, 8 for d = 64), 32 / (D / 8) rows per warp pass, 16 bytes per lane per tensor.
 template <int D>
 __global__ void sra_bwd_preprocess_kernel(const __nv_bfloat16* __restrict__ o_gen, const __nv_bfloat16* __restrict__ do_gen,
                                           const float* __restrict__ lse_gen, const __nv_bfloat16* __restrict__ o_ref,
                                           const __nv_bfloat16* __restrict__ do_ref, const float* __restrict__ lse_ref,
                                           float* __restrict__ delta, float* __restrict__ lse2, int B, int H, int n_gen,
                                           int n_ref, int n_pad) {
+  constexpr int LPR = D / 8;        // lanes per row
+  constexpr int RPW = 32 / LPR;     // rows per warp pass
   const int lane = threadIdx.x & 31;
+  const int sub = lane / LPR, li = lane % LPR;
   const size_t warp_id = (blockIdx.x * size_t(blockDim.x) + threadIdx.x) >> 5;
   const size_t n_warps = (gridDim.x * size_t(blockDim.x)) >> 5;
   const size_t n_cat = size_t(n_gen) + n_ref;
   const size_t total = size_t(B) * n_cat * H;
-  for (size_t r = warp_id; r < total; r += n_warps) {
-    const int h = int(r % H);
-    const size_t t = r / H;
+  for (size_t r0 = warp_id * RPW; r0 < total; r0 += n_warps * RPW) {
+    const size_t r = r0 + sub;
+    const bool ok = r < total;
+    const size_t rr = ok ? r : total - 1;
+    const int h = int(rr % H);
+    const size_t t = rr / H;
     const int n = int(t % n_cat);
     const int b = int(t / n_cat);
     const bool is_ref = n >= n_gen;
     const int row = is_ref ? n - n_gen : n;
     const int n_tok = is_ref ? n_ref : n_gen;
     const size_t off = ((size_t(b) * n_tok + row) * H + h) * D;
-    const __nv_bfloat16* o = (is_ref ? o_ref : o_gen) + off;
-    const __nv_bfloat16* d = (is_ref ? do_ref : do_gen) + off;
+    const uint4 a = reinterpret_cast<const uint4*>((is_ref ? o_ref : o_gen) + off)[li];
+    const uint4 c = reinterpret_cast<const uint4*>((is_ref ? do_ref : do_gen) + off)[li];
+    const __nv_bfloat162* a2 = reinterpret_cast<const __nv_bfloat162*>(&a);
+    const __nv_bfloat162* c2 = reinterpret_cast<const __nv_bfloat162*>(&c);
     float acc = 0.f;
-    if (D == 128) {
-      const uint2 a = reinterpret_cast<const uint2*>(o)[lane], c = reinterpret_cast<const uint2*>(d)[lane];
-      const __nv_bfloat162* a2 = reinterpret_cast<const __nv_bfloat162*>(&a);
-      const __nv_bfloat162* c2 = reinterpret_cast<const __nv_bfloat162*>(&c);
 #pragma unroll
-      for (int k = 0; k < 2; ++k) {
-        const float2 x = __bfloat1622float2(a2[k]), y = __bfloat1622float2(c2[k]);
-        acc = fmaf(x.x, y.x, acc);
-        acc = fmaf(x.y, y.y, acc);
-      }
-    } else {
-      const uint32_t a = reinterpret_cast<const uint32_t*>(o)[lane], c = reinterpret_cast<const uint32_t*>(d)[lane];
-      const float2 x = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&a));
-      const float2 y = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&c));
-      acc = fmaf(x.x, y.x, x.y * y.y);
+    for (int k = 0; k < 4; ++k) {
+      const float2 x = __bfloat1622float2(a2[k]), y = __bfloat1622float2(c2[k]);
+      acc = fmaf(x.x, y.x, acc);
+      acc = fmaf(x.y, y.y, acc);
     }
 #pragma unroll
-    for (int m = 16; m > 0; m >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, m);
-    if (lane == 0) {
+    for (int m = LPR / 2; m > 0; m >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, m);
+    if (ok && li == 0) {
       const size_t w = (size_t(b) * H + h) * n_pad + n;
       delta[w] = acc;
       const float l = (is_ref ? lse_ref : lse_gen)[(size_t(b) * H + h) * n_tok + row];
@@ -754,7 +753,7 @@ static int run_backward_core(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t s
   {  // a6
     const size_t rows = size_t(B) * n_cat * H;
     const int threads = 256;
-    const int blocks = grid_for(ctx, rows * 32, threads, 32);
+    const int blocks = grid_for(ctx, rows * (d / 8), threads, 32);  // d / 8 lanes per row
     KernelTimer kt(ctx, SRA_KERNEL_BWD_PREPROCESS, stream);
     auto launch = [&](auto kernel) {
       kernel<<<blocks, threads, 0, stream>>>(
