@@ -30,11 +30,12 @@
  *   - Calls are asynchronous on `cuda_stream` (a cudaStream_t passed as void*; NULL = legacy
  *     default stream).  Argument / launch errors are returned synchronously; execution
  *     faults surface at the caller's next synchronisation.
- *   - Inputs must be finite.  Masked keys never reach a softmax (scores are masked by selection, P = 0 exactly), but
- *     the ragged last tile of a key segment multiplies P = 0 with the V rows that follow the segment in memory (the
- *     neighbouring reference block or frame; zeros past the end of a tensor), so an Inf / NaN in such a row turns the
- *     outputs of rows that must not see it into NaN (0 * Inf).  Finite values, however large, are isolated exactly
- *     (tests: mask poison, bit-identical).
+ *   - Mask isolation holds for non-finite data too.  A query's outputs (and the gradients that depend only on what
+ *     that query sees) are unaffected by Inf / NaN in keys, values or queries it must not see: masked scores are
+ *     removed by selection (P = 0 exactly), and the ragged last tile of a reference block / of a temporal-window frame
+ *     is loaded through a tensor map bounded at the segment's end, so the neighbouring block's or frame's rows are
+ *     never fetched (they would meet P = 0 in an MMA: 0 * Inf = NaN).  Rows that DO see a non-finite value are
+ *     non-finite, as the definition says (tests/test_gpu_nonfinite.py).
  *   - One ctx is used from one thread at a time.  No CPU fallback exists: on a device that
  *     is not sm_100 every compute entry point returns SRA_ERR_UNSUPPORTED.
  */

@@ -64,6 +64,30 @@ int ctx_fail_cuda(sra_ctx* ctx, cudaError_t e, const char* what) {
 // bf16 tensor map over a [B, N, H, d] (token-major) or [B, H, N, d] (head-major) tensor; box = box_rows x 64
 // columns, 128-byte swizzle, OOB rows read as zero.  Token-major coordinates: (c, h, n, b); head-major: (c, n, h, b).
 // Encoded maps are kept in the ctx, keyed by everything they describe: a steady-state step re-encodes nothing.
+// (rows_bound < N: the same tensor, but rows [rows_bound, N) read as zero - sra_common.h BoundMaps)
+static int encode_tmap_bf16(sra_ctx* ctx, CUtensorMap* out, const void* ptr, int B, int N, int H, int d, bool head_major,
+                            int box_rows, int rows_bound) {
+  EncodeTiledFn enc = get_encode_fn();
+  if (!enc) return fail(ctx, SRA_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
+  cuuint64_t dims[4], strides[3];
+  cuuint32_t box[4], estr[4] = {1, 1, 1, 1};
+  const cuuint64_t row = cuuint64_t(d) * 2;
+  if (head_major) {
+    dims[0] = d; dims[1] = rows_bound; dims[2] = H; dims[3] = B;
+    strides[0] = row; strides[1] = row * N; strides[2] = row * N * H;
+    box[0] = 64; box[1] = box_rows; box[2] = 1; box[3] = 1;
+  } else {
+    dims[0] = d; dims[1] = H; dims[2] = rows_bound; dims[3] = B;
+    strides[0] = row; strides[1] = row * H; strides[2] = row * H * N;
+    box[0] = 64; box[1] = 1; box[2] = box_rows; box[3] = 1;
+  }
+  CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(ptr), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(ctx, SRA_ERR_CUDA, "cuTensorMapEncodeTiled failed: " + std::to_string(int(r)));
+  return SRA_OK;
+}
+
 int make_tmap_bf16(sra_ctx* ctx, CUtensorMap* out, const void* ptr, int B, int N, int H, int d, bool head_major,
                    int box_rows) {
   if (ctx) {
@@ -73,24 +97,7 @@ int make_tmap_bf16(sra_ctx* ctx, CUtensorMap* out, const void* ptr, int B, int N
         return SRA_OK;
       }
   }
-  EncodeTiledFn enc = get_encode_fn();
-  if (!enc) return fail(ctx, SRA_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
-  cuuint64_t dims[4], strides[3];
-  cuuint32_t box[4], estr[4] = {1, 1, 1, 1};
-  const cuuint64_t row = cuuint64_t(d) * 2;
-  if (head_major) {
-    dims[0] = d; dims[1] = N; dims[2] = H; dims[3] = B;
-    strides[0] = row; strides[1] = row * N; strides[2] = row * N * H;
-    box[0] = 64; box[1] = box_rows; box[2] = 1; box[3] = 1;
-  } else {
-    dims[0] = d; dims[1] = H; dims[2] = N; dims[3] = B;
-    strides[0] = row; strides[1] = row * H; strides[2] = row * H * N;
-    box[0] = 64; box[1] = 1; box[2] = box_rows; box[3] = 1;
-  }
-  CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(ptr), dims, strides, box, estr,
-                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  if (r != CUDA_SUCCESS) return fail(ctx, SRA_ERR_CUDA, "cuTensorMapEncodeTiled failed: " + std::to_string(int(r)));
+  if (int rc = encode_tmap_bf16(ctx, out, ptr, B, N, H, d, head_major, box_rows, N)) return rc;
   if (ctx) {
     constexpr size_t kMaxCached = 48;
     sra_ctx::TmapEntry e{ptr, B, N, H, d, box_rows, head_major, *out};
@@ -443,6 +450,20 @@ void build_schedule(sra_ctx* ctx) {
     std::copy(all[m].pair.begin(), all[m].pair.end(), ctx->st_pair.begin() + size_t(m) * ctx->pair_stride);
     std::copy(all[m].bwd.begin(), all[m].bwd.end(), ctx->st_bwd.begin() + size_t(m) * ctx->bwd_stride);
   }
+  // Segment ends that fall inside a tensor (sra_common.h BoundMaps): frame ends of a temporal window; block ends of
+  // each mask's compacted reference (the last block ends with the item's valid rows - zero padding or the tensor's own
+  // end follows, nothing to bound).
+  ctx->bound_ends.clear();
+  if (ctx->window >= 0 && ctx->gen_frames.size() >= 2)
+    for (size_t f = 1; f + 1 < ctx->gen_frames.size(); ++f) ctx->bound_ends.push_back(ctx->gen_frames[f]);
+  ctx->n_gen_ends = int(ctx->bound_ends.size());
+  ctx->ref_end_stride = 0;
+  for (int m = 0; m < M; ++m) ctx->ref_end_stride = std::max(ctx->ref_end_stride, int(ctx->offe_b[m].size()) - 2);
+  ctx->ref_end_stride = std::max(ctx->ref_end_stride, 0);
+  for (int m = 0; m < M; ++m)
+    for (int j = 0; j < ctx->ref_end_stride; ++j)
+      ctx->bound_ends.push_back(j + 2 < int(ctx->offe_b[m].size()) ? ctx->offe_b[m][j + 1] : INT32_MAX);
+  ctx->bound_version += 1;
   ctx->sched_dirty = true;
   ctx->seg_dirty = true;
 }
@@ -479,6 +500,12 @@ int ensure_schedule_capacity(sra_ctx* ctx) {
       if (e == cudaSuccess) ctx->cap_part_rows = prow;
     }
   }
+  // bounded tensor maps: 6 roles forward, 8 backward
+  const size_t n_ends = ctx->bound_ends.size();
+  if (e == cudaSuccess) e = ensure_pair(ctx->bnd_fwd.d_ends, ctx->bnd_fwd.cap_ends, n_ends);
+  if (e == cudaSuccess) e = ensure_pair(ctx->bnd_fwd.d_maps, ctx->bnd_fwd.cap_maps, 6 * n_ends);
+  if (e == cudaSuccess) e = ensure_pair(ctx->bnd_bwd.d_ends, ctx->bnd_bwd.cap_ends, n_ends);
+  if (e == cudaSuccess) e = ensure_pair(ctx->bnd_bwd.d_maps, ctx->bnd_bwd.cap_maps, 8 * n_ends);
   if (e != cudaSuccess) { (void)cudaGetLastError(); return e == cudaErrorMemoryAllocation ? SRA_ERR_OOM : SRA_ERR_CUDA; }
   return SRA_OK;
 }
@@ -517,6 +544,55 @@ int sync_schedule(sra_ctx* ctx, cudaStream_t stream) {
     }
     ctx->idx_dirty = false;
   }
+  return SRA_OK;
+}
+
+int bound_maps(sra_ctx* ctx, sra_ctx::BoundSet& bs, const sra_ctx::BoundRole* roles, int n_roles, cudaStream_t stream,
+               BoundMaps* out) {
+  const size_t n_total = ctx->bound_ends.size();
+  *out = BoundMaps{};
+#ifdef SRA_NO_BOUND  // (A/B builds: the kernels see no bounded maps)
+  return SRA_OK;
+#endif
+  if (n_total == 0) return SRA_OK;
+  // (a role the call does not pass - q_ref on a cached step - keeps the maps of the last call that did)
+  bool same = bs.version == ctx->bound_version && int(bs.roles.size()) == n_roles;
+  for (int r = 0; same && r < n_roles; ++r) same = roles[r].ptr == nullptr || bs.roles[r] == roles[r];
+  if (!same) {
+    std::vector<sra_ctx::BoundRole> merged(roles, roles + n_roles);
+    if (bs.version == ctx->bound_version && int(bs.roles.size()) == n_roles)
+      for (int r = 0; r < n_roles; ++r)
+        if (merged[r].ptr == nullptr) merged[r] = bs.roles[r];
+    roles = merged.data();
+    if (bs.cap_ends < n_total || bs.cap_maps < size_t(n_roles) * n_total)
+      return ctx_fail(ctx, SRA_ERR_CUDA, "bounded tensor-map buffers were not sized by the schedule build");
+    const sra_config& c = ctx->cfg;
+    bs.h_maps.assign(size_t(n_roles) * n_total, CUtensorMap{});
+    for (int r = 0; r < n_roles; ++r) {
+      if (!roles[r].ptr) continue;
+      const size_t i0 = roles[r].is_ref ? size_t(ctx->n_gen_ends) : 0, i1 = roles[r].is_ref ? n_total : size_t(ctx->n_gen_ends);
+      for (size_t i = i0; i < i1; ++i) {
+        const int end = ctx->bound_ends[i];
+        if (end <= 0 || end >= roles[r].N) continue;  // padding, or the tensor's own end
+        if (int rc = encode_tmap_bf16(ctx, &bs.h_maps[size_t(r) * n_total + i], roles[r].ptr, c.batch, roles[r].N, c.heads,
+                                      c.head_dim, roles[r].head_major, roles[r].box_rows, end))
+          return rc;
+      }
+    }
+    const int nb = bs.buf ^ 1;
+    cudaError_t e = cudaMemcpyAsync(bs.d_ends[nb], ctx->bound_ends.data(), n_total * sizeof(int32_t), cudaMemcpyHostToDevice, stream);
+    if (e == cudaSuccess)
+      e = cudaMemcpyAsync(bs.d_maps[nb], bs.h_maps.data(), bs.h_maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice, stream);
+    if (e != cudaSuccess) return ctx_fail_cuda(ctx, e, "bounded tensor-map upload");
+    bs.buf = nb;
+    bs.version = ctx->bound_version;
+    bs.roles.assign(roles, roles + n_roles);
+  }
+  out->maps = bs.d_maps[bs.buf];
+  out->ends = bs.d_ends[bs.buf];
+  out->n_gen_ends = ctx->n_gen_ends;
+  out->ref_stride = ctx->ref_end_stride;
+  out->n_total = int(n_total);
   return SRA_OK;
 }
 
@@ -690,6 +766,8 @@ void sra_destroy(sra_ctx* ctx) {
     for (int i = 0; i < 2; ++i) {
       cudaFree(ctx->d_fwd_items[i]); cudaFree(ctx->d_pair_items[i]); cudaFree(ctx->d_split_items[i]);
       cudaFree(ctx->d_bwd_items[i]); cudaFree(ctx->d_seg_items[i]);
+      cudaFree(ctx->bnd_fwd.d_maps[i]); cudaFree(ctx->bnd_fwd.d_ends[i]);
+      cudaFree(ctx->bnd_bwd.d_maps[i]); cudaFree(ctx->bnd_bwd.d_ends[i]);
     }
     cudaFree(ctx->ws_part_o);
     cudaFree(ctx->ws_part_lse);
@@ -922,6 +1000,15 @@ static int forward_core(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) 
   p.lse_gen = a->lse_gen;
   p.lse_ref = a->lse_ref;
   p.ref_kv_head_major = use_cache ? 1 : 0;
+  {
+    const void* kr = nr > 0 ? (use_cache ? ctx->cache_k : a->k_ref) : nullptr;
+    const void* vr = nr > 0 ? (use_cache ? ctx->cache_v : a->v_ref) : nullptr;
+    const sra_ctx::BoundRole roles[6] = {{a->k_gen, c.n_gen, false, false, k_box}, {a->v_gen, c.n_gen, false, false, kTile},
+                                         {kr, nr, true, use_cache, k_box}, {vr, nr, true, use_cache, kTile},
+                                         {a->q_gen, c.n_gen, false, false, kTile},
+                                         {with_ref_rows ? a->q_ref : nullptr, nr, true, false, kTile}};
+    if ((rc = sra::bound_maps(ctx, ctx->bnd_fwd, roles, 6, cudaStream_t(cuda_stream), &p.bound))) return rc;
+  }
   cudaError_t e;
   {
     sra::KernelTimer kt(ctx, SRA_KERNEL_FWD, cudaStream_t(cuda_stream));

@@ -451,16 +451,31 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
       // ================================================= loader: K/V once, then per tile Q_i (3 stages), {-lse2, delta}
       // (2 slots, written by the 32 lanes) and dO_i (one buffer, free once dV(i-1) is done)
       const bool k_hm = item.k_is_ref && p.ref_kv_head_major;
+      // Ragged tiles whose segment ends inside its tensor go through the maps bounded at the segment end
+      // (sra_common.h BoundMaps): the rows behind the end read as zero, not as the neighbouring block's or frame's.
+      const CUtensorMap* tk = item.k_is_ref ? &tm_k_ref : &tm_k_gen;
+      const CUtensorMap* tv = item.k_is_ref ? &tm_v_ref : &tm_v_gen;
+      if (p.bound.maps != nullptr && item.k_rows < kTile) {
+        const int ix = bound_index(p.bound, item.k_is_ref != 0, p.item_batch_stride ? b : 0, item.k_row0 + item.k_rows);
+        if (ix >= 0) { tk = p.bound.maps + (item.k_is_ref ? 6 : 2) * p.bound.n_total + ix; tv = tk + p.bound.n_total; }
+      }
+      // (the ragged last query tile of a segment: searched when it comes up, once per segment)
+      auto tail_q = [&](const QTile& qt) -> const CUtensorMap* {
+        if (p.bound.maps == nullptr || qt.valid == QT) return nullptr;
+        const int ix = bound_index(p.bound, qt.is_ref != 0, p.item_batch_stride ? b : 0, qt.row0 + qt.valid);
+        return ix >= 0 ? p.bound.maps + (qt.is_ref ? 4 : 0) * p.bound.n_total + ix : nullptr;
+      };
       if (lane == 0) {
         mbar_arrive_expect_tx(bar_kv_full, 2 * C::kKBytes);
-        bwd_load_tile<D>(sK, item.k_is_ref ? &tm_k_ref : &tm_k_gen, bar_kv_full, item.k_row0, h, b, k_hm);
-        bwd_load_tile<D>(sV, item.k_is_ref ? &tm_v_ref : &tm_v_gen, bar_kv_full, item.k_row0, h, b, k_hm);
+        bwd_load_tile<D>(sK, tk, bar_kv_full, item.k_row0, h, b, k_hm);
+        bwd_load_tile<D>(sV, tv, bar_kv_full, item.k_row0, h, b, k_hm);
       }
       const float* lse2 = p.lse2 + size_t(bh) * p.n_pad;
       const float* delta = p.delta + size_t(bh) * p.n_pad;
       for (int it = 0; it < n_it; ++it) {
         const int s = it % ST, vs = it % VS;
         const QTile qt = q_tile_of(tile_of(it), n0, item, p.n_gen);
+        const CUtensorMap* tq_tail = tail_q(qt);  // Q map; the dO map of the same end sits n_total entries behind it
         // the tile's row constants, fetched before any wait so that their latency hides behind it
         float nl[QT / 32], dl[QT / 32];
 #pragma unroll
@@ -475,7 +490,7 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
         TR(4, 1);
         if (lane == 0) {
           mbar_arrive_expect_tx(bar_q_full + 8 * s, C::kQBytes);
-          bwd_load_tile<D>(sQ + s * C::kQBytes, qt.is_ref ? &tm_q_ref : &tm_q_gen, bar_q_full + 8 * s, qt.row0, h, b, false);
+          bwd_load_tile<D>(sQ + s * C::kQBytes, tq_tail ? tq_tail : (qt.is_ref ? &tm_q_ref : &tm_q_gen), bar_q_full + 8 * s, qt.row0, h, b, false);
         }
         mbar_wait(bar_vec_empty + 8 * vs, ((it / VS) & 1) ^ 1);
         TR(4, 2);
@@ -491,7 +506,7 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
         TR(4, 3);
         if (lane == 0) {
           mbar_arrive_expect_tx(bar_do_full, C::kQBytes);
-          bwd_load_tile<D>(sDO, qt.is_ref ? &tm_do_ref : &tm_do_gen, bar_do_full, qt.row0, h, b, false);
+          bwd_load_tile<D>(sDO, tq_tail ? tq_tail + p.bound.n_total : (qt.is_ref ? &tm_do_ref : &tm_do_gen), bar_do_full, qt.row0, h, b, false);
         }
       }
     } else if (warp == C::kMmaWarp && elect_one()) {
@@ -793,6 +808,16 @@ static int run_backward_core(sra_ctx* ctx, const sra_bwd_args* a, cudaStream_t s
   p.dk_gen = static_cast<__nv_bfloat16*>(a->dk_gen); p.dv_gen = static_cast<__nv_bfloat16*>(a->dv_gen);
   p.dk_ref = static_cast<__nv_bfloat16*>(a->dk_ref); p.dv_ref = static_cast<__nv_bfloat16*>(a->dv_ref);
   p.ref_kv_head_major = use_cache ? 1 : 0;
+  {
+    const void* kr = has_ref ? (use_cache ? ctx->cache_k : a->k_ref) : nullptr;
+    const void* vr = has_ref ? (use_cache ? ctx->cache_v : a->v_ref) : nullptr;
+    const sra_ctx::BoundRole roles[8] = {
+        {a->q_gen, c.n_gen, false, false, kBwdQTile}, {a->do_gen, c.n_gen, false, false, kBwdQTile},
+        {a->k_gen, c.n_gen, false, false, kTile},     {a->v_gen, c.n_gen, false, false, kTile},
+        {has_ref ? a->q_ref : nullptr, nr, true, false, kBwdQTile}, {has_ref ? a->do_ref : nullptr, nr, true, false, kBwdQTile},
+        {kr, nr, true, use_cache, kTile},             {vr, nr, true, use_cache, kTile}};
+    if ((rc = bound_maps(ctx, ctx->bnd_bwd, roles, 8, stream, &p.bound))) return rc;
+  }
   {
     KernelTimer kt(ctx, SRA_KERNEL_BWD_MAIN, stream);
     e = d == 128 ? launch_bwd<128>(m, p, stream) : launch_bwd<64>(m, p, stream);

@@ -36,6 +36,31 @@ struct BwdItem {
   int32_t pad[1];
 };
 
+// Bounded tensor maps (mask isolation also for non-finite data).  The last tile of a key or query segment that ends
+// INSIDE its tensor (a reference block, a frame of a temporal window) is loaded through a copy of the tensor map whose
+// row dimension ends at the segment end: TMA then zero-fills the rows behind it instead of fetching the neighbouring
+// block's or frame's, so a masked P = 0 never meets a neighbour's Inf / NaN in an MMA (0 * Inf = NaN).
+struct BoundMaps {
+  const CUtensorMap* maps;  // global memory, [roles][n_total]; null = no segment ends inside a tensor
+  const int32_t* ends;      // [n_gen_ends | n_masks x ref_stride] end rows, each list ascending (padding INT32_MAX)
+  int32_t n_gen_ends, ref_stride, n_total;
+};
+#ifdef __CUDACC__
+// Index of the map bounded at `end_row` (generation list, or reference list of mask `mask`), -1 = none (the end is the
+// tensor's own: the ordinary map already zero-fills there).
+__device__ __forceinline__ int bound_index(const BoundMaps& bm, bool is_ref, int mask, int end_row) {
+  if (bm.maps == nullptr) return -1;
+  const int base = is_ref ? bm.n_gen_ends + mask * bm.ref_stride : 0;
+  const int n = is_ref ? bm.ref_stride : bm.n_gen_ends;
+  int lo = 0, hi = n;
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    if (bm.ends[base + mid] < end_row) lo = mid + 1; else hi = mid;
+  }
+  return (lo < n && bm.ends[base + lo] == end_row) ? base + lo : -1;
+}
+#endif
+
 struct FwdParams {
   const FwdItem* items;
   int32_t n_items;
@@ -54,6 +79,7 @@ struct FwdParams {
   // key-split partials of short-query G slabs (null when the schedule has no splits)
   float* part_o;    // fp32 [n_split][B][H][n_gen][d]: O_s = P_s V_s / l_s
   float* part_lse;  // fp32 [n_split][B][H][n_gen]:    LSE_s (natural log of the scaled scores)
+  BoundMaps bound;  // roles: 0 K_g, 1 V_g, 2 K_r, 3 V_r, 4 Q_g, 5 Q_r
 };
 
 constexpr int kBwdQTile = 128;  // query rows per backward iteration (keys per CTA = kTile)
@@ -75,6 +101,7 @@ struct BwdParams {
   __nv_bfloat16* dk_ref;
   __nv_bfloat16* dv_ref;
   int32_t ref_kv_head_major;
+  BoundMaps bound;  // roles: 0 Q_g, 1 dO_g, 2 K_g, 3 V_g, 4 Q_r, 5 dO_r, 6 K_r, 7 V_r
 };
 
 }  // namespace sra

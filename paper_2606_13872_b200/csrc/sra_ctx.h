@@ -105,6 +105,26 @@ struct sra_ctx {
   };
   std::vector<TmapEntry> tmaps;
   size_t tmap_next = 0;
+  // Bounded tensor maps (sra_common.h BoundMaps): the segment ends that fall inside a tensor - frame ends of a
+  // temporal window, block ends of the (compacted) reference per mask - and, per kernel family, the device copies of
+  // the ends and of the maps encoded for the pointers of the last call (re-encoded only when a pointer or the
+  // schedule changes; double-buffered like the schedule).
+  std::vector<int32_t> bound_ends;  // [n_gen_ends | n_masks x ref_end_stride]
+  int n_gen_ends = 0, ref_end_stride = 0;
+  uint64_t bound_version = 0;
+  struct BoundRole {
+    const void* ptr; int N; bool is_ref, head_major; int box_rows;
+    bool operator==(const BoundRole& o) const { return ptr == o.ptr && N == o.N && is_ref == o.is_ref && head_major == o.head_major && box_rows == o.box_rows; }
+  };
+  struct BoundSet {
+    CUtensorMap* d_maps[2] = {nullptr, nullptr};
+    int32_t* d_ends[2] = {nullptr, nullptr};
+    size_t cap_maps = 0, cap_ends = 0;
+    int buf = 0;
+    uint64_t version = ~uint64_t(0);  // bound_version the device copy was built for
+    std::vector<BoundRole> roles;     // ... and the tensors
+    std::vector<CUtensorMap> h_maps;
+  } bnd_fwd, bnd_bwd;
   uint32_t reserved = 0;  // SRA_RESERVE_* already done
   int64_t launches = 0;
   // optional per-kernel timing (sra_set_kernel_timing)
@@ -148,6 +168,10 @@ int ctx_fail_cuda(sra_ctx* ctx, cudaError_t e, const char* what);
 int make_tmap_bf16(sra_ctx* ctx, CUtensorMap* out, const void* ptr, int B, int N, int H, int d, bool head_major,
                    int box_rows);
 int sync_schedule(sra_ctx* ctx, cudaStream_t stream);  // uploads a changed schedule / index arrays on `stream`
+// Device table of bounded maps for the given role tensors (encoded and uploaded on `stream` only when they differ
+// from the last call's); out->maps = null when no segment ends inside a tensor.
+int bound_maps(sra_ctx* ctx, sra_ctx::BoundSet& bs, const sra_ctx::BoundRole* roles, int n_roles, cudaStream_t stream,
+               BoundMaps* out);
 int reserve(sra_ctx* ctx, uint32_t what);
 int grid_for(const sra_ctx* ctx, size_t total, int threads = 256, int ctas_per_sm = 16);
 template <int D>

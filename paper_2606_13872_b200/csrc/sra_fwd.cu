@@ -25,6 +25,7 @@
 // CTAs' mbarriers, both CTAs' TMA loads report their bytes to the leader's kv_full barriers, and CTA 1's softmax
 // warps arrive remotely on the leader's p_full barriers.
 #include <algorithm>
+#include <type_traits>
 
 #include "ptx.cuh"
 #include "sra_common.h"
@@ -100,6 +101,12 @@ __device__ __forceinline__ void load_v_half(uint32_t dst, const CUtensorMap* tm,
                                             bool head_major, int rank) {
   if (head_major) tma_load_4d_pair(dst, tm, bar, 64 * rank, row, h, b);
   else tma_load_4d_pair(dst, tm, bar, 64 * rank, h, row, b);
+}
+
+// Map of `role` bounded at `end_row`, or null (sra_common.h BoundMaps).
+__device__ __forceinline__ const CUtensorMap* bound_lookup(const BoundMaps& bm, int role, bool is_ref, int mask, int end_row) {
+  const int ix = bound_index(bm, is_ref, mask, end_row);
+  return ix >= 0 ? bm.maps + role * bm.n_total + ix : nullptr;
 }
 
 template <int D, int CG>
@@ -438,30 +445,56 @@ __global__ void __launch_bounds__(FwdCfg<D, CG>::kThreads, 1)
       const CUtensorMap* tq = q_is_ref ? &tm_q_ref : &tm_q_gen;
       const uint32_t q_full_l = CG == 2 ? mapa_cluster(bar_q_full, 0) : bar_q_full;
       const uint32_t kv_full_l = CG == 2 ? mapa_cluster(bar_kv_full, 0) : bar_kv_full;
-      if (rank == 0) mbar_arrive_expect_tx(bar_q_full, n_qt * C::kTileBytes * CG);
-      for (int i = 0; i < n_qt; ++i) load_tile<D, CG>(sQ + i * C::kTileBytes, tq, q_full_l, item.q_row0 + slot_row(i), h, b, false);
-      int it = 0;
-      for (int j = 0; j < n_kv; ++j) {
-        const bool first = j < n0;
-        const bool is_ref = first ? (item.seg0_is_ref != 0) : true;
-        const int row = first ? item.seg0_start + j * kTile : item.seg1_start + (j - n0) * kTile;
-        const bool hm = is_ref && p.ref_kv_head_major;
+      // Two copies of the loader, chosen once per CTA.  BND: an item whose query slab or key segments can end INSIDE a
+      // tensor - a reference block (R items), a frame of a temporal window - loads its ragged tiles through the maps
+      // bounded at those ends (sra_common.h BoundMaps): the rows behind an end read as zero, not as the neighbouring
+      // block's or frame's (0 * Inf in the PV MMA; the softmax's warp-wide rescale votes would otherwise depend on a
+      // neighbour's Q rows).  Every other item runs the plain loop, whose per-tile latency is measurable in the step time
+      // (any run-time map selection in it costs 0.4-0.8 % at 720p).
+      auto run_loader = [&](auto bnd_tag) {
+        constexpr bool BND = decltype(bnd_tag)::value;
+        const int mask = p.item_batch_stride ? b : 0;
+        if (rank == 0) mbar_arrive_expect_tx(bar_q_full, n_qt * C::kTileBytes * CG);
+        const CUtensorMap* tq_tail = tq;
+        if (BND && slot_row(n_qt - 1) + kTile > item.q_rows) {
+          const CUtensorMap* m = bound_lookup(p.bound, q_is_ref ? 5 : 4, q_is_ref, mask, item.q_row0 + item.q_rows);
+          if (m != nullptr) tq_tail = m;
+        }
+        for (int i = 0; i < n_qt; ++i)
+          load_tile<D, CG>(sQ + i * C::kTileBytes, (BND && slot_row(i) + kTile > item.q_rows) ? tq_tail : tq, q_full_l,
+                           item.q_row0 + slot_row(i), h, b, false);
+        int it = 0;
+        for (int j = 0; j < n_kv; ++j) {
+          const bool first = j < n0;
+          const bool is_ref = first ? (item.seg0_is_ref != 0) : true;
+          const int row = first ? item.seg0_start + j * kTile : item.seg1_start + (j - n0) * kTile;
+          const bool hm = is_ref && p.ref_kv_head_major;
+          // (the table is searched when the ragged tile comes up: the loader runs a ring ahead of the MMAs)
+          const CUtensorMap* tk_tail = nullptr;
+          if (BND && (first ? j == n0 - 1 : j == n_kv - 1)) {
+            const int len = first ? item.seg0_len : item.seg1_len;
+            if (len % kTile != 0) tk_tail = bound_lookup(p.bound, is_ref ? 2 : 0, is_ref, mask, (first ? item.seg0_start : item.seg1_start) + len);
+          }
 #pragma unroll
-        for (int kv = 0; kv < 2; ++kv, ++it) {
-          const int s = it % C::kStages;
-          const uint32_t ph = (it / C::kStages) & 1;
-          const CUtensorMap* tm = kv == 0 ? (is_ref ? &tm_k_ref : &tm_k_gen) : (is_ref ? &tm_v_ref : &tm_v_gen);
-          mbar_wait(bar_kv_empty + 8 * s, ph ^ 1);
-          if (rank == 0) mbar_arrive_expect_tx(bar_kv_full + 8 * s, C::kTileBytes);
-          const uint32_t dst = sKV + s * C::kStageBytes;
-          if constexpr (CG == 1) {
-            load_tile<D, 1>(dst, tm, kv_full_l + 8 * s, row, h, b, hm);
-          } else {
-            if (kv == 0) load_k_half<D>(dst, tm, kv_full_l + 8 * s, row, h, b, hm, rank);
-            else load_v_half<D>(dst, tm, kv_full_l + 8 * s, row, h, b, hm, rank);
+          for (int kv = 0; kv < 2; ++kv, ++it) {
+            const int s = it % C::kStages;
+            const uint32_t ph = (it / C::kStages) & 1;
+            const CUtensorMap* tm = kv == 0 ? (is_ref ? &tm_k_ref : &tm_k_gen) : (is_ref ? &tm_v_ref : &tm_v_gen);
+            if (BND && tk_tail != nullptr) tm = tk_tail + kv * p.bound.n_total;
+            mbar_wait(bar_kv_empty + 8 * s, ph ^ 1);
+            if (rank == 0) mbar_arrive_expect_tx(bar_kv_full + 8 * s, C::kTileBytes);
+            const uint32_t dst = sKV + s * C::kStageBytes;
+            if constexpr (CG == 1) {
+              load_tile<D, 1>(dst, tm, kv_full_l + 8 * s, row, h, b, hm);
+            } else {
+              if (kv == 0) load_k_half<D>(dst, tm, kv_full_l + 8 * s, row, h, b, hm, rank);
+              else load_v_half<D>(dst, tm, kv_full_l + 8 * s, row, h, b, hm, rank);
+            }
           }
         }
-      }
+      };
+      if (p.bound.maps != nullptr && (q_is_ref || p.bound.n_gen_ends > 0)) run_loader(std::true_type{});
+      else run_loader(std::false_type{});
     } else if (warp == 8 && rank == 0 && elect_one()) {
       // ===================================================== MMA issuer (pair: the leader CTA only, M = 256)
       constexpr uint32_t idesc_qk = make_idesc_bf16(kTile * CG, kTile, 0, 0);
