@@ -407,14 +407,9 @@ __device__ __forceinline__ void ex2_emu2(uint64_t x, float& p0, float& p1) {
   const uint64_t magic = pack2(12582912.0f, 12582912.0f);
   const uint64_t xr = add2(xc, magic);
   const uint64_t r = sub2(xc, sub2(xr, magic));
-#ifdef SRA_EX2_DEG2  // (A/B builds: degree-2 minimax, max rel. error 1.7e-3 - half a bf16 ulp)
-  uint64_t p = fma2(pack2(0.23842893540859222f, 0.23842893540859222f), r, pack2(0.7034479975700378f, 0.7034479975700378f));
-  p = fma2(p, r, pack2(1.0004431009292603f, 1.0004431009292603f));
-#else
   uint64_t p = fma2(pack2(0.05517149344086647f, 0.05517149344086647f), r, pack2(0.24261094629764557f, 0.24261094629764557f));
   p = fma2(p, r, pack2(0.6932609677314758f, 0.6932609677314758f));
   p = fma2(p, r, pack2(0.9999280571937561f, 0.9999280571937561f));
-#endif
   float q0, q1, n0, n1;
   unpack2(p, q0, q1);
   unpack2(xr, n0, n1);
