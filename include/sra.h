@@ -262,6 +262,15 @@ int sra_batch_schedule_copy(const sra_ctx* ctx, int32_t batch_item, int32_t* ite
  * rows, run by a cluster of two CTAs that share every K/V tile (same 8-int32 layout).  Pure host logic. */
 int sra_pair_schedule_copy(const sra_ctx* ctx, int32_t* use_pairs, int32_t* items, int32_t capacity, int32_t* n_items);
 
+/* The segment ends that fall INSIDE a tensor (PAPER.md:85 reference blocks, PAPER.md:143 frames of a temporal window):
+ * the kernels load the ragged last tile of such a segment through a tensor map bounded at its end, so the rows of the
+ * neighbouring block / frame are never fetched (mask isolation for non-finite data, see the contract above).
+ * ends (HOST, capacity int32, may be NULL to query the count): [*n_gen_ends generation-row ends | n_masks x
+ * *ref_stride reference-row ends of each mask's compacted reference, ascending, padded with INT32_MAX]; *n_ends = the
+ * total count.  Pure host logic. */
+int sra_bound_ends_copy(const sra_ctx* ctx, int32_t* ends, int32_t capacity, int32_t* n_gen_ends, int32_t* ref_stride,
+                        int32_t* n_ends);
+
 /* Short-query schedules (north_star "cache-bound short-query cases"): when a context has fewer generation
  * slabs than about two per SM, sra_create cuts every generation slab into *n_split key ranges of whole
  * 128-key tiles; each range runs as its own CTA, writes an fp32 partial (O_s, LSE_s) into a ctx-owned

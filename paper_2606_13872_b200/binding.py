@@ -25,7 +25,7 @@ EXPORTS = (
     "sra_create", "sra_cache_reference_kv", "sra_cache_reference_kv_rope", "sra_apply_rope", "sra_forward", "sra_forward_host", "sra_backward", "sra_destroy", "sra_useful_flops",
     "sra_schedule_info", "sra_schedule_copy", "sra_cache_bytes", "sra_launch_count", "sra_status_string",
     "sra_last_error", "sra_set_kernel_timing", "sra_kernel_time_ms", "sra_split_schedule_copy", "sra_set_reference_validity", "sra_set_temporal_window",
-    "sra_reserve", "sra_set_reference_validity_batched", "sra_batch_schedule_copy", "sra_pair_schedule_copy",
+    "sra_reserve", "sra_set_reference_validity_batched", "sra_batch_schedule_copy", "sra_pair_schedule_copy", "sra_bound_ends_copy",
 )
 
 RESERVE_BACKWARD, RESERVE_HOST, RESERVE_VALIDITY = 1, 2, 4
@@ -99,6 +99,9 @@ lib.sra_batch_schedule_copy.restype = ctypes.c_int
 lib.sra_pair_schedule_copy.argtypes = [_ctx_p, ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32), ctypes.c_int32,
                                        ctypes.POINTER(ctypes.c_int32)]
 lib.sra_pair_schedule_copy.restype = ctypes.c_int
+lib.sra_bound_ends_copy.argtypes = [_ctx_p, ctypes.POINTER(ctypes.c_int32), ctypes.c_int32, ctypes.POINTER(ctypes.c_int32),
+                                    ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32)]
+lib.sra_bound_ends_copy.restype = ctypes.c_int
 lib.sra_set_temporal_window.argtypes = [_ctx_p, ctypes.c_int32, ctypes.POINTER(ctypes.c_int32), ctypes.c_int32]
 lib.sra_set_temporal_window.restype = ctypes.c_int
 lib.sra_split_schedule_copy.argtypes = [_ctx_p, ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32), ctypes.c_int32,
@@ -287,6 +290,20 @@ def sra_batch_schedule_copy(ctx: int, batch_item: int):
     buf = (ctypes.c_int32 * (8 * max(n.value, 1)))()
     _check(lib.sra_batch_schedule_copy(ctx, int(batch_item), buf, n.value, ctypes.byref(n)), ctx)
     return _items(buf, n.value)
+
+
+def sra_bound_ends_copy(ctx: int):
+    """(generation-row ends, [per-mask reference-row ends]) that fall inside a tensor (include/sra.h)."""
+    ng, rs, n = ctypes.c_int32(0), ctypes.c_int32(0), ctypes.c_int32(0)
+    _check(lib.sra_bound_ends_copy(ctx, None, 0, ctypes.byref(ng), ctypes.byref(rs), ctypes.byref(n)), ctx)
+    buf = (ctypes.c_int32 * max(n.value, 1))()
+    _check(lib.sra_bound_ends_copy(ctx, buf, n.value, ctypes.byref(ng), ctypes.byref(rs), ctypes.byref(n)), ctx)
+    vals = list(buf[:n.value])
+    gen = vals[:ng.value]
+    n_masks = (n.value - ng.value) // rs.value if rs.value else 0
+    pad = 2 ** 31 - 1
+    ref = [[v for v in vals[ng.value + m * rs.value: ng.value + (m + 1) * rs.value] if v != pad] for m in range(n_masks)]
+    return gen, ref
 
 
 def sra_pair_schedule_copy(ctx: int):

@@ -1358,6 +1358,19 @@ int sra_pair_schedule_copy(const sra_ctx* ctx, int32_t* use_pairs, int32_t* item
   return copy_items(ctx->pair_items, items, capacity, n_items);
 }
 
+int sra_bound_ends_copy(const sra_ctx* ctx, int32_t* ends, int32_t capacity, int32_t* n_gen_ends, int32_t* ref_stride,
+                        int32_t* n_ends) {
+  if (!ctx || !n_ends) return SRA_ERR_INVALID_ARG;
+  *n_ends = int32_t(ctx->bound_ends.size());
+  if (n_gen_ends) *n_gen_ends = ctx->n_gen_ends;
+  if (ref_stride) *ref_stride = ctx->ref_end_stride;
+  if (ends) {
+    if (capacity < *n_ends) return SRA_ERR_INVALID_ARG;
+    std::copy(ctx->bound_ends.begin(), ctx->bound_ends.end(), ends);
+  }
+  return SRA_OK;
+}
+
 int sra_split_schedule_copy(const sra_ctx* ctx, int32_t* n_split, int32_t* items, int32_t capacity, int32_t* n_items) {
   if (!ctx || !n_split) return SRA_ERR_INVALID_ARG;
   *n_split = ctx->n_split;

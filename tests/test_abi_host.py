@@ -288,6 +288,44 @@ def test_pair_schedule_covers_the_slab_schedule(heads, n_gen, blocks, frames, w)
         B.sra_destroy(ctx)
 
 
+def test_bound_ends_are_the_segment_ends_inside_the_tensors():
+    """sra_bound_ends_copy (mask isolation for non-finite data): the ends the kernels bound their ragged tiles at are
+    exactly the segment ends of the schedule that fall strictly inside a tensor - every reference block end but the
+    last (per mask, in the mask's compacted rows), every frame end but the last once a temporal window is set - computed
+    here independently from the block offsets, the frames and the validity flags."""
+    n_gen, off = 1000, [0, 130, 387, 451, 700]
+    ctx = B.sra_create(2, 2, 128, n_gen, off)
+    try:
+        assert B.sra_bound_ends_copy(ctx) == ([], [off[1:-1]])
+        fr = [0, 100, 357, 400, 777, 1000]
+        B.sra_set_temporal_window(ctx, fr, 1)
+        assert B.sra_bound_ends_copy(ctx) == (fr[1:-1], [off[1:-1]])
+        # every segment end of the forward schedule that is not a tensor end is in the table
+        gen, ref = B.sra_bound_ends_copy(ctx)
+        for it in B.sra_schedule_copy(ctx):
+            e0 = it["seg0_start"] + it["seg0_len"]
+            assert e0 in ((ref[0] + [off[-1]]) if it["seg0_is_ref"] else (gen + [n_gen]))
+            if it["seg1_len"]:
+                assert it["seg1_start"] + it["seg1_len"] in ref[0] + [off[-1]]
+            eq = it["q_row0"] + it["q_rows"]
+            if it["q_rows"] % 128:
+                assert eq in ((ref[0] + [off[-1]]) if it["q_is_ref"] else (gen + [n_gen]))
+        B.sra_set_temporal_window(ctx, None, -1)
+        # per-sample validity: the ends of each item's COMPACTED blocks (empty blocks vanish)
+        rng = np.random.default_rng(2)
+        valid = rng.random((2, off[-1])) < 0.5
+        valid[1, off[1]:off[2]] = False
+        B.sra_set_reference_validity(ctx, valid)
+        gen, ref = B.sra_bound_ends_copy(ctx)
+        assert gen == []
+        for b in range(2):
+            counts = [int(valid[b, off[j]:off[j + 1]].sum()) for j in range(len(off) - 1)]
+            ends = np.cumsum([c for c in counts if c > 0]).tolist()
+            assert ref[b] == ends[:-1]
+    finally:
+        B.sra_destroy(ctx)
+
+
 def test_per_sample_validity_schedules():
     """sra_set_reference_validity_batched (reading A12; "validity masks are precomputed per-rank"): each
     batch item gets the schedule of its own compacted reference - mapped back through its compaction it covers exactly
