@@ -284,6 +284,41 @@ int sra_split_schedule_copy(const sra_ctx* ctx, int32_t* n_split, int32_t* items
  * a validity change until the cache is rebuilt).  The allocation itself is made at sra_create for n_ref rows. */
 int64_t sra_cache_bytes(const sra_ctx* ctx);
 
+/* ---- No-allocation entry point (an addition outside SURVEY.md 8; step a3) ------------------------
+ * For callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops, harnesses that forbid it): the
+ * generation rows' attention  O_g = softmax(s Q_g [K_g ; K_r]^T) [V_g ; V_r]  (+ LSE_g) with NO context - nothing to
+ * create, reserve or destroy.  It is sra_forward's key-split short-query path (fp32 partials per key range, then a
+ * merge); ALL of its scratch - work items and partials - lives in one file-scope `static __device__` array of
+ * SRA_STATIC_SCRATCH_BYTES that every GPU loading the library holds until the process exits.  The call does not
+ * allocate, free, copy from the host or synchronise, on any path.
+ *   - Tensors: DEVICE bf16 [batch, tokens, heads, head_dim] as for sra_forward; k_ref / v_ref are the caller's
+ *     (token-major) reference K / V - there is no resident cache without a context; NULL iff n_ref == 0.  Reference
+ *     ROWS are not computed (a cached denoising step).  lse_gen: DEVICE fp32 [batch, heads, n_gen] or NULL.
+ *   - n_split: key ranges per 256-row query slab, 0 = chosen to fill the GPU's SMs.
+ *   - Limit: 64 KiB + n_split * batch * heads * n_gen * (head_dim + 1) * 4 bytes (sra_static_scratch_bytes) must fit in
+ *     SRA_STATIC_SCRATCH_BYTES, and n_split * ceil(n_gen / 256) <= 2048; beyond that SRA_ERR_INVALID_ARG with the two
+ *     figures in sra_static_last_error() - use sra_create / sra_forward, whose workspaces are sized from the config.
+ *   - The array is SHARED by every call and keeps the last call's contents.  Nothing in it has to start at zero (each
+ *     call rewrites every byte it later reads), but calls that overlap on the GPU - two streams, two threads - race on
+ *     it: serialise them (one stream, or events).  Asynchronous on `cuda_stream` like every other entry point.
+ *   - Errors: status codes as above; the message is per host thread (sra_static_last_error). */
+#define SRA_STATIC_SCRATCH_BYTES (32u << 20)
+typedef struct {
+  int32_t batch, heads, head_dim; /* head_dim in {64, 128}                                                  */
+  int32_t n_gen, n_ref;           /* generation rows / keys, reference keys (0 = plain self-attention)      */
+  float softmax_scale;            /* <= 0: 1 / sqrt(head_dim)                                               */
+  int32_t device;                 /* CUDA ordinal, -1 = current                                             */
+  int32_t n_split;                /* 0 = automatic                                                          */
+  const void *q_gen, *k_gen, *v_gen;
+  const void *k_ref, *v_ref;
+  void* o_gen;
+  float* lse_gen;
+} sra_static_fwd_args;
+int sra_forward_gen_static(const sra_static_fwd_args* args, void* cuda_stream);
+/* Bytes of the static array a problem needs with `n_split` key ranges (pure host arithmetic). */
+int sra_static_scratch_bytes(const sra_static_fwd_args* args, int32_t n_split, int64_t* bytes);
+const char* sra_static_last_error(void);
+
 /* Optional per-kernel device timing (bench.py's roofline leg): when enabled, every launch is bracketed by
  * CUDA events recorded on the launching stream.  sra_kernel_time_ms returns the duration of the LAST launch
  * of kernel `which` (it synchronises on that launch's end event); SRA_ERR_INVALID_ARG if timing is off or the

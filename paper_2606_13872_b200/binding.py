@@ -26,7 +26,9 @@ EXPORTS = (
     "sra_schedule_info", "sra_schedule_copy", "sra_cache_bytes", "sra_launch_count", "sra_status_string",
     "sra_last_error", "sra_set_kernel_timing", "sra_kernel_time_ms", "sra_split_schedule_copy", "sra_set_reference_validity", "sra_set_temporal_window",
     "sra_reserve", "sra_set_reference_validity_batched", "sra_batch_schedule_copy", "sra_pair_schedule_copy", "sra_bound_ends_copy",
+    "sra_forward_gen_static", "sra_static_scratch_bytes", "sra_static_last_error",
 )
+STATIC_SCRATCH_BYTES = 32 << 20
 
 RESERVE_BACKWARD, RESERVE_HOST, RESERVE_VALIDITY = 1, 2, 4
 
@@ -63,7 +65,20 @@ class sra_bwd_args(ctypes.Structure):
                  "do_gen", "do_ref", "dq_gen", "dk_gen", "dv_gen", "dq_ref", "dk_ref", "dv_ref")]
 
 
+class sra_static_fwd_args(ctypes.Structure):
+    _fields_ = [("batch", ctypes.c_int32), ("heads", ctypes.c_int32), ("head_dim", ctypes.c_int32), ("n_gen", ctypes.c_int32),
+                ("n_ref", ctypes.c_int32), ("softmax_scale", ctypes.c_float), ("device", ctypes.c_int32),
+                ("n_split", ctypes.c_int32), ("q_gen", ctypes.c_void_p), ("k_gen", ctypes.c_void_p), ("v_gen", ctypes.c_void_p),
+                ("k_ref", ctypes.c_void_p), ("v_ref", ctypes.c_void_p), ("o_gen", ctypes.c_void_p), ("lse_gen", ctypes.c_void_p)]
+
+
 _ctx_p = ctypes.c_void_p
+lib.sra_forward_gen_static.argtypes = [ctypes.POINTER(sra_static_fwd_args), ctypes.c_void_p]
+lib.sra_forward_gen_static.restype = ctypes.c_int
+lib.sra_static_scratch_bytes.argtypes = [ctypes.POINTER(sra_static_fwd_args), ctypes.c_int32, ctypes.POINTER(ctypes.c_int64)]
+lib.sra_static_scratch_bytes.restype = ctypes.c_int
+lib.sra_static_last_error.argtypes = []
+lib.sra_static_last_error.restype = ctypes.c_char_p
 lib.sra_create.argtypes = [ctypes.POINTER(sra_config), ctypes.POINTER(_ctx_p)]
 lib.sra_create.restype = ctypes.c_int
 lib.sra_cache_reference_kv.argtypes = [_ctx_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
@@ -203,6 +218,30 @@ def sra_forward(ctx: int, q_gen, k_gen, v_gen, o_gen, q_ref=None, k_ref=None, v_
     a = sra_fwd_args(_ptr(q_gen), _ptr(k_gen), _ptr(v_gen), _ptr(q_ref), _ptr(k_ref), _ptr(v_ref),
                      _ptr(o_gen), _ptr(o_ref), _ptr(lse_gen), _ptr(lse_ref))
     _check(lib.sra_forward(ctx, ctypes.byref(a), _stream(stream)), ctx)
+
+
+def _static_args(q_gen, k_gen, v_gen, o_gen, k_ref, v_ref, lse_gen, n_split, softmax_scale, device):
+    bsz, n_gen, heads, d = q_gen.shape
+    n_ref = 0 if k_ref is None else k_ref.shape[1]
+    return sra_static_fwd_args(bsz, heads, d, n_gen, n_ref, float(softmax_scale), int(device), int(n_split), _ptr(q_gen),
+                               _ptr(k_gen), _ptr(v_gen), _ptr(k_ref), _ptr(v_ref), _ptr(o_gen), _ptr(lse_gen))
+
+
+def sra_forward_gen_static(q_gen, k_gen, v_gen, o_gen, k_ref=None, v_ref=None, lse_gen=None, n_split: int = 0,
+                           softmax_scale: float = 0.0, device: int = -1, stream=None) -> None:
+    """sra_forward_gen_static (include/sra.h): the generation rows' attention with no context and no allocation - its
+    scratch is the library's static device array (STATIC_SCRATCH_BYTES); calls that overlap on the GPU race on it."""
+    a = _static_args(q_gen, k_gen, v_gen, o_gen, k_ref, v_ref, lse_gen, n_split, softmax_scale, device)
+    status = lib.sra_forward_gen_static(ctypes.byref(a), _stream(stream))
+    if status != SRA_OK:
+        raise SRAError(status, lib.sra_static_last_error().decode())
+
+
+def sra_static_scratch_bytes(batch: int, heads: int, head_dim: int, n_gen: int, n_split: int) -> int:
+    a = sra_static_fwd_args(batch, heads, head_dim, n_gen, 0, 0.0, -1, n_split)
+    out = ctypes.c_int64(0)
+    _check(lib.sra_static_scratch_bytes(ctypes.byref(a), n_split, ctypes.byref(out)))
+    return out.value
 
 
 def _host_ptr(t) -> Optional[int]:

@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsra_b200.so")
-SOURCES = ["sra_api.cu", "sra_fwd.cu", "sra_bwd.cu"]
+SOURCES = ["sra_api.cu", "sra_fwd.cu", "sra_bwd.cu", "sra_static.cu"]
 HEADERS = ["ptx.cuh", "sra_common.h", "sra_ctx.h", os.path.join("..", "..", "include", "sra.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC",
