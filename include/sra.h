@@ -166,8 +166,10 @@ typedef struct {
  * enough to cover the upload) attend the resident reference K/V while K_g / V_g are in flight, then the generation
  * keys, and the two fp32 partials (O_s, LSE_s) of each row are merged exactly as in the key-split schedule - so
  * those rows can differ from sra_forward's single-pass result in the last bf16 bit (same tolerance against the
- * oracle; the other slabs and the reference rows are bit-identical).  Needs 2 * B * H * n_gen * (d + 1) * 4 bytes of
- * ctx-owned partial buffers.  The copy streams are ordered after prior work on `cuda_stream`, and `cuda_stream`
+ * oracle; the other slabs and the reference rows are bit-identical).  Copy-bound shapes (the reference-segment work
+ * of six slab groups is shorter than the K_g / V_g upload, by the two measured rates; no temporal window) stream the
+ * generation keys as well: K_g / V_g go up in two key halves, the first slabs attend each half as soon as it has
+ * landed, three partials per row.  Needs 3 * B * H * n_gen * (d + 1) * 4 bytes of ctx-owned partial buffers.  The copy streams are ordered after prior work on `cuda_stream`, and `cuda_stream`
  * waits for the last device->host copy, so the call is still asynchronous on - and ordered by - the caller's stream.
  * The same pipeline runs with batch > 1 (a slab is the same row range of every batch item, copied with one strided
  * copy), under a validity mask (the reference rows are gathered from / scattered into the staged tensors) and under

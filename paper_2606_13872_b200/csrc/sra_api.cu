@@ -642,14 +642,15 @@ int reserve(sra_ctx* ctx, uint32_t what) {
     for (int i = 0; i < 8 && e == cudaSuccess; ++i)
       if (!ctx->stage[i]) e = cudaMalloc(&ctx->stage[i], want[i]);
     // segment partials of the reference-first phase, per batch item
-    const size_t prow = 2 * size_t(c.batch) * c.heads * c.n_gen;
+    const size_t prow = 3 * size_t(c.batch) * c.heads * c.n_gen;  // reference segment + up to two generation-key chunks
     if (e == cudaSuccess && !ctx->ws_seg_o) e = cudaMalloc(&ctx->ws_seg_o, prow * c.head_dim * sizeof(float));
     if (e == cudaSuccess && !ctx->ws_seg_lse) e = cudaMalloc(&ctx->ws_seg_lse, prow * sizeof(float));
+    if (e == cudaSuccess) e = ensure_pair(ctx->d_seg_items, ctx->cap_seg, 3 * size_t(std::max(ctx->n_gen_items, 1)));  // [A ; B_0 ; B_1]
     if (e != cudaSuccess) { (void)cudaGetLastError(); return ctx_fail(ctx, SRA_ERR_OOM, "host staging allocation failed"); }
     if (!ctx->s_h2d) {
       e = cudaStreamCreateWithFlags(&ctx->s_h2d, cudaStreamNonBlocking);
       if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->s_d2h, cudaStreamNonBlocking);
-      ctx->pipe_ev.assign(2 * kChunks + 5, nullptr);
+      ctx->pipe_ev.assign(2 * kChunks + 6, nullptr);
       for (cudaEvent_t& ev : ctx->pipe_ev)
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
       if (e == cudaSuccess) e = cudaEventCreate(&ctx->rate_ev[0]);
@@ -981,7 +982,7 @@ static int forward_core(sra_ctx* ctx, const sra_fwd_args* a, void* cuda_stream) 
     if (pairs) {
       const int G = ctx->n_gen_items;
       auto pi = [&](int idx) {
-        if (seg && idx >= G) return ctx->n_gen_pairs + int(ctx->pair_of_item[idx - G]);
+        if (seg) return (idx / G) * ctx->n_gen_pairs + int(ctx->pair_of_item[idx % G]);  // list [A ; B_0 ; ...] of G slabs each
         if (idx >= G + ctx->n_ref_items) return ctx->pair_stride;  // end of the (padded) reference range
         return int(ctx->pair_of_item[idx]);
       };
@@ -1050,6 +1051,7 @@ static int forward_host_pipelined(sra_ctx* ctx, const sra_fwd_host_args* a, cuda
   // most kChunks - 2.  Both rates are measured: the copy bandwidth when the staging was reserved, the forward rate
   // from the previous call's launches (a first call assumes 1 PFLOP/s).
   int n_first = 0;
+  bool copy_bound = false;  // even kChunks - 2 slabs of reference-segment work do not cover the K_g / V_g upload
   if (ctx->nr > 0 && ctx->n_masks == 1) {
     if (ctx->rate_pending && cudaEventQuery(ctx->rate_ev[1]) == cudaSuccess) {
       float ms = 0.f;
@@ -1059,31 +1061,49 @@ static int forward_host_pipelined(sra_ctx* ctx, const sra_fwd_host_args* a, cuda
     (void)cudaGetLastError();
     const double t_up = 2.0 * double(gen_bytes) / (ctx->h2d_gbs * 1e9);
     const double t_chunk = 4.0 * c.head_dim * double(c.n_gen) * double(ctx->nr) * c.heads * Bn / ctx->fwd_flops_per_s / kChunks;
-    n_first = int(std::min<double>(kChunks - 2, std::ceil(t_up / t_chunk)));
+    const double need = std::ceil(t_up / t_chunk);
+    n_first = int(std::min<double>(kChunks - 2, need));
+    copy_bound = need > kChunks - 2;
   }
   const int G = ctx->n_gen_items;
-  if (n_first > 0 && ctx->seg_dirty) {
-    // (with CTA pairs the two lists are built from the generation PAIR items)
+  // Copy-bound shapes (480p, the training batch: the reference-segment work of the first slabs is shorter than the K_g /
+  // V_g upload) also stream the generation keys: K_g / V_g go up in kc = 2 halves and the first slabs attend half c as
+  // soon as it has landed (B_c items, partial 1 + c), instead of idling until the whole upload is in.
+  const int k_mid = (c.n_gen / kTile / 2) * kTile;
+  const int kc = (n_first > 0 && copy_bound && ctx->window < 0 && k_mid > 0) ? 2 : 1;
+  if (n_first > 0 && (ctx->seg_dirty || ctx->seg_kc != kc)) {
+    // (with CTA pairs the lists are built from the generation PAIR items)
     const std::vector<sra::FwdItem>& src = ctx->use_pairs ? ctx->pair_items : ctx->fwd_items;
     const int Gs = ctx->use_pairs ? ctx->n_gen_pairs : G;
-    std::vector<sra::FwdItem> seg(2 * size_t(Gs));
+    std::vector<sra::FwdItem> seg((1 + size_t(kc)) * Gs);
     for (int g = 0; g < Gs; ++g) {
-      sra::FwdItem A = src[g], Bi = src[g];
+      sra::FwdItem A = src[g];
       A.q_is_ref = 1 << 8; A.seg0_len = 0;                   // partial 0: reference keys only
-      Bi.q_is_ref = 2 << 8; Bi.seg1_len = 0;                 // partial 1: generation keys only
-      seg[g] = A; seg[size_t(Gs) + g] = Bi;
+      seg[g] = A;
+      for (int kp = 0; kp < kc; ++kp) {                      // partial 1 + kp: generation keys (of half kp) only
+        sra::FwdItem Bi = src[g];
+        Bi.q_is_ref = (2 + kp) << 8; Bi.seg1_len = 0;
+        if (kc == 2) {                                       // (no window: seg0 = [0, n_gen))
+          Bi.seg0_start = kp == 0 ? 0 : k_mid;
+          Bi.seg0_len = kp == 0 ? k_mid : c.n_gen - k_mid;
+        }
+        seg[(1 + size_t(kp)) * Gs + g] = Bi;
+      }
     }
-    cudaError_t e = ensure_pair(ctx->d_seg_items, ctx->cap_seg, seg.size());
+    // (sized for the three-list form at once: the measured rates may switch kc between calls, and no call after the
+    //  first may allocate)
+    cudaError_t e = ensure_pair(ctx->d_seg_items, ctx->cap_seg, 3 * size_t(Gs));
     const int nb = ctx->seg_buf ^ 1;
     if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->d_seg_items[nb], seg.data(), seg.size() * sizeof(sra::FwdItem), cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) { (void)cudaGetLastError(); return fail(ctx, SRA_ERR_OOM, "reference-first item list upload failed"); }
     ctx->seg_buf = nb;
     ctx->seg_dirty = false;
+    ctx->seg_kc = kc;
   }
   cudaEvent_t* ev_q = ctx->pipe_ev.data();            // [kChunks] slab c of Q is on the device
   cudaEvent_t* ev_c = ev_q + kChunks;                 // [kChunks] slab c of O is computed
   cudaEvent_t ev_start = ev_c[kChunks], ev_kv = ev_c[kChunks + 1], ev_qr = ev_c[kChunks + 2], ev_cr = ev_c[kChunks + 3],
-              ev_done = ev_c[kChunks + 4];
+              ev_done = ev_c[kChunks + 4], ev_kv0 = ev_c[kChunks + 5];
   char* dq = static_cast<char*>(ctx->stage[0]);
   char* dout = static_cast<char*>(ctx->stage[3]);
   const char* hq = static_cast<const char*>(a->q_gen);
@@ -1123,9 +1143,12 @@ static int forward_host_pipelined(sra_ctx* ctx, const sra_fwd_host_args* a, cuda
     if (e == cudaSuccess) e = cudaEventRecord(ev_q[ch], ctx->s_h2d);
   };
   for (int ch = 0; ch < n_first; ++ch) copy_q(ch);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->stage[1], a->k_gen, gen_bytes, cudaMemcpyHostToDevice, ctx->s_h2d);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->stage[2], a->v_gen, gen_bytes, cudaMemcpyHostToDevice, ctx->s_h2d);
-  if (e == cudaSuccess) e = cudaEventRecord(ev_kv, ctx->s_h2d);
+  for (int kp = 0; kp < kc; ++kp) {  // K_g / V_g, whole or in two key halves (rows [k0, k1) of every batch item)
+    const size_t k0 = kp == 0 ? 0 : size_t(k_mid), k1 = kp == kc - 1 ? size_t(c.n_gen) : size_t(k_mid);
+    if (e == cudaSuccess) e = copy_rows(static_cast<char*>(ctx->stage[1]), static_cast<const char*>(a->k_gen), k0, k1, cudaMemcpyHostToDevice, ctx->s_h2d);
+    if (e == cudaSuccess) e = copy_rows(static_cast<char*>(ctx->stage[2]), static_cast<const char*>(a->v_gen), k0, k1, cudaMemcpyHostToDevice, ctx->s_h2d);
+    if (e == cudaSuccess) e = cudaEventRecord(kp == kc - 1 ? ev_kv : ev_kv0, ctx->s_h2d);
+  }
   for (int ch = n_first; ch < kChunks; ++ch) copy_q(ch);
   if (e == cudaSuccess && with_ref_rows) {
     e = cudaMemcpyAsync(ctx->stage[4], a->q_ref, ref_bytes, cudaMemcpyHostToDevice, ctx->s_h2d);
@@ -1163,7 +1186,7 @@ static int forward_host_pipelined(sra_ctx* ctx, const sra_fwd_host_args* a, cuda
     if (e != cudaSuccess) break;
     if (int rc = launch(true, i0, i1 - i0, d, false)) return rc;
   }
-  if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev_kv, 0);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(st, kc == 2 ? ev_kv0 : ev_kv, 0);
   if (e != cudaSuccess) return fail_cuda(ctx, e, "pipelined host copy");
   auto run_ref_rows = [&]() -> int {
     // reference rows: their q_ref copy has had the first slabs' compute time to land; their output copy is
@@ -1185,14 +1208,20 @@ static int forward_host_pipelined(sra_ctx* ctx, const sra_fwd_host_args* a, cuda
   if (n_first > 0) {
     int i0, i1; size_t r0, r1;
     span(0, n_first, i0, i1, r0, r1);
-    if (int rc = launch(true, G + i0, i1 - i0, d, false)) return rc;
+    for (int kp = 0; kp < kc; ++kp) {
+      if (kp == 1) {  // the second half of K_g / V_g
+        e = cudaStreamWaitEvent(st, ev_kv, 0);
+        if (e != cudaSuccess) return fail_cuda(ctx, e, "pipelined host copy");
+      }
+      if (int rc = launch(true, (1 + kp) * G + i0, i1 - i0, d, false)) return rc;
+    }
     sra::FwdParams mp{};
     mp.part_o = ctx->ws_seg_o; mp.part_lse = ctx->ws_seg_lse;
     mp.o_gen = static_cast<__nv_bfloat16*>(d.o_gen); mp.lse_gen = d.lse_gen;
     mp.batch = Bn; mp.heads = c.heads; mp.n_gen = c.n_gen;
     {
       sra::KernelTimer kt(ctx, SRA_KERNEL_FWD_MERGE, st);
-      e = sra::launch_fwd_merge(mp, c.head_dim, 2, st, ctx->num_sms * 16, int(r0), int(r1 - r0));
+      e = sra::launch_fwd_merge(mp, c.head_dim, 1 + kc, st, ctx->num_sms * 16, int(r0), int(r1 - r0));
     }
     if (e != cudaSuccess) return fail_cuda(ctx, e, "sra_fwd_merge_kernel launch");
     if (r1 > r0) ctx->launches += 1;

@@ -96,8 +96,9 @@ struct sra_ctx {
   sra::FwdItem* d_seg_items[2] = {nullptr, nullptr};  // [2 * n_gen_items] (with use_pairs: [2 * n_gen_pairs] pair items): A items, then B items
   size_t cap_seg = 0;
   bool seg_dirty = true;
-  float* ws_seg_o = nullptr;            // fp32 [2][B][H][n_gen][d]
-  float* ws_seg_lse = nullptr;          // fp32 [2][B][H][n_gen]
+  int seg_kc = 1;                       // generation-key chunks of the B items in the device list ([A ; B_0 ; ... ; B_kc-1])
+  float* ws_seg_o = nullptr;            // fp32 [3][B][H][n_gen][d]  (A, B_0, B_1)
+  float* ws_seg_lse = nullptr;          // fp32 [3][B][H][n_gen]
   bool sub_seg = false;
   // encoded tensor maps, keyed by what they describe (cuTensorMapEncodeTiled is ~1 us of host time each)
   struct TmapEntry {
