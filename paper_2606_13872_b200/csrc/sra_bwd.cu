@@ -10,18 +10,18 @@
 //         dV  += P^T dO_i       [keys x d]         A = P^T (bf16) from TMEM, written over S^T
 //         dQ_i^T = K^T dS^T     [d x queries]      A = K (MN-major), B = dS^T (MN-major) -> TMEM dPdQ (over dP^T)
 //         dK  += dS^T Q_i       [keys x d]         A = dS^T (bf16) from shared memory
-//       Thread = key = TMEM lane for the elementwise math.  Eight compute warps (two per SM sub-partition: warp w
-//       and w + 4 own the same 32 keys and split the 128 query columns in halves) form P^T = exp2(S^T * scale*log2e
-//       - LSE*log2e), keep it in registers, and then dS^T = P^T o (dP^T - D) of the same tile.  dQ_i^T is drained by a
-//       fourth warpgroup (thread = d = TMEM lane) straight from registers into the fp32 workspace [B*H][n_pad][d]
-//       with coalesced red.global.add.f32 (many key tiles add into the same query rows; the summation order is not
-//       deterministic - SURVEY.md 8c A13).
+//       Thread = key = TMEM lane for the elementwise math.  The compute warps (one per SM sub-partition; two with
+//       SRA_BWD_SPLIT = 2) form P^T = exp2(S^T * scale*log2e - LSE*log2e), keep it in registers, and then dS^T = P^T o
+//       (dP^T - D) of the same tile.  dQ_i^T is drained by another warpgroup (thread = d = TMEM lane): registers ->
+//       a shared-memory staging buffer [query][d] -> cp.reduce.async.bulk .add.f32 into the fp32 workspace
+//       [B*H][n_pad][d] (many key tiles add into the same query rows; the summation order is not deterministic -
+//       SURVEY.md 8c A13).
 //       TMEM is exactly full at d = 128 (S 128 | dPdQ 128 | dV 128 | dK 128 columns), so nothing is double-buffered
 //       there; the issue order  dV(i), S^T(i+1), dQ^T(i), dK(i), dP^T(i+1)  gives every elementwise stage the
 //       shadow of at least one other tile-sized MMA: exp(i+1) runs under dQ^T(i), dK(i), dP^T(i+1); dS(i+1) under
-//       dV(i+1), S^T(i+2); the dQ^T(i) drain under dK(i).  Shared memory (224 KB at d = 128): K, V, dS^T, a 3-stage
+//       dV(i+1), S^T(i+2); the dQ^T(i) drain under dK(i).  Shared memory (226 KB at d = 128): K, V, dS^T, a 2-stage
 //       Q ring (Q_i is read first by S^T(i) and last by dK(i)), one dO buffer (read by dP^T(i) and dV(i), both early
-//       in a tile) and two slots of {LSE_i log2e, D_i}.
+//       in a tile), two slots of {LSE_i log2e, D_i} and 32 KB of dQ staging.
 //   a8  sra_bwd_dq_finalize_kernel  workspace * scale -> bf16 dQ [B, N, H, d]
 #include <type_traits>
 
@@ -42,6 +42,17 @@ __device__ long long* g_bwd_trace = nullptr;
 #define TR(role, ev) do { } while (0)
 #endif
 
+// dQ^T leaves the SM through a shared-memory staging buffer and cp.reduce.async.bulk (1, the default), or as per-thread
+// red.global.add.f32 straight from registers (0: the round-1 / early round-2 form, kept for A/B).
+#ifndef SRA_BWD_BULK
+#define SRA_BWD_BULK 1
+#endif
+#ifndef SRA_BWD_BULK_NQ
+#define SRA_BWD_BULK_NQ 4  // pieces per 128-query tile
+#endif
+#ifndef SRA_BWD_BULK_NB
+#define SRA_BWD_BULK_NB 2  // staging buffers
+#endif
 #ifndef SRA_BWD_RED_GAP
 #define SRA_BWD_RED_GAP 28  // cycles per dQ reduction instruction of a drain warp (0 = unpaced)
 #endif
@@ -61,12 +72,18 @@ struct BwdCfg {
   static constexpr int kKBytes = kTile * D * 2;         // K or V tile
   static constexpr int kQBytes = kQT * D * 2;           // Q_i or dO_i tile
   static constexpr int kBoxBytes = kTile * 128;         // one 64-column (128 B) box of a 128-row tile
-  static constexpr int kQStages = 3;                    // Q_i ring
+#if SRA_BWD_BULK
+  static constexpr int kQStages = 2;                    // Q_i ring (Q_i is read first by S^T(i), last by dK(i))
+  static constexpr int kStageBytes = SRA_BWD_BULK_NB * (kBwdQTile / SRA_BWD_BULK_NQ) * D * 4;  // dQ staging: kNB x [kRP queries][D] fp32
+#else
+  static constexpr int kQStages = 3;
+  static constexpr int kStageBytes = 0;
+#endif
   static constexpr int kVecSlots = 2;                   // {-LSE_i log2e [128], D_i [128]} ring
   static constexpr int kDsBytes = kTile * kQT * 2;      // dS^T tile: 2 boxes of [128 keys][64 queries] bf16
   static constexpr int kVecBytes = kVecSlots * 2 * kQT * 4;
   static constexpr int kNumBars = 1 + 2 * kQStages + 2 + 2 * kVecSlots + 8;
-  static constexpr int kSmemBytes = 2 * kKBytes + (kQStages + 1) * kQBytes + kDsBytes + kVecBytes + kNumBars * 8 + 16;
+  static constexpr int kSmemBytes = 2 * kKBytes + (kQStages + 1) * kQBytes + kDsBytes + kVecBytes + kNumBars * 8 + 16 + kStageBytes + (kStageBytes ? 128 : 0);
   // kSplit compute warps per SM sub-partition share a key row's 128 query columns.  Warps [0, 4 kSplit): compute (P^T,
   // dS^T; dV epilogue) | next 4: dQ^T drain (dK epilogue) | then the MMA issuer, the loader and 2 idle warps (the register
   // file is allocated per 4 warps).  A drain thread holds a whole 128-column row of dQ^T, so that the TMEM columns are
@@ -152,6 +169,7 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
   const uint32_t bar_dq_empty = bar_dq_full + 8;                // 4 drain warps
   const uint32_t bar_acc_full = bar_dq_empty + 8;
   const uint32_t s_tmem_ptr = bar_acc_full + 16;
+  const uint32_t sStage = (s_tmem_ptr + 16 + 127) & ~127u;      // (SRA_BWD_BULK) dQ staging: [64 queries][D] fp32
   uint32_t* tmem_ptr_generic = reinterpret_cast<uint32_t*>(smem_raw + (s_tmem_ptr - smem_base));
 
   const int warp = threadIdx.x >> 5;
@@ -373,12 +391,9 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
       mbar_wait(bar_dq_full, it & 1);
       if (wq == 0) TR(3, 1);
       tc_fence_after();
-      // dQ_it^T leaves the SM straight from registers: for a fixed query the 32 lanes of a warp hold 32 consecutive d,
-      // so each red.global.add.f32 is one coalesced 128-byte reduction into the fp32 workspace.  All 128 columns are
-      // taken into registers first, so that the TMEM columns are released (dq_empty) before the first reduction - the
-      // reductions run at the LSU -> L2 rate, far longer than dP^T(it+1) may wait.
+      // All 128 columns of dQ_it^T are taken into registers first, so that the TMEM columns are released (dq_empty)
+      // before the first reduction - the reductions run at the L2's rate, far longer than dP^T(it+1) may wait.
       const int drow = key;
-      float* dq_row = p.dq_ws + (size_t(bh) * p.n_pad + qt.cat0) * D + drow;
       uint32_t r[4][32];
 #pragma unroll
       for (int x = 0; x < 4; ++x) tmem_ld32(tmem + lane_off + C::kColDP + x * 32, r[x]);
@@ -387,6 +402,41 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
       __syncwarp();
       if (lane == 0) mbar_arrive(bar_dq_empty);  // dQ^T(it) is in registers: the columns are free for dP^T(it+1)
       if (wq == 0) TR(3, 2);
+#if SRA_BWD_BULK
+      // dQ_it leaves as kNQ bulk reductions of 128 / kNQ query rows each: registers -> shared-memory staging [query][d]
+      // (thread = d, so the 32 lanes of a store hit 32 consecutive words: conflict-free) -> cp.reduce.async.bulk .add.f32
+      // into the workspace rows of the tile, which are contiguous.  The reductions go through the TMA unit, not through the
+      // memory-instruction queue the compute warps' tcgen05.ld / st and shared-memory stores need (per-thread
+      // red.global.add.f32 had to be paced to 18 B/clk/SM for that reason; the L2 takes 23-24 from either source).  kNB
+      // staging buffers: the stores of piece q overlap the bulk reads of the pieces before it; a buffer is rewritten once
+      // the reduction issued kNB pieces earlier has read it.  (Many key tiles add into the same rows: the summation
+      // order is not deterministic - SURVEY.md 8c A13.)
+      constexpr int kNQ = SRA_BWD_BULK_NQ, kNB = SRA_BWD_BULK_NB, kRP = QT / kNQ;
+      static_assert(kNB * kRP * D * 4 <= C::kStageBytes, "staging budget");
+#pragma unroll
+      for (int qr = 0; qr < kNQ; ++qr) {
+        const uint32_t stg = sStage + (qr % kNB) * (kRP * D * 4);
+        if (wq == 0 && lane == 0) tma_wait_group_read<kNB - 1>();
+        named_bar_sync(1, 128);
+        if (drow < D) {
+#pragma unroll
+          for (int cc = 0; cc < kRP; ++cc) {
+            const int col = qr * kRP + cc;
+            st_shared_f32(stg + (cc * D + drow) * 4, __uint_as_float(r[col >> 5][col & 31]));
+          }
+        }
+        fence_proxy_async_smem();
+        named_bar_sync(1, 128);
+        if (wq == 0 && lane == 0) {
+          const int rows = min(kRP, qt.valid - qr * kRP);
+          if (rows > 0) bulk_reduce_add_f32(p.dq_ws + (size_t(bh) * p.n_pad + qt.cat0 + qr * kRP) * D, stg, uint32_t(rows) * D * 4);
+          tma_commit_group();
+        }
+      }
+#else
+      // (A/B form: dQ_it^T straight from registers - for a fixed query the 32 lanes of a warp hold 32 consecutive d, so each
+      //  red.global.add.f32 is one coalesced 128-byte reduction)
+      float* dq_row = p.dq_ws + (size_t(bh) * p.n_pad + qt.cat0) * D + drow;
       if (drow < D) {
         if (qt.valid == QT) {
           // The reductions share each sub-partition's memory-instruction queue with the compute warp's tcgen05.ld / st and
@@ -415,8 +465,12 @@ __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
               if (x * 32 + c < qt.valid) red_add_f32(dq_row + (x * 32 + c) * D, __uint_as_float(r[x][c]));
         }
       }
+#endif
       if (wq == 0) TR(3, 3);
     }
+#if SRA_BWD_BULK
+    if (wq == 0 && lane == 0) tma_wait_group<0>();
+#endif
     // ---------------------------------------------------- epilogue: dK = scale * acc (lanes = keys)
     mbar_wait(bar_acc_full, 0);
     tc_fence_after();
