@@ -198,7 +198,8 @@ typedef struct {
  * mask): D = rowsum(dO o O); P = exp(sQK^T - LSE); dV = P^T dO; dP = dO V^T;
  * dS = P o (dP - D); dQ = s dS K; dK = s dS^T Q.  dK_r/dV_r receive contributions from all G
  * rows and from the R rows of the same block.  head_dim 64 and 128.  dQ is accumulated in a ctx-owned fp32 workspace
- * with red.global.add (the order of the additions is not fixed: results can differ in the last bit between runs). */
+ * with fp32 reductions in L2 (cp.reduce.async.bulk; the order of the additions is not fixed: results can differ in
+ * the last bit between runs). */
 int sra_backward(sra_ctx* ctx, const sra_bwd_args* args, void* cuda_stream);
 
 /* Frees the cache, workspace and schedule.  NULL-safe. */
